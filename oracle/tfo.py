@@ -1,0 +1,146 @@
+"""ctypes binding of the CPU oracle (oracle/tfo.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this module.  It imports nothing from the CUDA package.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tfo.c")
+OK, NOT_CONVERGED = 0, 1
+
+
+def build(force=False):
+    """Compile tfo.c with gcc: libtfo.so (serial) and libtfo_omp.so (-fopenmp)."""
+    outs = []
+    for name, extra in (("libtfo.so", []), ("libtfo_omp.so", ["-fopenmp"])):
+        out = os.path.join(_HERE, name)
+        if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(_SRC):
+            subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-std=c11", "-fPIC", "-shared",
+                                   *extra, "-o", out, _SRC, "-lm"])
+        outs.append(out)
+    return outs
+
+
+_libs = {}
+_dp = ctypes.POINTER(ctypes.c_double)
+
+
+def lib(omp=False):
+    key = bool(omp)
+    if key not in _libs:
+        build()
+        L = ctypes.CDLL(os.path.join(_HERE, "libtfo_omp.so" if omp else "libtfo.so"))
+        L.tfo_create.argtypes = [ctypes.POINTER(ctypes.c_void_p), ctypes.c_int, ctypes.c_int, ctypes.c_double,
+                                 ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
+                                 ctypes.c_int]
+        L.tfo_set_model_linear.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_double]
+        L.tfo_set_newton.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_int, ctypes.c_int]
+        L.tfo_set_state.argtypes = [ctypes.c_void_p, _dp]
+        L.tfo_get_state.argtypes = [ctypes.c_void_p, _dp]
+        L.tfo_step.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.POINTER(ctypes.c_int), _dp]
+        L.tfo_mass.argtypes = [ctypes.c_void_p, _dp]
+        L.tfo_destroy.argtypes = [ctypes.c_void_p]
+        L.tfo_destroy.restype = None
+        L.tfo_operator_D.argtypes = [ctypes.c_void_p, _dp, _dp]
+        L.tfo_jacobian_bands.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, _dp, _dp, _dp, _dp, _dp]
+        L.tfo_directional_solve.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double, _dp, _dp, _dp]
+        L.tfo_penta_solve.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int] + [_dp] * 7
+        _libs[key] = L
+    return _libs[key]
+
+
+def _p(a):
+    assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data_as(_dp)
+
+
+class OracleError(RuntimeError):
+    pass
+
+
+def _chk(rc, what):
+    if rc < 0:
+        raise OracleError(f"{what} failed with status {rc}")
+    return rc
+
+
+class ThinFilmOracle:
+    """Same call names as the CUDA binding (create/set_newton/set_state/step/get_state/mass)."""
+
+    def __init__(self, nx, ny, dx, dy, kappa=100.0, hstar=0.1, n=3, m=2, bc=0, omp=False):
+        self.L = lib(omp)
+        self.nx, self.ny = nx, ny
+        self._h = ctypes.c_void_p()
+        _chk(self.L.tfo_create(ctypes.byref(self._h), nx, ny, dx, dy, kappa, hstar, n, m, bc), "tfo_create")
+
+    def close(self):
+        if self._h:
+            self.L.tfo_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    __del__ = close
+
+    def set_model_linear(self, c0, c1):
+        _chk(self.L.tfo_set_model_linear(self._h, c0, c1), "tfo_set_model_linear")
+
+    def set_newton(self, tol=1e-10, max_iter=10, fixed_iters=0):
+        _chk(self.L.tfo_set_newton(self._h, tol, max_iter, fixed_iters), "tfo_set_newton")
+
+    def set_state(self, h):
+        h = np.ascontiguousarray(h, dtype=np.float64)
+        assert h.shape == (self.ny, self.nx)
+        _chk(self.L.tfo_set_state(self._h, _p(h)), "tfo_set_state")
+
+    def get_state(self):
+        out = np.empty((self.ny, self.nx))
+        _chk(self.L.tfo_get_state(self._h, _p(out)), "tfo_get_state")
+        return out
+
+    def step(self, dt):
+        """Returns (status, newton_iters, residual); status 0 = accepted, 1 = rejected (state unchanged)."""
+        it, res = ctypes.c_int(0), ctypes.c_double(0.0)
+        rc = _chk(self.L.tfo_step(self._h, dt, ctypes.byref(it), ctypes.byref(res)), "tfo_step")
+        return rc, it.value, res.value
+
+    def mass(self):
+        m = ctypes.c_double(0.0)
+        _chk(self.L.tfo_mass(self._h, ctypes.byref(m)), "tfo_mass")
+        return m.value
+
+    # pieces for pins / per-kernel parity
+    def operator_D(self, h):
+        h = np.ascontiguousarray(h, dtype=np.float64)
+        D = np.empty_like(h)
+        _chk(self.L.tfo_operator_D(self._h, _p(h), _p(D)), "tfo_operator_D")
+        return D
+
+    def jacobian_bands(self, direction, h):
+        h = np.ascontiguousarray(h, dtype=np.float64)
+        out = [np.zeros_like(h) for _ in range(5)]
+        _chk(self.L.tfo_jacobian_bands(self._h, direction, _p(h), *[_p(o) for o in out]), "tfo_jacobian_bands")
+        return out
+
+    def directional_solve(self, direction, s, uk, rhs):
+        uk = np.ascontiguousarray(uk, dtype=np.float64)
+        rhs = np.ascontiguousarray(rhs, dtype=np.float64)
+        out = np.empty_like(uk)
+        _chk(self.L.tfo_directional_solve(self._h, direction, s, _p(uk), _p(rhs), _p(out)), "tfo_directional_solve")
+        return out
+
+
+def penta_solve(direction, e, c, d, a, b, rhs, omp=False):
+    """Batched pentadiagonal solve on [nrow][ncol] arrays; direction 0: rows are systems, 1: columns."""
+    arrs = [np.ascontiguousarray(t, dtype=np.float64) for t in (e, c, d, a, b, rhs)]
+    nrow, ncol = arrs[0].shape
+    x = np.zeros_like(arrs[0])
+    _chk(lib(omp).tfo_penta_solve(nrow, ncol, direction, *[_p(t) for t in arrs], _p(x)), "tfo_penta_solve")
+    return x
+
+
+def num_threads(omp=False):
+    return int(lib(omp).tfo_num_threads())
