@@ -1,0 +1,121 @@
+/*
+ * tf.h -- C-ABI of the B200-native ADI sweep for the thin-film equation
+ *
+ *     h_t + div[ h^3 grad( lap h + Pi(h) ) ] = 0,   Pi(h) = kappa[(hstar/h)^n - (hstar/h)^m]
+ *
+ * i.e. eq (1.1)/(2.1) of Lam, Cummings, Kondic (arXiv:1806.10550) with
+ * f0 = h^3, f1 = h^3 Pi'(h) (eqs (1.7)-(1.8)), no-flux boundaries (2.28)
+ * (PAPER.md:297-302), Crank-Nicolson in time (2.14), solved by the ADI
+ * pseudo-Newton iteration (2.19)-(2.21).  All arithmetic is fp64 and runs
+ * in hand-written sm_100a CUDA kernels; there is NO CPU fallback: every entry point that
+ * needs the GPU returns TF_ERR_CUDA when no device / kernel image is usable.
+ *
+ * Layout: a field is nx*ny doubles, row-major h[j*nx + i], i along x (contiguous), j along y;
+ * cell centre ((i+1/2)dx, (j+1/2)dy).
+ * Ownership: the context owns its device buffers (tf_create) or borrows the caller's
+ * workspace for its lifetime (tf_create_with_workspace).  No pointer passed to any other
+ * call is retained after the call returns.
+ * Errors: every call returns a tf_status; nothing throws or aborts across this boundary.
+ * CUDA errors map to TF_ERR_CUDA with text in tf_last_error().
+ * Threading: one context is used from one host thread at a time; all work of a context is
+ * ordered on its stream.
+ */
+#ifndef TF_B200_H
+#define TF_B200_H
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tf_ctx tf_ctx;   /* opaque */
+
+typedef enum {
+    TF_OK = 0,
+    TF_NOT_CONVERGED = 1,       /* soft: step rejected, state still u^n   */
+    TF_ERR_INVALID_ARG = -1,
+    TF_ERR_UNSUPPORTED = -2,
+    TF_ERR_CUDA = -3,
+    TF_ERR_ALLOC = -4,
+    TF_ERR_STATE = -5
+} tf_status;
+
+typedef enum { TF_BC_NOFLUX = 0 } tf_bc;   /* (2.28): h_n = h_nnn = 0 on all four sides */
+
+/* Bytes of device workspace a context for an nx*ny grid needs (so the caller, e.g. PyTorch,
+ * can allocate it).  0 if nx or ny < 5. */
+size_t tf_workspace_bytes(int nx, int ny);
+
+/*
+ * Create a context (problem statement: PAPER.md:47 (1.1), 86-91 (1.7)-(1.8), 297-302 (2.28)).
+ *   nx, ny >= 5; dx, dy, kappa, hstar > 0; integer exponents n > m >= 1; bc = TF_BC_NOFLUX
+ *   (anything else: TF_ERR_UNSUPPORTED -- the paper defines no other boundary condition).
+ * tf_create allocates tf_workspace_bytes() of device memory itself and uses the legacy
+ * default stream.  tf_create_with_workspace borrows `dev_ws` (device pointer, 256-byte
+ * aligned, `bytes` >= tf_workspace_bytes) and launches on `cuda_stream` (a cudaStream_t
+ * cast to void*; NULL = default stream).
+ */
+tf_status tf_create(tf_ctx** out, int nx, int ny, double dx, double dy,
+                    double kappa, double hstar, int n, int m, tf_bc bc);
+tf_status tf_create_with_workspace(tf_ctx** out, int nx, int ny, double dx, double dy,
+                                   double kappa, double hstar, int n, int m, tf_bc bc,
+                                   void* dev_ws, size_t bytes, void* cuda_stream);
+void tf_destroy(tf_ctx* ctx);
+
+/* Newton controls, (2.22) and Notes 1-2.  Defaults: tol = 1e-10,
+ * max_iter = 10, fixed_iters = 0 (off).  tol >= 1e-14;
+ * 1 <= max_iter <= 4096; 0 <= fixed_iters <= 4096.  fixed_iters = K > 0: exactly K
+ * iterations per step and the step is always accepted (parity mode). */
+tf_status tf_set_newton(tf_ctx* ctx, double tol, int max_iter, int fixed_iters);
+
+/* Copy nx*ny doubles into the context as u^n.  `h` is a device pointer if is_device_ptr != 0,
+ * else a host pointer.  Rejects non-finite or non-positive values (Pi is singular at h = 0)
+ * with TF_ERR_INVALID_ARG; the previous state is then kept. */
+tf_status tf_set_state(tf_ctx* ctx, const double* h, int is_device_ptr);
+
+/* Copy the current state u^n out (nx*ny doubles, same layout). */
+tf_status tf_get_state(tf_ctx* ctx, double* h_out, int is_device_ptr);
+
+/*
+ * One Crank-Nicolson time step of size dt > 0 by the ADI pseudo-Newton iteration:
+ *   b^n = u^n - (dt/2) D(u^n);  u_(0) = u^n;  for k = 0, 1, ...:
+ *     (I + dt/2 J_y(u_k)) w = b^n - u_k - (dt/2) D(u_k)          (2.19)  y-sweep
+ *     (I + dt/2 J_x(u_k)) v = w                                  (2.20)  x-sweep
+ *     res = max |v / u_k|;  u_(k+1) = u_k + v                    (2.22), (2.21)
+ * until res < tol (TF_OK, state advanced) or max_iter iterations were done or an iterate
+ * became non-finite / non-positive (TF_NOT_CONVERGED, state unchanged).  *newton_iters
+ * (>= 1) and *residual (last res) are filled in both cases; either may be NULL.
+ */
+tf_status tf_step(tf_ctx* ctx, double dt, int* newton_iters, double* residual);
+
+/* mass = dx*dy*sum(h)  ((3.2), times the domain area); fixed-order fp64 tree. */
+tf_status tf_mass(tf_ctx* ctx, double* mass);
+
+/*
+ * Isolated batched pentadiagonal solve (LU without pivoting, (A.5)).
+ * Seven DEVICE arrays, each nrow*ncol doubles, row-major [r*ncol + c]; row i of a system is
+ *   e_i x_{i-2} + c_i x_{i-1} + d_i x_i + a_i x_{i+1} + b_i x_{i+2} = rhs_i,
+ * band entries that fall outside a system are ignored.
+ *   dir = 0: system s = row s    (contiguous; nsys = nrow, len = ncol)   -- the x-sweep shape
+ *   dir = 1: system s = column s (strided;   nsys = ncol, len = nrow)   -- the y-sweep shape
+ * dev_ws: device scratch of tf_penta_workspace_bytes(nrow, ncol) bytes.  x may not alias inputs.
+ * len >= 3.  Runs on cuda_stream; returns after enqueueing (no host sync).
+ */
+size_t    tf_penta_workspace_bytes(int nrow, int ncol);
+tf_status tf_penta_solve(int nrow, int ncol, int dir,
+                         const double* e, const double* c, const double* d,
+                         const double* a, const double* b, const double* rhs, double* x,
+                         void* dev_ws, void* cuda_stream);
+
+/* Text of the last error on this context ("" if none); ctx == NULL: last error of a failed
+ * tf_create* / tf_penta_solve on this thread.  Valid until the next call. */
+const char* tf_last_error(const tf_ctx* ctx);
+
+/* Number of kernels this library has launched since load (all contexts); for bench.py's
+ * gpu_launches claim. */
+unsigned long long tf_kernel_launches(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TF_B200_H */

@@ -1,0 +1,333 @@
+// tf_b200.cu -- C-ABI (include/tf.h) and host step driver of the B200 thin-film ADI sweep.
+// Host side only orders kernels on one stream and reads one 16-byte residual record per Newton
+// iteration (the paper reads IJ/256 flag bytes per iteration; S8 of DESIGN.md).
+#include "../../include/tf.h"
+#include "tf_penta.cuh"
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+namespace {
+
+using namespace tf;
+
+constexpr int MAX_ITERS = 4096;
+constexpr size_t ALIGN = 256;
+
+std::atomic<unsigned long long> g_launches{0};
+thread_local std::string g_err;
+
+size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+size_t field_bytes(int nx, int ny) { return align_up((size_t)nx * ny * sizeof(double)); }
+size_t scratch_bytes() { return align_up(sizeof(double) * (2 * (MAX_ITERS + 1) + RED_BLOCKS + 8)); }
+constexpr int NFIELDS = 7;   // u, uk, bn, w, alpha, beta, z
+
+}  // namespace
+
+struct tf_ctx {
+    Params P;
+    double kappa, hstar;
+    double tol;
+    int max_iter, fixed_iters;
+    bool have_state, owns_ws;
+    cudaStream_t stream;
+    char* ws;
+    double *u, *uk, *bn, *w, *al, *be, *zz;    // fields
+    double *red;                               // [2*(MAX_ITERS+1)] residual / bad flag per iteration
+    double *part;                              // [RED_BLOCKS]
+    double *scal;                              // [8] : scal[0] mass, (int*)(scal+1) flag
+    double *pinned;                            // [4] host pinned readback
+    std::string err;
+};
+
+namespace {
+
+tf_status fail(tf_ctx* c, tf_status st, const std::string& msg)
+{
+    if (c) c->err = msg; else g_err = msg;
+    return st;
+}
+
+tf_status cuda_fail(tf_ctx* c, cudaError_t e, const char* what)
+{
+    return fail(c, TF_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define TF_CUDA(c, call)                                              \
+    do {                                                              \
+        cudaError_t e__ = (call);                                     \
+        if (e__ != cudaSuccess) return cuda_fail((c), e__, #call);    \
+    } while (0)
+
+inline void count_launch(int n = 1) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
+
+Dir make_dir(double s, double d) { Dir D; D.ca = s / (2.0 * d * d * d * d); D.cb = s / (2.0 * d * d); return D; }
+
+// one pseudo-Newton iteration k: reads src (u^n if k == 0 else uk), writes uk, red[2k..2k+1]
+template <int N, int M>
+cudaError_t launch_iteration(tf_ctx* c, double s, int k)
+{
+    const Params& P = c->P;
+    const Dir DX = make_dir(s, P.dx), DY = make_dir(s, P.dy);
+    const double* src = (k == 0) ? c->u : c->uk;
+    const int gy = (P.nx + YF_VALID - 1) / YF_VALID;
+    if (k == 0)
+        yfwd_kernel<N, M, true><<<gy, 32, 0, c->stream>>>(P, DX, DY, src, c->bn, c->al, c->be, c->zz);
+    else
+        yfwd_kernel<N, M, false><<<gy, 32, 0, c->stream>>>(P, DX, DY, src, c->bn, c->al, c->be, c->zz);
+    ybwd_kernel<<<(P.nx + 31) / 32, 32, 0, c->stream>>>(P.nx, P.ny, c->al, c->be, c->zz, c->w);
+    const int gx = (P.ny + XT - 1) / XT;
+    xfwd_kernel<N, M><<<gx, 32, 0, c->stream>>>(P, DX, src, c->w, c->al, c->be, c->zz);
+    xbwd_kernel<<<gx, 32, 0, c->stream>>>(P.nx, P.ny, c->al, c->be, c->zz, src, c->uk, c->red + 2 * k);
+    count_launch(4);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_iteration(tf_ctx* c, double s, int k)
+{
+    if (c->P.n == 3 && c->P.m == 2) return launch_iteration<3, 2>(c, s, k);
+    return launch_iteration<0, 0>(c, s, k);
+}
+
+tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, double kappa, double hstar,
+                        int n, int m, tf_bc bc, void* dev_ws, size_t bytes, void* stream, bool own)
+{
+    if (!out) return fail(nullptr, TF_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (nx < 5 || ny < 5) return fail(nullptr, TF_ERR_INVALID_ARG, "nx, ny must be >= 5");
+    if (!(dx > 0) || !(dy > 0) || !(kappa > 0) || !(hstar > 0) || !std::isfinite(dx) || !std::isfinite(dy) ||
+        !std::isfinite(kappa) || !std::isfinite(hstar))
+        return fail(nullptr, TF_ERR_INVALID_ARG, "dx, dy, kappa, hstar must be positive and finite");
+    if (m < 1 || n <= m || n > 16) return fail(nullptr, TF_ERR_INVALID_ARG, "exponents must satisfy 16 >= n > m >= 1");
+    if (bc != TF_BC_NOFLUX) return fail(nullptr, TF_ERR_UNSUPPORTED, "only TF_BC_NOFLUX (2.28) is defined");
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0)
+        return fail(nullptr, TF_ERR_CUDA, std::string("no CUDA device: ") + cudaGetErrorString(e));
+    tf_ctx* c = new (std::nothrow) tf_ctx();
+    if (!c) return fail(nullptr, TF_ERR_ALLOC, "host allocation failed");
+    Params& P = c->P;
+    P.nx = nx; P.ny = ny; P.dx = dx; P.dy = dy;
+    P.rdx2 = 1.0 / (dx * dx); P.rdy2 = 1.0 / (dy * dy);
+    P.n = n; P.m = m;
+    double hm = 1.0, hn = 1.0;
+    for (int k = 0; k < m; ++k) hm *= hstar;
+    for (int k = 0; k < n; ++k) hn *= hstar;
+    P.cm = kappa * m * hm; P.cn = kappa * n * hn;
+    c->kappa = kappa; c->hstar = hstar;
+    c->tol = 1e-10; c->max_iter = 10; c->fixed_iters = 0;
+    c->have_state = false; c->owns_ws = own;
+    c->stream = (cudaStream_t)stream;
+    const size_t need = tf_workspace_bytes(nx, ny);
+    if (own) {
+        void* p = nullptr;
+        e = cudaMalloc(&p, need);
+        if (e != cudaSuccess) { delete c; return fail(nullptr, TF_ERR_ALLOC, std::string("cudaMalloc: ") + cudaGetErrorString(e)); }
+        c->ws = (char*)p;
+    } else {
+        if (!dev_ws || bytes < need || ((uintptr_t)dev_ws % ALIGN) != 0) {
+            delete c;
+            return fail(nullptr, TF_ERR_INVALID_ARG, "workspace NULL, misaligned (256 B) or smaller than tf_workspace_bytes");
+        }
+        c->ws = (char*)dev_ws;
+    }
+    const size_t fb = field_bytes(nx, ny);
+    double** f[NFIELDS] = {&c->u, &c->uk, &c->bn, &c->w, &c->al, &c->be, &c->zz};
+    for (int k = 0; k < NFIELDS; ++k) *f[k] = (double*)(c->ws + (size_t)k * fb);
+    char* sc = c->ws + (size_t)NFIELDS * fb;
+    c->red = (double*)sc;
+    c->part = c->red + 2 * (MAX_ITERS + 1);
+    c->scal = c->part + RED_BLOCKS;
+    e = cudaMallocHost((void**)&c->pinned, 4 * sizeof(double));
+    if (e != cudaSuccess) {
+        if (own) cudaFree(c->ws);
+        delete c;
+        return fail(nullptr, TF_ERR_ALLOC, std::string("cudaMallocHost: ") + cudaGetErrorString(e));
+    }
+    *out = c;
+    return TF_OK;
+}
+
+// sum + validity of a field on the context's stream; host gets (scale*sum, flag)
+tf_status reduce_field(tf_ctx* c, const double* dev_field, double scale, double* sum, int* flag)
+{
+    const size_t n = (size_t)c->P.nx * c->P.ny;
+    int* dflag = (int*)(c->scal + 1);
+    TF_CUDA(c, cudaMemsetAsync(dflag, 0, sizeof(int), c->stream));
+    sum_check_kernel<<<RED_BLOCKS, RED_THREADS, 0, c->stream>>>(n, dev_field, c->part, dflag);
+    sum_final_kernel<<<1, 1024, 0, c->stream>>>(c->part, scale, c->scal);
+    count_launch(2);
+    TF_CUDA(c, cudaGetLastError());
+    TF_CUDA(c, cudaMemcpyAsync(c->pinned, c->scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    TF_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (sum) *sum = c->pinned[0];
+    if (flag) std::memcpy(flag, &c->pinned[1], sizeof(int));
+    return TF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t tf_workspace_bytes(int nx, int ny)
+{
+    if (nx < 5 || ny < 5) return 0;
+    return (size_t)NFIELDS * field_bytes(nx, ny) + scratch_bytes();
+}
+
+tf_status tf_create(tf_ctx** out, int nx, int ny, double dx, double dy, double kappa, double hstar, int n, int m,
+                    tf_bc bc)
+{
+    return create_common(out, nx, ny, dx, dy, kappa, hstar, n, m, bc, nullptr, 0, nullptr, true);
+}
+
+tf_status tf_create_with_workspace(tf_ctx** out, int nx, int ny, double dx, double dy, double kappa, double hstar,
+                                   int n, int m, tf_bc bc, void* dev_ws, size_t bytes, void* cuda_stream)
+{
+    return create_common(out, nx, ny, dx, dy, kappa, hstar, n, m, bc, dev_ws, bytes, cuda_stream, false);
+}
+
+void tf_destroy(tf_ctx* c)
+{
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    if (c->owns_ws) cudaFree(c->ws);
+    cudaFreeHost(c->pinned);
+    delete c;
+}
+
+tf_status tf_set_newton(tf_ctx* c, double tol, int max_iter, int fixed_iters)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    if (!(tol >= 1e-14) || !std::isfinite(tol)) return fail(c, TF_ERR_INVALID_ARG, "tol must be >= 1e-14 (PAPER.md:338)");
+    if (max_iter < 1 || max_iter > MAX_ITERS || fixed_iters < 0 || fixed_iters > MAX_ITERS)
+        return fail(c, TF_ERR_INVALID_ARG, "max_iter in [1,4096], fixed_iters in [0,4096]");
+    c->tol = tol; c->max_iter = max_iter; c->fixed_iters = fixed_iters;
+    return TF_OK;
+}
+
+tf_status tf_set_state(tf_ctx* c, const double* h, int is_device_ptr)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    if (!h) return fail(c, TF_ERR_INVALID_ARG, "h is NULL");
+    const size_t bytes = (size_t)c->P.nx * c->P.ny * sizeof(double);
+    // stage in uk, validate on the device, then swap in (the previous state survives a rejection)
+    TF_CUDA(c, cudaMemcpyAsync(c->uk, h, bytes, is_device_ptr ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
+                               c->stream));
+    int flag = 0;
+    tf_status st = reduce_field(c, c->uk, 1.0, nullptr, &flag);
+    if (st != TF_OK) return st;
+    if (flag) return fail(c, TF_ERR_INVALID_ARG, "state has non-finite or non-positive values");
+    std::swap(c->u, c->uk);
+    c->have_state = true;
+    return TF_OK;
+}
+
+tf_status tf_get_state(tf_ctx* c, double* h_out, int is_device_ptr)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    if (!h_out) return fail(c, TF_ERR_INVALID_ARG, "h_out is NULL");
+    if (!c->have_state) return fail(c, TF_ERR_STATE, "no state set");
+    const size_t bytes = (size_t)c->P.nx * c->P.ny * sizeof(double);
+    TF_CUDA(c, cudaMemcpyAsync(h_out, c->u, bytes, is_device_ptr ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
+                               c->stream));
+    TF_CUDA(c, cudaStreamSynchronize(c->stream));
+    return TF_OK;
+}
+
+tf_status tf_step(tf_ctx* c, double dt, int* newton_iters, double* residual)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    if (!(dt > 0) || !std::isfinite(dt)) return fail(c, TF_ERR_INVALID_ARG, "dt must be positive and finite");
+    if (!c->have_state) return fail(c, TF_ERR_STATE, "no state set");
+    const double s = 0.5 * dt;
+    const bool fixed = c->fixed_iters > 0;
+    const int kmax = fixed ? c->fixed_iters : c->max_iter;
+    TF_CUDA(c, cudaMemsetAsync(c->red, 0, sizeof(double) * 2 * (size_t)kmax, c->stream));
+    int k = 0;
+    double res = 0.0;
+    tf_status status = TF_NOT_CONVERGED;
+    if (fixed) {
+        // parity mode: no host decision inside the step, one read at the end
+        for (; k < kmax; ++k) TF_CUDA(c, launch_iteration(c, s, k));
+        TF_CUDA(c, cudaMemcpyAsync(c->pinned, c->red + 2 * (kmax - 1), 2 * sizeof(double), cudaMemcpyDeviceToHost,
+                                   c->stream));
+        TF_CUDA(c, cudaStreamSynchronize(c->stream));
+        res = c->pinned[0];
+        status = TF_OK;
+    } else {
+        while (k < kmax) {
+            TF_CUDA(c, launch_iteration(c, s, k));
+            TF_CUDA(c, cudaMemcpyAsync(c->pinned, c->red + 2 * k, 2 * sizeof(double), cudaMemcpyDeviceToHost,
+                                       c->stream));
+            TF_CUDA(c, cudaStreamSynchronize(c->stream));
+            ++k;
+            res = c->pinned[0];
+            const bool bad = c->pinned[1] != 0.0;
+            if (bad || res != res) break;
+            if (res < c->tol) { status = TF_OK; break; }
+        }
+    }
+    if (status == TF_OK) std::swap(c->u, c->uk);     // pointer swap
+    if (newton_iters) *newton_iters = k;
+    if (residual) *residual = res;
+    return status;
+}
+
+tf_status tf_mass(tf_ctx* c, double* mass)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    if (!mass) return fail(c, TF_ERR_INVALID_ARG, "mass is NULL");
+    if (!c->have_state) return fail(c, TF_ERR_STATE, "no state set");
+    return reduce_field(c, c->u, c->P.dx * c->P.dy, mass, nullptr);
+}
+
+size_t tf_penta_workspace_bytes(int nrow, int ncol)
+{
+    if (nrow < 1 || ncol < 1) return 0;
+    return 3 * align_up((size_t)nrow * ncol * sizeof(double));
+}
+
+tf_status tf_penta_solve(int nrow, int ncol, int dir, const double* e, const double* c, const double* d,
+                         const double* a, const double* b, const double* rhs, double* x, void* dev_ws,
+                         void* cuda_stream)
+{
+    if (nrow < 1 || ncol < 1 || (dir != 0 && dir != 1)) return fail(nullptr, TF_ERR_INVALID_ARG, "bad shape or dir");
+    if ((dir ? nrow : ncol) < 3) return fail(nullptr, TF_ERR_INVALID_ARG, "system length must be >= 3");
+    if (!e || !c || !d || !a || !b || !rhs || !x || !dev_ws) return fail(nullptr, TF_ERR_INVALID_ARG, "NULL pointer");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t fb = align_up((size_t)nrow * ncol * sizeof(double));
+    double* al = (double*)dev_ws;
+    double* be = (double*)((char*)dev_ws + fb);
+    double* zz = (double*)((char*)dev_ws + 2 * fb);
+    if (dir == 1) {
+        const int g = (ncol + 31) / 32;
+        penta_col_fwd_kernel<<<g, 32, 0, st>>>(nrow, ncol, e, c, d, a, b, rhs, al, be, zz);
+        ybwd_kernel<<<g, 32, 0, st>>>(ncol, nrow, al, be, zz, x);
+    } else {
+        const int g = (nrow + XT - 1) / XT;
+        const size_t sm = sizeof(double) * PT_ARR * XT * XTP;
+        static bool attr_set = false;
+        if (!attr_set) {
+            cudaError_t ee = cudaFuncSetAttribute(penta_row_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+            if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
+            attr_set = true;
+        }
+        penta_row_fwd_kernel<<<g, 32, sm, st>>>(nrow, ncol, e, c, d, a, b, rhs, al, be, zz);
+        penta_row_bwd_kernel<<<g, 32, 0, st>>>(nrow, ncol, al, be, zz, x);
+    }
+    count_launch(2);
+    cudaError_t ee = cudaGetLastError();
+    if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "tf_penta_solve launch");
+    return TF_OK;
+}
+
+const char* tf_last_error(const tf_ctx* c) { return c ? c->err.c_str() : g_err.c_str(); }
+
+unsigned long long tf_kernel_launches(void) { return g_launches.load(); }
+
+}  // extern "C"

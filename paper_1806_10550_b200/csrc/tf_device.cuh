@@ -1,0 +1,120 @@
+// tf_device.cuh -- device-side arithmetic shared by the sweep kernels (sm_100a, fp64).
+//
+// What is computed (citations are PAPER.md lines of arXiv:1806.10550):
+//   cell functions  f0 = h^3, f0' = 3h^2, f1 = h^3 Pi'(h), f1' = d f1/dh      (1.7)-(1.8), :84-91
+//   face flux       F = fb0 * d(lap h)/ds + fb1 * dh/ds, fb = mean of 2 cells  (2.1), (2.27), :134, :290
+//   directional Jacobian partials of the face flux                             (2.26), :274-278
+//   pentadiagonal LU forward elimination / back substitution                   :729-734, (A.5)
+// Everything is scaled by s = dt/2 and the grid spacings up front so that a row of the
+// system matrix I + s*J costs the fewest fp64 instructions (the fp64 pipe is the co-limiter
+// of this path next to HBM).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tf {
+
+struct Params {
+    int nx, ny;
+    double dx, dy;
+    double rdx2, rdy2;      // 1/dx^2, 1/dy^2
+    int n, m;               // Pi exponents, n > m >= 1
+    double cm, cn;          // kappa*m*hstar^m, kappa*n*hstar^n
+};
+
+// per-direction constants for one dt:  ca = s/(2 d^4),  cb = s/(2 d^2)
+struct Dir { double ca, cb; };
+
+__device__ __forceinline__ int refl(int k, int N) { return k < 0 ? -k - 1 : (k >= N ? 2 * N - 1 - k : k); }
+__device__ __forceinline__ int clampi(int k, int lo, int hi) { return k < lo ? lo : (k > hi ? hi : k); }
+// reflected then clamped: safe address for any k, exact ghost for k in [-N, 2N)
+__device__ __forceinline__ int ghost(int k, int N) { return clampi(refl(k, N), 0, N - 1); }
+
+__device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
+
+struct Cell { double f0, f1, g0, g1; };
+
+// r^k for k >= 0, h^(-k) for k < 0 (small integer k; unrolled by the compiler when k is constant)
+__device__ __forceinline__ double ipow_rh(double r, double h, int k)
+{
+    double b = k >= 0 ? r : h, p = 1.0;
+    for (int t = (k >= 0 ? k : -k); t > 0; --t) p *= b;
+    return p;
+}
+
+// Cell-centre functions.  With r = 1/h:  h^3 Pi'(h) = cm r^(m-2) - cn r^(n-2)  and its derivative
+// (2-m) cm r^(m-1) + (n-2) cn r^(n-1)  (the same polynomials as 3h^2 Pi' + h^3 Pi'', summed exactly).
+template <int N, int M>
+__device__ __forceinline__ Cell cell_functions(double h, const Params& P)
+{
+    Cell c;
+    const double r = rcp(h);
+    const double h2 = h * h;
+    c.f0 = h2 * h;
+    c.g0 = 3.0 * h2;
+    if (N == 3 && M == 2) {
+        c.f1 = fma(-P.cn, r, P.cm);
+        c.g1 = P.cn * r * r;
+    } else {
+        const int n = P.n, m = P.m;
+        c.f1 = P.cm * ipow_rh(r, h, m - 2) - P.cn * ipow_rh(r, h, n - 2);
+        c.g1 = (2 - m) * P.cm * ipow_rh(r, h, m - 1) + (n - 2) * P.cn * ipow_rh(r, h, n - 1);
+    }
+    return c;
+}
+
+// Scaled partials of one interior face between line points k and k+1 (spacing d):
+//   A  = s/d * dF/dh_{k+2} = -s/d * dF/dh_{k-1} = ca*(f0_k + f0_{k+1})
+//   p1 = s/d * dF/dh_k,  p2 = s/d * dF/dh_{k+1}            (unfolded)
+struct Face { double A, p1, p2; };
+
+// hm1..hp2 = h_{k-1}, h_k, h_{k+1}, h_{k+2};  sf0 = f0_k + f0_{k+1}, sf1 likewise;  dh = h_{k+1} - h_k
+__device__ __forceinline__ Face face_partials(double hm1, double hp2, double dh, double sf0, double sf1,
+                                              const Cell& ck, const Cell& ck1, const Dir& D)
+{
+    Face f;
+    f.A = D.ca * sf0;
+    const double B = D.cb * sf1;
+    const double t = fma(-3.0, dh, hp2 - hm1);        // third difference * d^3
+    const double tt = D.ca * t, gg = D.cb * dh;
+    const double c3 = fma(3.0, f.A, -B);
+    f.p1 = fma(ck.g0, tt, fma(ck.g1, gg, c3));
+    f.p2 = fma(ck1.g0, tt, fma(ck1.g1, gg, -c3));
+    return f;
+}
+
+// One row of the LU forward elimination.  State: (a1,b1,z1) = row i-1, (a2,b2,z2) = row i-2.
+struct Elim { double a1, b1, z1, a2, b2, z2; };
+
+__device__ __forceinline__ void elim_row(Elim& S, double e, double c, double q, double a, double b, double y,
+                                         double& al, double& be, double& zz)
+{
+    const double gam = fma(-S.a2, e, c);
+    const double mu = fma(-S.a1, gam, fma(-S.b2, e, q));
+    const double rmu = rcp(mu);
+    al = fma(-S.b1, gam, a) * rmu;
+    be = b * rmu;
+    zz = fma(-S.z1, gam, fma(-S.z2, e, y)) * rmu;
+    S.a2 = S.a1; S.b2 = S.b1; S.z2 = S.z1;
+    S.a1 = al; S.b1 = be; S.z1 = zz;
+}
+
+// order-preserving max for non-negative doubles (NaN bit patterns compare above +inf, so a NaN
+// anywhere surfaces in the result)
+__device__ __forceinline__ void atomic_max_nonneg(double* addr, double v)
+{
+    atomicMax(reinterpret_cast<unsigned long long*>(addr), (unsigned long long)__double_as_longlong(v));
+}
+
+__device__ __forceinline__ double warp_max_nonneg(double v)
+{
+    unsigned long long b = (unsigned long long)__double_as_longlong(v);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        unsigned long long t = __shfl_xor_sync(0xffffffffu, b, o);
+        b = t > b ? t : b;
+    }
+    return __longlong_as_double((long long)b);
+}
+
+}  // namespace tf

@@ -1,0 +1,185 @@
+"""Thin Python binding of the C-ABI in include/tf.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of libtf_b200.so.  PyTorch supplies device
+memory (the workspace, user tensors) and the stream.  There is no fallback: if the library is
+missing or cannot be loaded, importing the symbols below raises.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+OK, NOT_CONVERGED = 0, 1
+ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_ALLOC, ERR_STATE = -1, -2, -3, -4, -5
+BC_NOFLUX = 0
+
+_dp = ctypes.POINTER(ctypes.c_double)
+_vp = ctypes.c_void_p
+_lib = None
+
+# every symbol include/tf.h declares: name -> (restype, argtypes)
+SYMBOLS = {
+    "tf_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int, ctypes.c_int]),
+    "tf_create": (ctypes.c_int, [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double,
+                                 ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
+    "tf_create_with_workspace": (ctypes.c_int, [ctypes.POINTER(_vp), ctypes.c_int, ctypes.c_int, ctypes.c_double,
+                                                ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int,
+                                                ctypes.c_int, ctypes.c_int, _vp, ctypes.c_size_t, _vp]),
+    "tf_destroy": (None, [_vp]),
+    "tf_set_newton": (ctypes.c_int, [_vp, ctypes.c_double, ctypes.c_int, ctypes.c_int]),
+    "tf_set_state": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
+    "tf_get_state": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
+    "tf_step": (ctypes.c_int, [_vp, ctypes.c_double, ctypes.POINTER(ctypes.c_int), _dp]),
+    "tf_mass": (ctypes.c_int, [_vp, _dp]),
+    "tf_penta_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int, ctypes.c_int]),
+    "tf_penta_solve": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int] + [_vp] * 9),
+    "tf_last_error": (ctypes.c_char_p, [_vp]),
+    "tf_kernel_launches": (ctypes.c_ulonglong, []),
+}
+
+
+class TfError(RuntimeError):
+    def __init__(self, status, what, text=""):
+        super().__init__(f"{what} failed: status {status} {text}")
+        self.status = status
+
+
+def lib():
+    """Load libtf_b200.so (building it with nvcc if the sources are newer).  Raises if impossible."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if _build.stale():
+            path = _build.build()
+        L = ctypes.CDLL(path)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(L, name)          # AttributeError if a declared symbol is not exported
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _err(handle, status, what):
+    text = lib().tf_last_error(handle)
+    raise TfError(status, what, text.decode() if text else "")
+
+
+def kernel_launches():
+    return int(lib().tf_kernel_launches())
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise TfError(ERR_CUDA, "cuda", "no CUDA device: this package has no CPU path")
+    return torch
+
+
+class ThinFilm:
+    """tf_create / tf_set_newton / tf_set_state / tf_step / tf_get_state / tf_mass on one GPU."""
+
+    def __init__(self, nx, ny, dx, dy, kappa=100.0, hstar=0.1, n=3, m=2, bc=BC_NOFLUX, device=None, stream=None):
+        torch = _torch()
+        L = lib()
+        self.nx, self.ny = int(nx), int(ny)
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        self._h = _vp()
+        nbytes = L.tf_workspace_bytes(self.nx, self.ny)
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(max(nbytes, 256) + 256, dtype=torch.uint8, device=self.device)
+            base = self._ws.data_ptr()
+            off = (-base) % 256
+            self._stream = torch.cuda.current_stream(self.device) if stream is None else stream
+            st = L.tf_create_with_workspace(ctypes.byref(self._h), self.nx, self.ny, dx, dy, kappa, hstar, n, m, bc,
+                                            base + off, nbytes, self._stream.cuda_stream)
+        if st != OK:
+            self._h = _vp()
+            _err(None, st, "tf_create_with_workspace")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().tf_destroy(self._h)
+            self._h = _vp()
+            self._ws = None
+
+    __del__ = close
+
+    def set_newton(self, tol=1e-10, max_iter=10, fixed_iters=0):
+        st = lib().tf_set_newton(self._h, tol, max_iter, fixed_iters)
+        if st != OK:
+            _err(self._h, st, "tf_set_newton")
+
+    def set_state(self, h):
+        """h: torch CUDA float64 tensor [ny][nx] (device copy) or numpy / CPU tensor (host copy)."""
+        ptr, is_dev, keep = self._marshal(h, writable=False)
+        st = lib().tf_set_state(self._h, ptr, is_dev)
+        if st != OK:
+            _err(self._h, st, "tf_set_state")
+
+    def get_state(self, out=None):
+        """Returns the state: into `out` (torch CUDA tensor or numpy array) or a new numpy array."""
+        if out is None:
+            out = np.empty((self.ny, self.nx), dtype=np.float64)
+        ptr, is_dev, keep = self._marshal(out, writable=True)
+        st = lib().tf_get_state(self._h, ptr, is_dev)
+        if st != OK:
+            _err(self._h, st, "tf_get_state")
+        return out
+
+    def step(self, dt):
+        """One time step; returns (status, newton_iters, residual).  status 1 = rejected, state unchanged."""
+        it, res = ctypes.c_int(0), ctypes.c_double(0.0)
+        st = lib().tf_step(self._h, dt, ctypes.byref(it), ctypes.byref(res))
+        if st < 0:
+            _err(self._h, st, "tf_step")
+        return st, it.value, res.value
+
+    def mass(self):
+        m = ctypes.c_double(0.0)
+        st = lib().tf_mass(self._h, ctypes.byref(m))
+        if st != OK:
+            _err(self._h, st, "tf_mass")
+        return m.value
+
+    def _marshal(self, h, writable):
+        if isinstance(h, np.ndarray):
+            if h.dtype != np.float64 or not h.flags["C_CONTIGUOUS"] or h.shape != (self.ny, self.nx):
+                if writable:
+                    raise ValueError("output must be a C-contiguous float64 [ny][nx] array")
+                h = np.ascontiguousarray(h, dtype=np.float64)
+                if h.shape != (self.ny, self.nx):
+                    raise ValueError(f"expected shape {(self.ny, self.nx)}, got {h.shape}")
+            return h.ctypes.data, 0, h
+        torch = _torch()
+        if not isinstance(h, torch.Tensor):
+            raise TypeError("expected numpy array or torch tensor")
+        if h.dtype != torch.float64 or not h.is_contiguous() or tuple(h.shape) != (self.ny, self.nx):
+            raise ValueError("expected a contiguous float64 [ny][nx] tensor")
+        return h.data_ptr(), (1 if h.is_cuda else 0), h
+
+
+def penta_solve(direction, e, c, d, a, b, rhs, out=None, workspace=None, stream=None):
+    """tf_penta_solve on torch CUDA float64 tensors [nrow][ncol]; direction 0: rows are systems, 1: columns.
+    Enqueues on the current stream and returns `out` without synchronising."""
+    torch = _torch()
+    ts = (e, c, d, a, b, rhs)
+    nrow, ncol = e.shape
+    for t in ts:
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                and tuple(t.shape) == (nrow, ncol)):
+            raise ValueError("expected contiguous CUDA float64 tensors of one shape")
+    if out is None:
+        out = torch.empty_like(e)
+    L = lib()
+    need = L.tf_penta_workspace_bytes(nrow, ncol)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=e.device)
+    if workspace.numel() * workspace.element_size() < need or workspace.data_ptr() % 256:
+        raise ValueError("workspace too small or not 256-byte aligned")
+    st = (torch.cuda.current_stream(e.device) if stream is None else stream).cuda_stream
+    rc = L.tf_penta_solve(nrow, ncol, direction, *[t.data_ptr() for t in ts], out.data_ptr(), workspace.data_ptr(), st)
+    if rc != OK:
+        _err(None, rc, "tf_penta_solve")
+    return out

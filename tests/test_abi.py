@@ -1,0 +1,55 @@
+"""No-GPU checks of the boundary: the C-ABI library builds, loads and exports every symbol that
+include/tf.h declares; argument validation that needs no device."""
+import ctypes
+import os
+import re
+
+from paper_1806_10550_b200 import tf
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "tf.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return set(re.findall(r"\b(tf_[a-z_]+)\s*\(", src))
+
+
+def test_library_exports_every_declared_symbol():
+    L = tf.lib()
+    decl = declared_symbols()
+    assert decl == set(tf.SYMBOLS), (decl ^ set(tf.SYMBOLS))
+    for name in decl:
+        assert hasattr(L, name), name
+
+
+def test_workspace_sizes_and_host_side_validation():
+    L = tf.lib()
+    assert L.tf_workspace_bytes(4, 128) == 0
+    n = L.tf_workspace_bytes(128, 128)
+    assert n >= 7 * 128 * 128 * 8 and n % 256 == 0
+    assert L.tf_penta_workspace_bytes(64, 32) >= 3 * 64 * 32 * 8
+    h = ctypes.c_void_p()
+    # invalid arguments are rejected before any device work
+    assert L.tf_create(ctypes.byref(h), 3, 128, 0.1, 0.1, 100.0, 0.1, 3, 2, 0) == tf.ERR_INVALID_ARG
+    assert L.tf_create(ctypes.byref(h), 128, 128, 0.1, 0.1, 100.0, 0.1, 2, 3, 0) == tf.ERR_INVALID_ARG
+    assert L.tf_create(ctypes.byref(h), 128, 128, -0.1, 0.1, 100.0, 0.1, 3, 2, 0) == tf.ERR_INVALID_ARG
+    assert L.tf_create(ctypes.byref(h), 128, 128, 0.1, 0.1, 100.0, 0.1, 3, 2, 1) == tf.ERR_UNSUPPORTED
+    assert b"2.28" in L.tf_last_error(None)
+    assert L.tf_penta_solve(8, 8, 2, *([None] * 9)) == tf.ERR_INVALID_ARG
+    assert L.tf_kernel_launches() == 0
+
+
+def test_product_path_does_not_touch_the_oracle():
+    """The package must not import, link or call anything under oracle/ (and vice versa)."""
+    pkg = os.path.join(ROOT, "paper_1806_10550_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in txt.lower() or f == "inputs.py", f
+                assert "tfo_" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_1806_10550_b200 import" not in txt and "libtf_b200" not in txt, f
