@@ -1,0 +1,280 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the ADI time step (all S0-S9 rows of DESIGN.md) on BASELINE.json config 3.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl b200|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A "step" is one tf_step (b^n, then pseudo-Newton iterations of y-sweep + x-sweep + residual until
+res < tol) on the 8192x8192 spinodal film of config 3.  value = grid points x steps / seconds over all
+ranks (weak scaling: every rank advances its own 8192^2 replica; the path has no exchange step on one
+GPU).  Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1806_10550_b200 import inputs  # noqa: E402
+
+METRIC = "grid-point ADI steps/sec (fp64)"
+UNIT = "grid-point-steps/s"
+# algorithmic HBM bytes per grid point per launch
+ALG_BYTES = {"y_forward": 40, "y_backward": 32, "x_forward": 40, "x_backward_update": 40}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (0-3); 3 is the headline")
+    ap.add_argument("--fixed-iters", type=int, default=0, help="fixed Newton count per step (0: converge to tol)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons of one GPU every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [t.strip() for t in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.th.join(timeout=2)
+        rows = [r for t, r in self.rows if t0 <= t <= t1 and len(r) >= 7] or [r for _, r in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(r[3 + k].lower().startswith("active") for r in rows)]
+        pw = [float(r[2]) for r in rows if r[2].replace(".", "", 1).isdigit()]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons,
+                "samples": len(rows), "power_w_max": max(pw) if pw else None}
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(kernel):
+    """dram bytes per launch of `kernel` from the committed ncu --set full summary, or None."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get(kernel, {}).get("dram_bytes_per_launch")
+        except Exception:
+            return None
+    return None
+
+
+# ----------------------------------------------------------------------------------------- CPU oracle legs
+def oracle_sample_run(cfg, n, steps, warmup, fixed_iters):
+    """Times the CPU oracle AS IT STANDS (serial build) on an n x n cut of the config's recipe."""
+    from oracle import tfo
+    o = tfo.ThinFilmOracle(n, n, cfg["dx"], cfg["dy"], cfg["kappa"], cfg["hstar"], cfg["n"], cfg["m"])
+    o.set_newton(cfg["tol"], cfg["max_iter"], fixed_iters)
+    o.set_state(inputs.initial_condition(cfg, n, n))
+    for _ in range(warmup):
+        o.step(cfg["dt"])
+    t0 = time.perf_counter()
+    iters = 0
+    for _ in range(steps):
+        st, it, _ = o.step(cfg["dt"])
+        iters += it
+    dt = time.perf_counter() - t0
+    return dict(seconds=dt, iters=iters, pts=n * n, steps=steps, cores=tfo.num_threads(False))
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n = min(1024 if (args.steps + args.warmup) <= 30 else 512, cfg["nx"], cfg["ny"])
+    r = oracle_sample_run(cfg, n, args.steps, args.warmup, args.fixed_iters)
+    value = r["pts"] * r["steps"] / r["seconds"]
+    sample = f"{n}x{n} cut of {cfg['name']} (same dx, dt, IC recipe and seed), {args.steps} steps after {args.warmup} warm-up"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * r["seconds"] / r["steps"],
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "grid": [cfg["nx"], cfg["ny"]], "dt": cfg["dt"], "tol": cfg["tol"],
+                   "note": "CPU oracle (oracle/tfo.c, serial, untuned) on a bounded sample; size-independent unit"},
+        "newton_iters_total": r["iters"],
+        "point_iterations_per_s": r["pts"] * r["iters"] / r["seconds"],
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------- B200 arm
+def run_b200(args, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_1806_10550_b200 import tf
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl b200 needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    nx, ny, dt = cfg["nx"], cfg["ny"], cfg["dt"]
+    npts = nx * ny
+    h_host = torch.from_numpy(inputs.initial_condition(cfg)).pin_memory()     # every rank: its own replica
+    h_dev = h_host.cuda(non_blocking=True)
+    ctx = tf.ThinFilm(nx, ny, cfg["dx"], cfg["dy"], cfg["kappa"], cfg["hstar"], cfg["n"], cfg["m"])
+    ctx.set_newton(cfg["tol"], cfg["max_iter"], args.fixed_iters)
+
+    def timed_run(e2e):
+        """W warm-up + K timed steps from the initial condition; returns (seconds, iters, launches, t0, t1)."""
+        ctx.set_state(h_dev)
+        hbuf = h_host.clone().pin_memory() if e2e else None
+
+        def one():
+            if e2e:
+                ctx.set_state(hbuf)              # H2D of the step's input from pinned host memory
+            st, it, res = ctx.step(dt)
+            if st != tf.OK:
+                raise SystemExit(f"tf_step did not converge (status {st}, iters {it}, res {res})")
+            if e2e:
+                ctx.get_state(hbuf)              # D2H of the step's result
+            return it
+
+        for _ in range(args.warmup):
+            one()
+        ctx.set_profiling(not e2e)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        l0, w0 = tf.kernel_launches(), time.time()
+        ev0.record()
+        iters = sum(one() for _ in range(args.steps))
+        ev1.record()
+        barrier()
+        w1 = time.time()
+        sec = ev0.elapsed_time(ev1) / 1e3
+        if world > 1:
+            t = torch.tensor([sec], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            sec = float(t.item())
+        return sec, iters, tf.kernel_launches() - l0, w0, w1
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    sec, iters, launches, w0, w1 = timed_run(e2e=False)
+    clocks = sampler.stop(w0, w1) if sampler else None
+    prof = ctx.get_profile()
+    mass_drift = None
+    if rank == 0:
+        m1 = ctx.mass()
+        m0 = float(h_host.sum(dtype=torch.float64).item()) * cfg["dx"] * cfg["dy"]
+        mass_drift = abs(m1 - m0) / m0
+    e2e = None
+    if not args.no_e2e:
+        esec, eiters, _, _, _ = timed_run(e2e=True)
+        e2e = {"value": world * npts * args.steps / esec, "unit": UNIT, "h2d_bytes_per_step": npts * 8,
+               "d2h_bytes_per_step": npts * 8, "ms_per_step": 1e3 * esec / args.steps, "newton_iters_total": eiters}
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src = measured_peak()
+    kern = {}
+    for name, (ms, n) in prof.items():
+        if n:
+            avg = ms / n
+            kern[name] = {"avg_ms": avg, "launches": n, "alg_bytes_per_launch": ALG_BYTES[name] * npts,
+                          "alg_gbs": ALG_BYTES[name] * npts / (avg * 1e-3) / 1e9}
+    dom = max(kern, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"]) if kern else None
+    roofline = None
+    if dom:
+        a = kern[dom]["alg_gbs"]
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": a, "peak": peak, "unit": "GB/s", "frac": a / peak,
+                    "peak_source": peak_src, "traffic": ncu_traffic(dom),
+                    "alg_bytes_per_launch": kern[dom]["alg_bytes_per_launch"], "avg_launch_ms": kern[dom]["avg_ms"]}
+    ksum = sum(k["avg_ms"] * k["launches"] for k in kern.values())
+    line = {
+        "metric": METRIC, "value": world * npts * args.steps / sec, "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "grid": [nx, ny], "dx": cfg["dx"], "dt": dt, "tol": cfg["tol"],
+                   "max_iter": cfg["max_iter"], "fixed_iters": args.fixed_iters,
+                   "ic": "1 + 0.01 U[-1,1] seeded noise", "parallelism": f"replicas x{world} (no exchange step)",
+                   "l2": "working set 7 fields x 512 MiB >> 126 MB L2: every launch streams from HBM, no flush needed"},
+        "newton_iters_total": iters, "newton_iters_per_step": iters / args.steps,
+        "point_iterations_per_s": world * npts * iters / sec,
+        "penta_unknowns_per_s": 2 * world * npts * iters / sec,
+        "iteration_model": {"bytes_per_point_iter": 152, "gbs": 152 * npts * iters / sec / 1e9,
+                            "frac_of_peak": 152 * npts * iters / sec / 1e9 / peak,
+                            "compulsory_48B_gbs": 48 * npts * iters / sec / 1e9},
+        "kernels": kern, "kernel_time_share_of_step": ksum / (sec * 1e3) if kern else None,
+        "roofline": roofline, "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+        "mass_rel_drift": mass_drift,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        n = 2048 if min(nx, ny) >= 2048 else min(nx, ny)
+        r = oracle_sample_run(cfg, n, 1, 0, args.fixed_iters)
+        line["cpu_baseline"] = {
+            "value": r["pts"] * r["steps"] / r["seconds"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
+            "sample": f"{n}x{n} cut of {cfg['name']} (same dx, dt, IC recipe, seed), first step, {r['iters']} Newton "
+                      f"iterations, {r['seconds']:.1f} s",
+            "point_iterations_per_s": r["pts"] * r["iters"] / r["seconds"]}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    cfg = inputs.config(args.config)
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_b200(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

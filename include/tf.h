@@ -111,6 +111,19 @@ tf_status tf_penta_solve(int nrow, int ncol, int dir,
  * tf_create* / tf_penta_solve on this thread.  Valid until the next call. */
 const char* tf_last_error(const tf_ctx* ctx);
 
+/*
+ * Per-kernel device timing of the Newton iteration (for bench.py's roofline object).  When on,
+ * tf_step brackets each of its four kernels with CUDA events on the context's stream and
+ * accumulates the elapsed times.  Slots: 0 = y forward (assembly + elimination), 1 = y backward,
+ * 2 = x forward, 3 = x backward + update + residual.  tf_get_profile copies the accumulated
+ * milliseconds and launch counts (either may be NULL) and does not reset them;
+ * tf_set_profiling(ctx, on) resets them.  Only steps with a per-iteration host decision
+ * (fixed_iters = 0) or fixed_iters <= 64 are profiled.
+ */
+#define TF_PROFILE_SLOTS 4
+tf_status tf_set_profiling(tf_ctx* ctx, int on);
+tf_status tf_get_profile(tf_ctx* ctx, double ms[TF_PROFILE_SLOTS], unsigned long long launches[TF_PROFILE_SLOTS]);
+
 /* Number of kernels this library has launched since load (all contexts); for bench.py's
  * gpu_launches claim. */
 unsigned long long tf_kernel_launches(void);

@@ -41,6 +41,10 @@ struct tf_ctx {
     double *part;                              // [RED_BLOCKS]
     double *scal;                              // [8] : scal[0] mass, (int*)(scal+1) flag
     double *pinned;                            // [4] host pinned readback
+    bool profiling;
+    cudaEvent_t ev[65 * 5];                    // 5 events per iteration, up to 65 iterations in flight
+    double prof_ms[TF_PROFILE_SLOTS];
+    unsigned long long prof_n[TF_PROFILE_SLOTS];
     std::string err;
 };
 
@@ -69,28 +73,48 @@ Dir make_dir(double s, double d) { Dir D; D.ca = s / (2.0 * d * d * d * d); D.cb
 
 // one pseudo-Newton iteration k: reads src (u^n if k == 0 else uk), writes uk, red[2k..2k+1]
 template <int N, int M>
-cudaError_t launch_iteration(tf_ctx* c, double s, int k)
+cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
 {
     const Params& P = c->P;
     const Dir DX = make_dir(s, P.dx), DY = make_dir(s, P.dy);
     const double* src = (k == 0) ? c->u : c->uk;
     const int gy = (P.nx + YF_VALID - 1) / YF_VALID;
+    cudaEvent_t* ev = (c->profiling && slot >= 0) ? c->ev + 5 * slot : nullptr;
+    if (ev) cudaEventRecord(ev[0], c->stream);
     if (k == 0)
         yfwd_kernel<N, M, true><<<gy, 32, 0, c->stream>>>(P, DX, DY, src, c->bn, c->al, c->be, c->zz);
     else
         yfwd_kernel<N, M, false><<<gy, 32, 0, c->stream>>>(P, DX, DY, src, c->bn, c->al, c->be, c->zz);
+    if (ev) cudaEventRecord(ev[1], c->stream);
     ybwd_kernel<<<(P.nx + 31) / 32, 32, 0, c->stream>>>(P.nx, P.ny, c->al, c->be, c->zz, c->w);
+    if (ev) cudaEventRecord(ev[2], c->stream);
     const int gx = (P.ny + XT - 1) / XT;
     xfwd_kernel<N, M><<<gx, 32, 0, c->stream>>>(P, DX, src, c->w, c->al, c->be, c->zz);
+    if (ev) cudaEventRecord(ev[3], c->stream);
     xbwd_kernel<<<gx, 32, 0, c->stream>>>(P.nx, P.ny, c->al, c->be, c->zz, src, c->uk, c->red + 2 * k);
+    if (ev) cudaEventRecord(ev[4], c->stream);
     count_launch(4);
     return cudaGetLastError();
 }
 
-cudaError_t launch_iteration(tf_ctx* c, double s, int k)
+cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
 {
-    if (c->P.n == 3 && c->P.m == 2) return launch_iteration<3, 2>(c, s, k);
-    return launch_iteration<0, 0>(c, s, k);
+    if (c->P.n == 3 && c->P.m == 2) return launch_iteration<3, 2>(c, s, k, slot);
+    return launch_iteration<0, 0>(c, s, k, slot);
+}
+
+// after a stream sync: fold the event intervals of `niter` profiled iterations into the totals
+void collect_profile(tf_ctx* c, int niter)
+{
+    if (!c->profiling) return;
+    for (int it = 0; it < niter; ++it)
+        for (int q = 0; q < TF_PROFILE_SLOTS; ++q) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, c->ev[5 * it + q], c->ev[5 * it + q + 1]) == cudaSuccess) {
+                c->prof_ms[q] += ms;
+                c->prof_n[q] += 1;
+            }
+        }
 }
 
 tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, double kappa, double hstar,
@@ -148,6 +172,9 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
         delete c;
         return fail(nullptr, TF_ERR_ALLOC, std::string("cudaMallocHost: ") + cudaGetErrorString(e));
     }
+    c->profiling = false;
+    for (auto& ev : c->ev) ev = nullptr;
+    for (int q = 0; q < TF_PROFILE_SLOTS; ++q) { c->prof_ms[q] = 0.0; c->prof_n[q] = 0; }
     *out = c;
     return TF_OK;
 }
@@ -196,6 +223,7 @@ void tf_destroy(tf_ctx* c)
     if (!c) return;
     cudaStreamSynchronize(c->stream);
     if (c->owns_ws) cudaFree(c->ws);
+    for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
     cudaFreeHost(c->pinned);
     delete c;
 }
@@ -253,18 +281,21 @@ tf_status tf_step(tf_ctx* c, double dt, int* newton_iters, double* residual)
     tf_status status = TF_NOT_CONVERGED;
     if (fixed) {
         // parity mode: no host decision inside the step, one read at the end
-        for (; k < kmax; ++k) TF_CUDA(c, launch_iteration(c, s, k));
+        const bool prof = c->profiling && kmax <= 64;
+        for (; k < kmax; ++k) TF_CUDA(c, launch_iteration(c, s, k, prof ? k : -1));
         TF_CUDA(c, cudaMemcpyAsync(c->pinned, c->red + 2 * (kmax - 1), 2 * sizeof(double), cudaMemcpyDeviceToHost,
                                    c->stream));
         TF_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (prof) collect_profile(c, kmax);
         res = c->pinned[0];
         status = TF_OK;
     } else {
         while (k < kmax) {
-            TF_CUDA(c, launch_iteration(c, s, k));
+            TF_CUDA(c, launch_iteration(c, s, k, 0));
             TF_CUDA(c, cudaMemcpyAsync(c->pinned, c->red + 2 * k, 2 * sizeof(double), cudaMemcpyDeviceToHost,
                                        c->stream));
             TF_CUDA(c, cudaStreamSynchronize(c->stream));
+            collect_profile(c, 1);
             ++k;
             res = c->pinned[0];
             const bool bad = c->pinned[1] != 0.0;
@@ -284,6 +315,27 @@ tf_status tf_mass(tf_ctx* c, double* mass)
     if (!mass) return fail(c, TF_ERR_INVALID_ARG, "mass is NULL");
     if (!c->have_state) return fail(c, TF_ERR_STATE, "no state set");
     return reduce_field(c, c->u, c->P.dx * c->P.dy, mass, nullptr);
+}
+
+tf_status tf_set_profiling(tf_ctx* c, int on)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    if (on)
+        for (auto& ev : c->ev)
+            if (!ev) TF_CUDA(c, cudaEventCreate(&ev));
+    c->profiling = on != 0;
+    for (int q = 0; q < TF_PROFILE_SLOTS; ++q) { c->prof_ms[q] = 0.0; c->prof_n[q] = 0; }
+    return TF_OK;
+}
+
+tf_status tf_get_profile(tf_ctx* c, double ms[TF_PROFILE_SLOTS], unsigned long long launches[TF_PROFILE_SLOTS])
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    for (int q = 0; q < TF_PROFILE_SLOTS; ++q) {
+        if (ms) ms[q] = c->prof_ms[q];
+        if (launches) launches[q] = c->prof_n[q];
+    }
+    return TF_OK;
 }
 
 size_t tf_penta_workspace_bytes(int nrow, int ncol)

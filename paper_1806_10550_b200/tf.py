@@ -35,6 +35,8 @@ SYMBOLS = {
     "tf_mass": (ctypes.c_int, [_vp, _dp]),
     "tf_penta_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int, ctypes.c_int]),
     "tf_penta_solve": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int] + [_vp] * 9),
+    "tf_set_profiling": (ctypes.c_int, [_vp, ctypes.c_int]),
+    "tf_get_profile": (ctypes.c_int, [_vp, _dp, ctypes.POINTER(ctypes.c_ulonglong)]),
     "tf_last_error": (ctypes.c_char_p, [_vp]),
     "tf_kernel_launches": (ctypes.c_ulonglong, []),
 }
@@ -142,6 +144,22 @@ class ThinFilm:
         if st != OK:
             _err(self._h, st, "tf_mass")
         return m.value
+
+    PROFILE_SLOTS = ("y_forward", "y_backward", "x_forward", "x_backward_update")
+
+    def set_profiling(self, on=True):
+        st = lib().tf_set_profiling(self._h, 1 if on else 0)
+        if st != OK:
+            _err(self._h, st, "tf_set_profiling")
+
+    def get_profile(self):
+        """{kernel: (total_ms, launches)} accumulated since set_profiling(True)."""
+        ms = (ctypes.c_double * 4)()
+        n = (ctypes.c_ulonglong * 4)()
+        st = lib().tf_get_profile(self._h, ms, n)
+        if st != OK:
+            _err(self._h, st, "tf_get_profile")
+        return {k: (ms[i], int(n[i])) for i, k in enumerate(self.PROFILE_SLOTS)}
 
     def _marshal(self, h, writable):
         if isinstance(h, np.ndarray):
