@@ -2,7 +2,9 @@
 // Host side only orders kernels on one stream and reads one 16-byte residual record per Newton
 // iteration (the paper reads IJ/256 flag bytes per iteration; S8 of DESIGN.md).
 #include "../../include/tf.h"
+#include <cuda.h>
 #include "tf_penta.cuh"
+#include "tf_bwd.cuh"
 
 #include <atomic>
 #include <cmath>
@@ -41,6 +43,10 @@ struct tf_ctx {
     double *part;                              // [RED_BLOCKS]
     double *scal;                              // [8] : scal[0] mass, (int*)(scal+1) flag
     double *pinned;                            // [4] host pinned readback
+    bool tma_y, tma_x;                         // TMA rings usable (row pitch multiple of 16 B, grid >= one box)
+    CUtensorMap mY[3], mX[3];                  // alpha,beta,z as [ny][nx] (box RS x 32) and as [nx][ny] (box CS x 32)
+    CUtensorMap mU[2];                         // the two state buffers as [ny][nx], box 32 x 16, 128-byte swizzle
+    double* ubuf[2];                           // buffer addresses mU[0], mU[1] were encoded for
     bool profiling;
     cudaEvent_t ev[65 * 5];                    // 5 events per iteration, up to 65 iterations in flight
     double prof_ms[TF_PROFILE_SLOTS];
@@ -71,6 +77,116 @@ inline void count_launch(int n = 1) { g_launches.fetch_add((unsigned long long)n
 
 Dir make_dir(double s, double d) { Dir D; D.ca = s / (2.0 * d * d * d * d); D.cb = s / (2.0 * d * d); return D; }
 
+// ---- TMA tensor maps (driver entry point fetched through the runtime: no link-time libcuda dependency)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// fp64 matrix [outer][inner] (row pitch inner*8 bytes), box [box_outer][box_inner]
+bool make_map2d(CUtensorMap* m, const double* base, int inner, int outer, int box_inner, int box_outer, bool swz128)
+{
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return false;
+    cuuint64_t dims[2] = {(cuuint64_t)inner, (cuuint64_t)outer};
+    cuuint64_t strides[1] = {(cuuint64_t)inner * sizeof(double)};
+    cuuint32_t box[2] = {(cuuint32_t)box_inner, (cuuint32_t)box_outer};
+    cuuint32_t estr[2] = {1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              swz128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// ---- ring-kernel launchers (dynamic shared memory above 48 KB needs the opt-in attribute once per kernel)
+constexpr int YB_NST = 8, YB_RS = 16;     // 8 stages x 16 rows x 3 arrays x 256 B = 96 KiB per warp
+constexpr int XB_NST = 6, XB_CS = 16;     // 6 stages x (3 x 16 x 256 B + 32 x 18 x 8 B) = 99 KiB per warp
+
+template <typename K>
+cudaError_t opt_in_smem(K kernel, size_t bytes)
+{
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+constexpr int YT_NST = 6, YT_RS = 16;     // TMA ring: 6 stages x 3 boxes of 16 x 32 doubles = 72 KiB per warp
+constexpr int XT_NST = 6;                 // TMA ring: 6 stages x 16 KiB
+
+cudaError_t launch_ybwd_tma(const CUtensorMap* m, int nx, int ny, double* w, cudaStream_t st)
+{
+    constexpr size_t SM = (size_t)YT_NST * 3 * YT_RS * 32 * 8 + 8 * YT_NST + 1024;
+    static bool ready = false;
+    if (!ready) {
+        cudaError_t e = opt_in_smem(ybwd_tma_kernel<YT_NST, YT_RS>, SM);
+        if (e != cudaSuccess) return e;
+        ready = true;
+    }
+    ybwd_tma_kernel<YT_NST, YT_RS><<<(nx + 31) / 32, 32, SM, st>>>(m[0], m[1], m[2], nx, ny, w);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_xbwd_tma(const CUtensorMap* m, const CUtensorMap& uin, const CUtensorMap& uout, int nx, int ny,
+                            double* red, cudaStream_t st)
+{
+    constexpr size_t SM = (size_t)XT_NST * 4 * 16 * 32 * 8 + 8 * XT_NST + 1024;
+    static bool ready = false;
+    if (!ready) {
+        cudaError_t e = opt_in_smem(xbwd_tma_kernel<XT_NST>, SM);
+        if (e != cudaSuccess) return e;
+        ready = true;
+    }
+    xbwd_tma_kernel<XT_NST><<<(ny + 31) / 32, 32, SM, st>>>(m[0], m[1], m[2], uin, uout, nx, ny, red);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ybwd(int nx, int ny, const double* al, const double* be, const double* zz, double* w,
+                        cudaStream_t st)
+{
+    constexpr size_t SM = sizeof(double) * YB_NST * 3 * YB_RS * 32;
+    static bool ready = false;
+    if (!ready) {
+        cudaError_t e = opt_in_smem(ybwd_ring_kernel<YB_NST, YB_RS, true>, SM);
+        if (e == cudaSuccess) e = opt_in_smem(ybwd_ring_kernel<YB_NST, YB_RS, false>, SM);
+        if (e != cudaSuccess) return e;
+        ready = true;
+    }
+    const int g = (nx + 31) / 32;
+    if (nx % 2 == 0) ybwd_ring_kernel<YB_NST, YB_RS, true><<<g, 32, SM, st>>>(nx, ny, al, be, zz, w);
+    else ybwd_ring_kernel<YB_NST, YB_RS, false><<<g, 32, SM, st>>>(nx, ny, al, be, zz, w);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_xbwd(int nx, int ny, const double* alT, const double* beT, const double* zzT, const double* uk,
+                        double* unew, double* red, cudaStream_t st)
+{
+    constexpr size_t SM = sizeof(double) * XB_NST * (3 * XB_CS * 32 + 32 * (XB_CS + 2));
+    static bool ready = false;
+    if (!ready) {
+        cudaError_t e = opt_in_smem(xbwd_ring_kernel<XB_NST, XB_CS, true>, SM);
+        if (e == cudaSuccess) e = opt_in_smem(xbwd_ring_kernel<XB_NST, XB_CS, false>, SM);
+        if (e != cudaSuccess) return e;
+        ready = true;
+    }
+    const int g = (ny + 31) / 32;
+    if (nx % 2 == 0 && ny % 2 == 0)
+        xbwd_ring_kernel<XB_NST, XB_CS, true><<<g, 32, SM, st>>>(nx, ny, alT, beT, zzT, uk, unew, red);
+    else
+        xbwd_ring_kernel<XB_NST, XB_CS, false><<<g, 32, SM, st>>>(nx, ny, alT, beT, zzT, uk, unew, red);
+    return cudaGetLastError();
+}
+
 // one pseudo-Newton iteration k: reads src (u^n if k == 0 else uk), writes uk, red[2k..2k+1]
 template <int N, int M>
 cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
@@ -86,12 +202,19 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
     else
         yfwd_kernel<N, M, false><<<gy, 32, 0, c->stream>>>(P, DX, DY, src, c->bn, c->al, c->be, c->zz);
     if (ev) cudaEventRecord(ev[1], c->stream);
-    ybwd_kernel<<<(P.nx + 31) / 32, 32, 0, c->stream>>>(P.nx, P.ny, c->al, c->be, c->zz, c->w);
+    cudaError_t le = c->tma_y ? launch_ybwd_tma(c->mY, P.nx, P.ny, c->w, c->stream)
+                              : launch_ybwd(P.nx, P.ny, c->al, c->be, c->zz, c->w, c->stream);
+    if (le != cudaSuccess) return le;
     if (ev) cudaEventRecord(ev[2], c->stream);
     const int gx = (P.ny + XT - 1) / XT;
     xfwd_kernel<N, M><<<gx, 32, 0, c->stream>>>(P, DX, src, c->w, c->al, c->be, c->zz);
     if (ev) cudaEventRecord(ev[3], c->stream);
-    xbwd_kernel<<<gx, 32, 0, c->stream>>>(P.nx, P.ny, c->al, c->be, c->zz, src, c->uk, c->red + 2 * k);
+    if (c->tma_x)
+        le = launch_xbwd_tma(c->mX, c->mU[src == c->ubuf[0] ? 0 : 1], c->mU[c->uk == c->ubuf[0] ? 0 : 1], P.nx, P.ny,
+                             c->red + 2 * k, c->stream);
+    else
+        le = launch_xbwd(P.nx, P.ny, c->al, c->be, c->zz, src, c->uk, c->red + 2 * k, c->stream);
+    if (le != cudaSuccess) return le;
     if (ev) cudaEventRecord(ev[4], c->stream);
     count_launch(4);
     return cudaGetLastError();
@@ -171,6 +294,18 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
         if (own) cudaFree(c->ws);
         delete c;
         return fail(nullptr, TF_ERR_ALLOC, std::string("cudaMallocHost: ") + cudaGetErrorString(e));
+    }
+    c->ubuf[0] = c->u; c->ubuf[1] = c->uk;
+    c->tma_y = (nx % 2 == 0) && nx >= 32 && ny >= YT_RS;
+    c->tma_x = (nx % 2 == 0) && (ny % 2 == 0) && nx >= 16 && ny >= 32;
+    if (c->tma_y) {
+        const double* f3[3] = {c->al, c->be, c->zz};
+        for (int k = 0; k < 3; ++k) c->tma_y = c->tma_y && make_map2d(&c->mY[k], f3[k], nx, ny, 32, YT_RS, false);
+    }
+    if (c->tma_x) {
+        const double* f3[3] = {c->al, c->be, c->zz};
+        for (int k = 0; k < 3; ++k) c->tma_x = c->tma_x && make_map2d(&c->mX[k], f3[k], ny, nx, 32, 16, false);
+        for (int k = 0; k < 2; ++k) c->tma_x = c->tma_x && make_map2d(&c->mU[k], c->ubuf[k], nx, ny, 16, 32, true);
     }
     c->profiling = false;
     for (auto& ev : c->ev) ev = nullptr;
@@ -359,7 +494,8 @@ tf_status tf_penta_solve(int nrow, int ncol, int dir, const double* e, const dou
     if (dir == 1) {
         const int g = (ncol + 31) / 32;
         penta_col_fwd_kernel<<<g, 32, 0, st>>>(nrow, ncol, e, c, d, a, b, rhs, al, be, zz);
-        ybwd_kernel<<<g, 32, 0, st>>>(ncol, nrow, al, be, zz, x);
+        cudaError_t le = launch_ybwd(ncol, nrow, al, be, zz, x, st);
+        if (le != cudaSuccess) return cuda_fail(nullptr, le, "ybwd launch");
     } else {
         const int g = (nrow + XT - 1) / XT;
         const size_t sm = sizeof(double) * PT_ARR * XT * XTP;
