@@ -5,6 +5,7 @@
 #include <cuda.h>
 #include "tf_penta.cuh"
 #include "tf_bwd.cuh"
+#include "tf_fwd.cuh"
 
 #include <atomic>
 #include <cmath>
@@ -187,6 +188,10 @@ cudaError_t launch_xbwd(int nx, int ny, const double* alT, const double* beT, co
     return cudaGetLastError();
 }
 
+constexpr int YW_NP = 4, YW_RP = 8, YW_NSTG = 2;   // yfwd: 4 producer warps x 8 rows per tile, 2 stages (80 KiB)
+
+constexpr int XW_NP = 4, XW_NSTG = 2;              // xfwd: 4 producer warps x 8 rows per 28-column tile, 2 stages (72 KiB)
+
 // one pseudo-Newton iteration k: reads src (u^n if k == 0 else uk), writes uk, red[2k..2k+1]
 template <int N, int M>
 cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
@@ -197,17 +202,37 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
     const int gy = (P.nx + YF_VALID - 1) / YF_VALID;
     cudaEvent_t* ev = (c->profiling && slot >= 0) ? c->ev + 5 * slot : nullptr;
     if (ev) cudaEventRecord(ev[0], c->stream);
-    if (k == 0)
-        yfwd_kernel<N, M, true><<<gy, 32, 0, c->stream>>>(P, DX, DY, src, c->bn, c->al, c->be, c->zz);
-    else
-        yfwd_kernel<N, M, false><<<gy, 32, 0, c->stream>>>(P, DX, DY, src, c->bn, c->al, c->be, c->zz);
+    {
+        constexpr size_t SM = (size_t)YW_NSTG * 5 * YW_NP * YW_RP * 32 * 8 + 16 * YW_NSTG;
+        static bool ready = false;
+        if (!ready) {
+            cudaError_t e = opt_in_smem(yfwd_ws_kernel<N, M, true, YW_NP, YW_RP, YW_NSTG>, SM);
+            if (e == cudaSuccess) e = opt_in_smem(yfwd_ws_kernel<N, M, false, YW_NP, YW_RP, YW_NSTG>, SM);
+            if (e != cudaSuccess) return e;
+            ready = true;
+        }
+        const int nthr = 32 * (YW_NP + 1);
+        if (k == 0)
+            yfwd_ws_kernel<N, M, true, YW_NP, YW_RP, YW_NSTG><<<gy, nthr, SM, c->stream>>>(P, DX, DY, src, c->bn, c->al, c->be, c->zz);
+        else
+            yfwd_ws_kernel<N, M, false, YW_NP, YW_RP, YW_NSTG><<<gy, nthr, SM, c->stream>>>(P, DX, DY, src, c->bn, c->al, c->be, c->zz);
+    }
     if (ev) cudaEventRecord(ev[1], c->stream);
     cudaError_t le = c->tma_y ? launch_ybwd_tma(c->mY, P.nx, P.ny, c->w, c->stream)
                               : launch_ybwd(P.nx, P.ny, c->al, c->be, c->zz, c->w, c->stream);
     if (le != cudaSuccess) return le;
     if (ev) cudaEventRecord(ev[2], c->stream);
     const int gx = (P.ny + XT - 1) / XT;
-    xfwd_kernel<N, M><<<gx, 32, 0, c->stream>>>(P, DX, src, c->w, c->al, c->be, c->zz);
+    {
+        constexpr size_t SM = (size_t)XW_NSTG * 5 * XW_CT * XW_LD * 8 + 16 * XW_NSTG;
+        static bool ready = false;
+        if (!ready) {
+            cudaError_t e = opt_in_smem(xfwd_ws_kernel<N, M, XW_NP, XW_NSTG>, SM);
+            if (e != cudaSuccess) return e;
+            ready = true;
+        }
+        xfwd_ws_kernel<N, M, XW_NP, XW_NSTG><<<gx, 32 * (XW_NP + 1), SM, c->stream>>>(P, DX, src, c->w, c->al, c->be, c->zz);
+    }
     if (ev) cudaEventRecord(ev[3], c->stream);
     if (c->tma_x)
         le = launch_xbwd_tma(c->mX, c->mU[src == c->ubuf[0] ? 0 : 1], c->mU[c->uk == c->ubuf[0] ? 0 : 1], P.nx, P.ny,
