@@ -183,14 +183,25 @@ ybwd_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__ 
         const int s = q % NST;
         mbar_wait(full + s, (q / NST) & 1);
         const int j0 = (ntile - 1 - q) * RS;
-        const double* d = sm + (size_t)s * 3 * BOX;
-        double* wp = w + (size_t)j0 * nx + i;
+        const double* d = sm + (size_t)s * 3 * BOX + lane;
+        if (j0 + RS <= ny) {                                 // full tile: branch-free, one running pointer
+            double* wp = w + (size_t)(j0 + RS - 1) * nx + i;
 #pragma unroll
-        for (int r = RS - 1; r >= 0; --r) {
-            if (j0 + r < ny) {
-                const double x = fma(-d[r * 32 + lane], w1, fma(-d[BOX + r * 32 + lane], w2, d[2 * BOX + r * 32 + lane]));
-                if (i < nx) wp[(size_t)r * nx] = x;
+            for (int r = RS - 1; r >= 0; --r) {
+                const double x = fma(-d[r * 32], w1, fma(-d[BOX + r * 32], w2, d[2 * BOX + r * 32]));
+                if (i < nx) *wp = x;
+                wp -= nx;
                 w2 = w1; w1 = x;
+            }
+        } else {
+            double* wp = w + (size_t)j0 * nx + i;
+#pragma unroll
+            for (int r = RS - 1; r >= 0; --r) {
+                if (j0 + r < ny) {
+                    const double x = fma(-d[r * 32], w1, fma(-d[BOX + r * 32], w2, d[2 * BOX + r * 32]));
+                    if (i < nx) wp[(size_t)r * nx] = x;
+                    w2 = w1; w1 = x;
+                }
             }
         }
         __syncwarp();
@@ -244,22 +255,37 @@ xbwd_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__ 
         mbar_wait(full + s, (q / NST) & 1);
         const int i0 = (ntile - 1 - q) * CS, cols_ok = min(CS, nx - i0);
         unsigned char* d = base + (size_t)s * STAGE;
-        const double* cf = reinterpret_cast<const double*>(d);
+        const double* cf = reinterpret_cast<const double*>(d) + lane;
         unsigned char* su = d + 3 * BOX * 8;
+        unsigned char* sur = su + lane * 128;                // this lane's swizzled row
+        const int sx = (lane & 7) << 4;
+        if (cols_ok == CS) {                                 // full tile: branch-free
 #pragma unroll
-        for (int c = CS - 1; c >= 0; --c) {
-            if (c < cols_ok) {
-                const double v = fma(-cf[c * 32 + lane], v1, fma(-cf[BOX + c * 32 + lane], v2, cf[2 * BOX + c * 32 + lane]));
-                double* pu = reinterpret_cast<double*>(su + swz128(lane, c));
+            for (int c = CS - 1; c >= 0; --c) {
+                const double v = fma(-cf[c * 32], v1, fma(-cf[BOX + c * 32], v2, cf[2 * BOX + c * 32]));
+                double* pu = reinterpret_cast<double*>(sur + ((((c >> 1) << 4) ^ sx) + ((c & 1) << 3)));
                 const double uo = *pu;
                 const double un = uo + v;
-                const double rr = fabs(v / uo);
-                if (rowok) {
-                    if (!(rr <= res)) res = rr;              // NaN sticks
-                    if (!(un > 0.0) || isinf(un)) bad = 1;
-                }
+                const double rr = fabs(v) * rcp(uo);
+                res = fmax(res, rowok ? rr : 0.0);           // a NaN/inf iterate is caught by `bad`
+                bad |= (rowok && !(un > 0.0 && un <= 1.7976931348623157e308)) ? 1 : 0;
                 *pu = un;
                 v2 = v1; v1 = v;
+            }
+        } else {
+#pragma unroll
+            for (int c = CS - 1; c >= 0; --c) {
+                if (c < cols_ok) {
+                    const double v = fma(-cf[c * 32], v1, fma(-cf[BOX + c * 32], v2, cf[2 * BOX + c * 32]));
+                    double* pu = reinterpret_cast<double*>(su + swz128(lane, c));
+                    const double uo = *pu;
+                    const double un = uo + v;
+                    const double rr = fabs(v) * rcp(uo);
+                    res = fmax(res, rowok ? rr : 0.0);
+                    bad |= (rowok && !(un > 0.0 && un <= 1.7976931348623157e308)) ? 1 : 0;
+                    *pu = un;
+                    v2 = v1; v1 = v;
+                }
             }
         }
         fence_proxy_async();

@@ -30,7 +30,18 @@ __device__ __forceinline__ int clampi(int k, int lo, int hi) { return k < lo ? l
 // reflected then clamped: safe address for any k, exact ghost for k in [-N, 2N)
 __device__ __forceinline__ int ghost(int k, int N) { return clampi(refl(k, N), 0, N - 1); }
 
-__device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
+// Reciprocal on the critical path of every recurrence (pivot 1/mu) and of every cell (1/h):
+// MUFU.RCP64H seed (rel. error ~1.5e-7 measured) + one cubically convergent step y(1 + e + e^2):
+// 20 + 3x8 cycles of dependent latency instead of ~72 for the IEEE division sequence, error <= 1 ulp.
+// Arguments are positive normal numbers here (h > 0 is validated; pivots of I + sJ are ~1..2).
+__device__ __forceinline__ double rcp(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    const double t = fma(e, e, e);
+    return fma(y, t, y);
+}
 
 struct Cell { double f0, f1, g0, g1; };
 

@@ -28,7 +28,8 @@ struct YState {
 
 // MODE 0: bring in cell (j+1) only;  1: also face j+1/2;  2: also produce row j (bands + R).
 // out5 = {A_{j+1/2}, c, q, a, R}
-template <int N, int M, int MODE>
+// INTERIOR: all faces touched are interior and unfolded (1 <= j <= ny-3): no boundary logic at all.
+template <int N, int M, int MODE, bool INTERIOR>
 __device__ __forceinline__ void y_advance(YState& S, int j, double hp2, const Params& P, const Dir& DX, const Dir& DY,
                                           bool xface, double rhs_in, double* out5, double& sD_out)
 {
@@ -45,9 +46,11 @@ __device__ __forceinline__ void y_advance(YState& S, int j, double hp2, const Pa
         const double sf0 = S.c0.f0 + cp.f0, sf1 = S.c0.f1 + cp.f1;
         fp = face_partials(S.hm1, hp2, dh, sf0, sf1, S.c0, cp, DY);
         phip = DY.cb * fma(sf0, Lp - S.L0, sf1 * dh);
-        if (j == 0) fp.p1 -= fp.A;
-        if (j == ny - 2) fp.p2 += fp.A;
-        if (!yface) { fp.A = 0.0; fp.p1 = 0.0; fp.p2 = 0.0; phip = 0.0; }
+        if (!INTERIOR) {
+            if (j == 0) fp.p1 -= fp.A;
+            if (j == ny - 2) fp.p2 += fp.A;
+            if (!yface) { fp.A = 0.0; fp.p1 = 0.0; fp.p2 = 0.0; phip = 0.0; }
+        }
     }
     if (MODE == 2) {
         const double f0R = __shfl_down_sync(FULL, S.c0.f0, 1), f1R = __shfl_down_sync(FULL, S.c0.f1, 1);
@@ -100,28 +103,52 @@ yfwd_ws_kernel(Params P, Dir DX, Dir DY, const double* __restrict__ u, double* _
         for (int t = 0; t < ntile; ++t) {
             const int s = t % NSTG;
             const int j0 = t * RT + warp * RP;
+            const bool interior = (j0 >= 2) && (j0 + RP + 1 <= ny - 2);
             double hq[RP + 4], bq[RP];
-            if (j0 < ny) {
+            if (interior) {
+                const double* hp = up + (size_t)(j0 - 2) * nx;
+#pragma unroll
+                for (int k = 0; k < RP + 4; ++k) hq[k] = hp[(size_t)k * nx];
+                const double* bq0 = bp + (size_t)j0 * nx;
+#pragma unroll
+                for (int k = 0; k < RP; ++k) bq[k] = FIRST ? 0.0 : bq0[(size_t)k * nx];
+            } else if (j0 < ny) {
 #pragma unroll
                 for (int k = 0; k < RP + 4; ++k) hq[k] = up[(size_t)ghost(j0 - 2 + k, ny) * nx];
 #pragma unroll
                 for (int k = 0; k < RP; ++k) bq[k] = FIRST ? 0.0 : bp[(size_t)clampi(j0 + k, 0, ny - 1) * nx];
             }
             mbar_wait(empty + s, ((t / NSTG) & 1) ^ 1);
-            if (j0 < ny) {
-                YState S;
-                S.hm1 = 0.0; S.h0 = hq[0]; S.hp1 = hq[1]; S.hR0 = 0.0;
-                S.c0 = {0, 0, 0, 0}; S.L0 = 0.0; S.fm = {0, 0, 0}; S.phim = 0.0;
-                double o5[5], sD;
-                y_advance<N, M, 0>(S, j0 - 2, hq[2], P, DX, DY, xface, 0.0, o5, sD);
-                y_advance<N, M, 1>(S, j0 - 1, hq[3], P, DX, DY, xface, 0.0, o5, sD);
-                double* st = sm + (size_t)s * 5 * SV + (warp * RP) * 32 + lane;
+            double* st = sm + (size_t)s * 5 * SV + (warp * RP) * 32 + lane;
+            YState S;
+            S.hm1 = 0.0; S.h0 = hq[0]; S.hp1 = hq[1]; S.hR0 = 0.0;
+            S.c0 = {0, 0, 0, 0}; S.L0 = 0.0; S.fm = {0, 0, 0}; S.phim = 0.0;
+            double o5[5], sD;
+            if (interior) {
+                y_advance<N, M, 0, true>(S, j0 - 2, hq[2], P, DX, DY, xface, 0.0, o5, sD);
+                y_advance<N, M, 1, true>(S, j0 - 1, hq[3], P, DX, DY, xface, 0.0, o5, sD);
+                double* bo = bn + (size_t)j0 * nx + i;
+#pragma unroll
+                for (int r = 0; r < RP; ++r) {
+                    const double hcur = S.h0;
+                    y_advance<N, M, 2, true>(S, j0 + r, hq[r + 4], P, DX, DY, xface, FIRST ? hcur : bq[r], o5, sD);
+                    if (FIRST) {
+                        const double b = hcur - sD;
+                        if (outl) bo[(size_t)r * nx] = b;
+                        o5[4] = (b - hcur) - sD;
+                    }
+#pragma unroll
+                    for (int v = 0; v < 5; ++v) st[v * SV + r * 32] = o5[v];
+                }
+            } else if (j0 < ny) {
+                y_advance<N, M, 0, false>(S, j0 - 2, hq[2], P, DX, DY, xface, 0.0, o5, sD);
+                y_advance<N, M, 1, false>(S, j0 - 1, hq[3], P, DX, DY, xface, 0.0, o5, sD);
 #pragma unroll
                 for (int r = 0; r < RP; ++r) {
                     const int j = j0 + r;
                     if (j < ny) {
                         const double hcur = S.h0;
-                        y_advance<N, M, 2>(S, j, hq[r + 4], P, DX, DY, xface, FIRST ? hcur : bq[r], o5, sD);
+                        y_advance<N, M, 2, false>(S, j, hq[r + 4], P, DX, DY, xface, FIRST ? hcur : bq[r], o5, sD);
                         if (FIRST) {
                             const double b = hcur - sD;
                             if (outl) bn[(size_t)j * nx + i] = b;
@@ -147,14 +174,27 @@ yfwd_ws_kernel(Params P, Dir DX, Dir DY, const double* __restrict__ u, double* _
             const int jt = t * RT;
             const int nrow = min(RT, ny - jt);
             size_t o = (size_t)jt * nx + i;
-            for (int r = 0; r < nrow; ++r) {
-                const double A = st[r * 32], c = st[SV + r * 32], q = st[2 * SV + r * 32], a = st[3 * SV + r * 32];
-                const double R = st[4 * SV + r * 32];
-                double va, vb, vz;
-                elim_row(S, e, c, q, a, A, R, va, vb, vz);
-                e = A;
-                if (outl) { al[o] = va; be[o] = vb; zz[o] = vz; }
-                o += nx;
+            if (nrow == RT) {
+#pragma unroll 8
+                for (int r = 0; r < RT; ++r) {
+                    const double A = st[r * 32], c = st[SV + r * 32], q = st[2 * SV + r * 32], a = st[3 * SV + r * 32];
+                    const double R = st[4 * SV + r * 32];
+                    double va, vb, vz;
+                    elim_row(S, e, c, q, a, A, R, va, vb, vz);
+                    e = A;
+                    if (outl) { al[o] = va; be[o] = vb; zz[o] = vz; }
+                    o += nx;
+                }
+            } else {
+                for (int r = 0; r < nrow; ++r) {
+                    const double A = st[r * 32], c = st[SV + r * 32], q = st[2 * SV + r * 32], a = st[3 * SV + r * 32];
+                    const double R = st[4 * SV + r * 32];
+                    double va, vb, vz;
+                    elim_row(S, e, c, q, a, A, R, va, vb, vz);
+                    e = A;
+                    if (outl) { al[o] = va; be[o] = vb; zz[o] = vz; }
+                    o += nx;
+                }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(empty + s);
