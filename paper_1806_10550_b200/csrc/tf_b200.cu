@@ -44,6 +44,7 @@ struct tf_ctx {
     double *part;                              // [RED_BLOCKS]
     double *scal;                              // [8] : scal[0] mass, (int*)(scal+1) flag
     double *pinned;                            // [4] host pinned readback
+    int mid_y, mid_x;                          // split rows / columns of the two-sided sweeps
     bool tma_y, tma_x;                         // TMA rings usable (row pitch multiple of 16 B, grid >= one box)
     CUtensorMap mY[3], mX[3];                  // alpha,beta,z as [ny][nx] (box RS x 32) and as [nx][ny] (box CS x 32)
     CUtensorMap mU[2];                         // the two state buffers as [ny][nx], box 32 x 16, 128-byte swizzle
@@ -138,6 +139,26 @@ cudaError_t launch_ybwd_tma(const CUtensorMap* m, int nx, int ny, double* w, cud
     return cudaGetLastError();
 }
 
+// two-sided y back substitution (the y forward kernel is two-sided): TMA ring when the maps exist, else plain
+cudaError_t launch_ybwd2(const CUtensorMap* m, bool tma, int nx, int ny, int mid, const double* al, const double* be,
+                         const double* zz, double* w, cudaStream_t st)
+{
+    const dim3 g((nx + 31) / 32, 2);
+    if (!tma) {
+        ybwd2_plain_kernel<<<g, 32, 0, st>>>(nx, ny, mid, al, be, zz, w);
+        return cudaGetLastError();
+    }
+    constexpr size_t SM = (size_t)YT_NST * 3 * YT_RS * 32 * 8 + 8 * YT_NST + 1024;
+    static bool ready = false;
+    if (!ready) {
+        cudaError_t e = opt_in_smem(ybwd2_tma_kernel<YT_NST, YT_RS>, SM);
+        if (e != cudaSuccess) return e;
+        ready = true;
+    }
+    ybwd2_tma_kernel<YT_NST, YT_RS><<<g, 32, SM, st>>>(m[0], m[1], m[2], nx, ny, mid, al, be, zz, w);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_xbwd_tma(const CUtensorMap* m, const CUtensorMap& uin, const CUtensorMap& uout, int nx, int ny,
                             double* red, cudaStream_t st)
 {
@@ -149,6 +170,27 @@ cudaError_t launch_xbwd_tma(const CUtensorMap* m, const CUtensorMap& uin, const 
         ready = true;
     }
     xbwd_tma_kernel<XT_NST><<<(ny + 31) / 32, 32, SM, st>>>(m[0], m[1], m[2], uin, uout, nx, ny, red);
+    return cudaGetLastError();
+}
+
+// two-sided x back substitution + update + residual
+cudaError_t launch_xbwd2(const CUtensorMap* m, const CUtensorMap& uin, const CUtensorMap& uout, bool tma, int nx, int ny,
+                         int mid, const double* alT, const double* beT, const double* zzT, const double* uk,
+                         double* unew, double* red, cudaStream_t st)
+{
+    const dim3 g((ny + 31) / 32, 2);
+    if (!tma) {
+        xbwd2_plain_kernel<<<g, 32, 0, st>>>(nx, ny, mid, alT, beT, zzT, uk, unew, red);
+        return cudaGetLastError();
+    }
+    constexpr size_t SM = (size_t)XT_NST * 4 * 16 * 32 * 8 + 8 * XT_NST + 1024;
+    static bool ready = false;
+    if (!ready) {
+        cudaError_t e = opt_in_smem(xbwd2_tma_kernel<XT_NST>, SM);
+        if (e != cudaSuccess) return e;
+        ready = true;
+    }
+    xbwd2_tma_kernel<XT_NST><<<g, 32, SM, st>>>(m[0], m[1], m[2], uin, uout, nx, ny, mid, alT, beT, zzT, red);
     return cudaGetLastError();
 }
 
@@ -188,9 +230,9 @@ cudaError_t launch_xbwd(int nx, int ny, const double* alT, const double* beT, co
     return cudaGetLastError();
 }
 
-constexpr int YW_NP = 4, YW_RP = 8, YW_NSTG = 2;   // yfwd: 4 producer warps x 8 rows per tile, 2 stages (80 KiB)
+constexpr int YW_NP = 3, YW_RP = 8, YW_NSTG = 4;   // yfwd: consumer warp 0 + 3 producer warps, chunks of 8 rows, ring of 4 chunk slots (40 KiB)
 
-constexpr int XW_NP = 4, XW_NSTG = 2;              // xfwd: 4 producer warps x 8 rows per 28-column tile, 2 stages (72 KiB)
+constexpr int XW_NP = 3, XW_NSTG = 3;              // xfwd: per sub-problem 1 consumer + 3 producer warps, ring of 3 slots of 14 columns (48 KiB)
 
 // one pseudo-Newton iteration k: reads src (u^n if k == 0 else uk), writes uk, red[2k..2k+1]
 template <int N, int M>
@@ -199,11 +241,11 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
     const Params& P = c->P;
     const Dir DX = make_dir(s, P.dx), DY = make_dir(s, P.dy);
     const double* src = (k == 0) ? c->u : c->uk;
-    const int gy = (P.nx + YF_VALID - 1) / YF_VALID;
+    const int gy = ((P.nx + YW_VALID - 1) / YW_VALID + 1) / 2;     // one CTA = two strips x two halves
     cudaEvent_t* ev = (c->profiling && slot >= 0) ? c->ev + 5 * slot : nullptr;
     if (ev) cudaEventRecord(ev[0], c->stream);
     {
-        constexpr size_t SM = (size_t)YW_NSTG * 5 * YW_NP * YW_RP * 32 * 8 + 16 * YW_NSTG;
+        constexpr size_t SM = 4 * ((size_t)YW_NSTG * 5 * YW_RP * 32 * 8 + 16 * YW_NSTG);
         static bool ready = false;
         if (!ready) {
             cudaError_t e = opt_in_smem(yfwd_ws_kernel<N, M, true, YW_NP, YW_RP, YW_NSTG>, SM);
@@ -211,34 +253,30 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
             if (e != cudaSuccess) return e;
             ready = true;
         }
-        const int nthr = 32 * (YW_NP + 1);
+        const int nthr = 128 * (YW_NP + 1);
         if (k == 0)
-            yfwd_ws_kernel<N, M, true, YW_NP, YW_RP, YW_NSTG><<<gy, nthr, SM, c->stream>>>(P, DX, DY, src, c->bn, c->al, c->be, c->zz);
+            yfwd_ws_kernel<N, M, true, YW_NP, YW_RP, YW_NSTG><<<gy, nthr, SM, c->stream>>>(P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz);
         else
-            yfwd_ws_kernel<N, M, false, YW_NP, YW_RP, YW_NSTG><<<gy, nthr, SM, c->stream>>>(P, DX, DY, src, c->bn, c->al, c->be, c->zz);
+            yfwd_ws_kernel<N, M, false, YW_NP, YW_RP, YW_NSTG><<<gy, nthr, SM, c->stream>>>(P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz);
     }
     if (ev) cudaEventRecord(ev[1], c->stream);
-    cudaError_t le = c->tma_y ? launch_ybwd_tma(c->mY, P.nx, P.ny, c->w, c->stream)
-                              : launch_ybwd(P.nx, P.ny, c->al, c->be, c->zz, c->w, c->stream);
+    cudaError_t le = launch_ybwd2(c->mY, c->tma_y, P.nx, P.ny, c->mid_y, c->al, c->be, c->zz, c->w, c->stream);
     if (le != cudaSuccess) return le;
     if (ev) cudaEventRecord(ev[2], c->stream);
-    const int gx = (P.ny + XT - 1) / XT;
+    const int gx = ((P.ny + XW_R - 1) / XW_R + 1) / 2;           // one CTA = two row blocks x two halves
     {
-        constexpr size_t SM = (size_t)XW_NSTG * 5 * XW_CT * XW_LD * 8 + 16 * XW_NSTG;
+        constexpr size_t SM = 4 * ((size_t)XW_NSTG * 5 * XW_CK * XW_LD * 8 + 16 * XW_NSTG);
         static bool ready = false;
         if (!ready) {
             cudaError_t e = opt_in_smem(xfwd_ws_kernel<N, M, XW_NP, XW_NSTG>, SM);
             if (e != cudaSuccess) return e;
             ready = true;
         }
-        xfwd_ws_kernel<N, M, XW_NP, XW_NSTG><<<gx, 32 * (XW_NP + 1), SM, c->stream>>>(P, DX, src, c->w, c->al, c->be, c->zz);
+        xfwd_ws_kernel<N, M, XW_NP, XW_NSTG><<<gx, 128 * (XW_NP + 1), SM, c->stream>>>(P, DX, c->mid_x, src, c->w, c->al, c->be, c->zz);
     }
     if (ev) cudaEventRecord(ev[3], c->stream);
-    if (c->tma_x)
-        le = launch_xbwd_tma(c->mX, c->mU[src == c->ubuf[0] ? 0 : 1], c->mU[c->uk == c->ubuf[0] ? 0 : 1], P.nx, P.ny,
-                             c->red + 2 * k, c->stream);
-    else
-        le = launch_xbwd(P.nx, P.ny, c->al, c->be, c->zz, src, c->uk, c->red + 2 * k, c->stream);
+    le = launch_xbwd2(c->mX, c->mU[src == c->ubuf[0] ? 0 : 1], c->mU[c->uk == c->ubuf[0] ? 0 : 1], c->tma_x, P.nx, P.ny,
+                      c->mid_x, c->al, c->be, c->zz, src, c->uk, c->red + 2 * k, c->stream);
     if (le != cudaSuccess) return le;
     if (ev) cudaEventRecord(ev[4], c->stream);
     count_launch(4);
@@ -321,8 +359,11 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
         return fail(nullptr, TF_ERR_ALLOC, std::string("cudaMallocHost: ") + cudaGetErrorString(e));
     }
     c->ubuf[0] = c->u; c->ubuf[1] = c->uk;
+    // split index of the two-sided sweeps: half the line, on a 16-row tile boundary when the line is long enough
+    c->mid_y = ny >= 64 ? (ny / 2) / 16 * 16 : ny / 2;
+    c->mid_x = nx >= 64 ? (nx / 2) / 16 * 16 : nx / 2;
     c->tma_y = (nx % 2 == 0) && nx >= 32 && ny >= YT_RS;
-    c->tma_x = (nx % 2 == 0) && (ny % 2 == 0) && nx >= 16 && ny >= 32;
+    c->tma_x = (nx % 2 == 0) && (ny % 2 == 0) && nx >= 64 && ny >= 32 && (c->mid_x % 16 == 0);
     if (c->tma_y) {
         const double* f3[3] = {c->al, c->be, c->zz};
         for (int k = 0; k < 3; ++k) c->tma_y = c->tma_y && make_map2d(&c->mY[k], f3[k], nx, ny, 32, YT_RS, false);

@@ -209,6 +209,157 @@ ybwd_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__ 
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Two-sided back substitution (pairs with the two-sided forward kernels of tf_fwd.cuh).
+// The forward pass left, for a line x_0 .. x_{N-1} split at mid:
+//   k <  mid :  x_k = z_k - al_k x_{k+1} - be_k x_{k+2}        (eliminated from the low end)
+//   k >= mid :  x_k = z_k - al_k x_{k-1} - be_k x_{k-2}        (eliminated from the high end)
+// The four unknowns around the split, (p,q,r,s) = x_{mid-2}, x_{mid-1}, x_mid, x_{mid+1}, satisfy the rows
+// mid-2 .. mid+1 of these relations: a 4x4 system, reduced to 2x2 by substituting p and s.
+// ---------------------------------------------------------------------------------------------
+struct Join { double p, q, r, s; };
+
+// c[3*k + {0,1,2}] = al, be, z of row mid-2+k
+__device__ __forceinline__ Join babe_join(const double* c)
+{
+    const double a1 = c[0], b1 = c[1], z1 = c[2], a2 = c[3], b2 = c[4], z2 = c[5];
+    const double a3 = c[6], b3 = c[7], z3 = c[8], a4 = c[9], b4 = c[10], z4 = c[11];
+    const double A11 = fma(-b3, a1, a3), A12 = fma(-b3, b1, 1.0), rA = fma(-b3, z1, z3);
+    const double B21 = fma(-b2, b4, 1.0), B22 = fma(-b2, a4, a2), rB = fma(-b2, z4, z2);
+    const double det = A11 * B22 - A12 * B21;
+    Join J;
+    J.q = (rA * B22 - A12 * rB) / det;
+    J.r = (A11 * rB - rA * B21) / det;
+    J.p = z1 - a1 * J.q - b1 * J.r;
+    J.s = z4 - b4 * J.q - a4 * J.r;
+    return J;
+}
+
+// y direction: coefficient fields [ny][nx], lane <-> column.  grid (ceil(nx/32), 2): blockIdx.y = half.
+template <int NST, int RS>
+__global__ void __launch_bounds__(32)
+ybwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__ CUtensorMap mB,
+                 const __grid_constant__ CUtensorMap mZ, int nx, int ny, int mid, const double* __restrict__ al,
+                 const double* __restrict__ be, const double* __restrict__ zz, double* __restrict__ w)
+{
+    extern __shared__ unsigned char raw[];
+    unsigned char* base = align1024(raw);
+    constexpr int BOX = RS * 32;                             // doubles per box
+    double* sm = reinterpret_cast<double*>(base);            // [NST][3][RS][32]
+    uint64_t* full = reinterpret_cast<uint64_t*>(base + (size_t)NST * 3 * BOX * 8);
+    const int lane = threadIdx.x;
+    const int i0 = blockIdx.x * 32, i = i0 + lane;
+    const int dir = blockIdx.y;
+    const bool colok = i < nx;
+    const int nrows = dir ? ny - mid : mid;
+    const int ntile = (nrows + RS - 1) / RS;
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < NST; ++s) mbar_init(full + s, 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+    // first row of the box of the q-th tile in marching order (may be < 0 or reach past ny: TMA zero-fills)
+    auto box_row = [&](int q) { return dir ? mid + q * RS : mid - (q + 1) * RS; };
+    auto issue = [&](int q) {
+        if (q < ntile && lane == 0) {
+            const int s = q % NST;
+            double* d = sm + (size_t)s * 3 * BOX;
+            mbar_expect_tx(full + s, 3 * BOX * 8);
+            tma_load_2d(d, &mA, i0, box_row(q), full + s);
+            tma_load_2d(d + BOX, &mB, i0, box_row(q), full + s);
+            tma_load_2d(d + 2 * BOX, &mZ, i0, box_row(q), full + s);
+        }
+    };
+#pragma unroll
+    for (int q = 0; q < NST; ++q) issue(q);
+    // interface solve (both halves do it; each keeps the two unknowns on the other side of the split)
+    double c12[12];
+    {
+        const size_t o = (size_t)(mid - 2) * nx + min(i, nx - 1);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            c12[3 * k] = al[o + (size_t)k * nx]; c12[3 * k + 1] = be[o + (size_t)k * nx]; c12[3 * k + 2] = zz[o + (size_t)k * nx];
+        }
+    }
+    const Join J = babe_join(c12);
+    double w1 = dir ? J.q : J.r, w2 = dir ? J.p : J.s;
+    for (int q = 0; q < ntile; ++q) {
+        const int s = q % NST;
+        mbar_wait(full + s, (q / NST) & 1);
+        const int jb = box_row(q);
+        const double* d = sm + (size_t)s * 3 * BOX + lane;
+        if (dir == 0) {
+            if (jb >= 0) {                                   // full tile: branch-free, one running pointer
+                double* wp = w + (size_t)(jb + RS - 1) * nx + i;
+#pragma unroll
+                for (int r = RS - 1; r >= 0; --r) {
+                    const double x = fma(-d[r * 32], w1, fma(-d[BOX + r * 32], w2, d[2 * BOX + r * 32]));
+                    st_if(colok, wp, x);
+                    wp -= nx;
+                    w2 = w1; w1 = x;
+                }
+            } else {
+#pragma unroll
+                for (int r = RS - 1; r >= 0; --r) {
+                    if (jb + r >= 0) {
+                        const double x = fma(-d[r * 32], w1, fma(-d[BOX + r * 32], w2, d[2 * BOX + r * 32]));
+                        if (colok) w[(size_t)(jb + r) * nx + i] = x;
+                        w2 = w1; w1 = x;
+                    }
+                }
+            }
+        } else {
+            if (jb + RS <= ny) {
+                double* wp = w + (size_t)jb * nx + i;
+#pragma unroll
+                for (int r = 0; r < RS; ++r) {
+                    const double x = fma(-d[r * 32], w1, fma(-d[BOX + r * 32], w2, d[2 * BOX + r * 32]));
+                    st_if(colok, wp, x);
+                    wp += nx;
+                    w2 = w1; w1 = x;
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < RS; ++r) {
+                    if (jb + r < ny) {
+                        const double x = fma(-d[r * 32], w1, fma(-d[BOX + r * 32], w2, d[2 * BOX + r * 32]));
+                        if (colok) w[(size_t)(jb + r) * nx + i] = x;
+                        w2 = w1; w1 = x;
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        issue(q + NST);
+    }
+}
+
+// Plain fallback of the same two-sided back substitution (any nx, ny; no TMA): lane <-> column, direct loads.
+__global__ void __launch_bounds__(32)
+ybwd2_plain_kernel(int nx, int ny, int mid, const double* __restrict__ al, const double* __restrict__ be,
+                   const double* __restrict__ zz, double* __restrict__ w)
+{
+    const int i = blockIdx.x * 32 + threadIdx.x;
+    const int dir = blockIdx.y;
+    if (i >= nx) return;
+    double c12[12];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const size_t o = (size_t)(mid - 2 + k) * nx + i;
+        c12[3 * k] = al[o]; c12[3 * k + 1] = be[o]; c12[3 * k + 2] = zz[o];
+    }
+    const Join J = babe_join(c12);
+    double w1 = dir ? J.q : J.r, w2 = dir ? J.p : J.s;
+    const int nrows = dir ? ny - mid : mid;
+    for (int k = 0; k < nrows; ++k) {
+        const size_t o = (size_t)(dir ? mid + k : mid - 1 - k) * nx + i;
+        const double x = fma(-al[o], w1, fma(-be[o], w2, zz[o]));
+        w[o] = x;
+        w2 = w1; w1 = x;
+    }
+}
+
 // byte offset of element (r, c) in a [32][16] fp64 tile written by TMA with CU_TENSOR_MAP_SWIZZLE_128B
 __device__ __forceinline__ int swz128(int r, int c) { return r * 128 + ((((c >> 1) ^ (r & 7))) << 4) + ((c & 1) << 3); }
 
@@ -299,6 +450,160 @@ xbwd_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__ 
         issue(q + NST - 1);                                  // refill the stage of tile q-1
     }
     if (lane == 0) tma_store_wait_all<0>();
+    if (res != res) res = __longlong_as_double(0x7ff8000000000000LL);
+    res = warp_max_nonneg(res);
+    bad = __any_sync(0xffffffffu, bad);
+    if (lane == 0) {
+        atomic_max_nonneg(red, res);
+        if (bad) atomic_max_nonneg(red + 1, 1.0);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// x direction, two-sided: coefficient fields transposed [nx][ny], lane <-> row j; then S7: u_{k+1} = u_k + v,
+// res = max|v/u_k| ((2.21)-(2.22)).  grid (ceil(ny/32), 2): blockIdx.y = half.
+// Half 0 marches columns mid-1 .. 0, half 1 columns mid .. nx-1; mid is a multiple of the tile width (16),
+// so the u tiles of the two halves (TMA load, in-place update, TMA store) never overlap.
+// ---------------------------------------------------------------------------------------------
+template <int NST>
+__global__ void __launch_bounds__(32)
+xbwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__ CUtensorMap mB,
+                 const __grid_constant__ CUtensorMap mZ, const __grid_constant__ CUtensorMap mUin,
+                 const __grid_constant__ CUtensorMap mUout, int nx, int ny, int mid, const double* __restrict__ alT,
+                 const double* __restrict__ beT, const double* __restrict__ zzT, double* __restrict__ red)
+{
+    constexpr int CS = 16;                                   // columns per stage (= one 128-byte swizzled row)
+    constexpr int BOX = CS * 32;                             // doubles per coefficient box
+    constexpr int STAGE = 4 * BOX * 8;                       // bytes per stage: 3 coefficient boxes + the u tile
+    extern __shared__ unsigned char raw[];
+    unsigned char* base = align1024(raw);
+    uint64_t* full = reinterpret_cast<uint64_t*>(base + (size_t)NST * STAGE);
+    const int lane = threadIdx.x;
+    const int j0 = blockIdx.x * 32;
+    const int dir = blockIdx.y;
+    const bool rowok = j0 + lane < ny;
+    const int ncols = dir ? nx - mid : mid;
+    const int ntile = (ncols + CS - 1) / CS;
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < NST; ++s) mbar_init(full + s, 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+    auto tile_col = [&](int q) { return dir ? mid + q * CS : mid - (q + 1) * CS; };
+    auto issue = [&](int q) {
+        if (q < ntile && lane == 0) {
+            const int s = q % NST;
+            unsigned char* d = base + (size_t)s * STAGE;
+            const int i0 = tile_col(q);
+            mbar_expect_tx(full + s, STAGE);
+            tma_load_2d(d, &mA, j0, i0, full + s);
+            tma_load_2d(d + BOX * 8, &mB, j0, i0, full + s);
+            tma_load_2d(d + 2 * BOX * 8, &mZ, j0, i0, full + s);
+            tma_load_2d(d + 3 * BOX * 8, &mUin, i0, j0, full + s);
+        }
+    };
+#pragma unroll
+    for (int q = 0; q < NST - 1; ++q) issue(q);
+    double c12[12];
+    {
+        const size_t o = (size_t)(mid - 2) * ny + min(j0 + lane, ny - 1);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            c12[3 * k] = alT[o + (size_t)k * ny]; c12[3 * k + 1] = beT[o + (size_t)k * ny]; c12[3 * k + 2] = zzT[o + (size_t)k * ny];
+        }
+    }
+    const Join J = babe_join(c12);
+    double v1 = dir ? J.q : J.r, v2 = dir ? J.p : J.s;
+    double res = 0.0;
+    int bad = 0;
+    for (int q = 0; q < ntile; ++q) {
+        const int s = q % NST;
+        mbar_wait(full + s, (q / NST) & 1);
+        const int i0 = tile_col(q), cols_ok = min(CS, nx - i0);
+        unsigned char* d = base + (size_t)s * STAGE;
+        const double* cf = reinterpret_cast<const double*>(d) + lane;
+        unsigned char* su = d + 3 * BOX * 8;
+        unsigned char* sur = su + lane * 128;                // this lane's swizzled row
+        const int sx = (lane & 7) << 4;
+        auto column = [&](int c) {
+            const double v = fma(-cf[c * 32], v1, fma(-cf[BOX + c * 32], v2, cf[2 * BOX + c * 32]));
+            double* pu = reinterpret_cast<double*>(sur + ((((c >> 1) << 4) ^ sx) + ((c & 1) << 3)));
+            const double uo = *pu;
+            const double un = uo + v;
+            const double rr = fabs(v) * rcp(uo);
+            res = fmax(res, rowok ? rr : 0.0);               // a NaN/inf iterate is caught by `bad`
+            bad |= (rowok && !(un > 0.0 && un <= 1.7976931348623157e308)) ? 1 : 0;
+            *pu = un;
+            v2 = v1; v1 = v;
+        };
+        if (dir == 0) {                                      // always full tiles (mid is a multiple of CS)
+#pragma unroll
+            for (int c = CS - 1; c >= 0; --c) column(c);
+        } else if (cols_ok == CS) {
+#pragma unroll
+            for (int c = 0; c < CS; ++c) column(c);
+        } else {
+#pragma unroll
+            for (int c = 0; c < CS; ++c)
+                if (c < cols_ok) column(c);
+        }
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) {
+            tma_store_2d(&mUout, i0, j0, su);
+            tma_store_commit();
+            tma_store_wait_read<1>();                        // the store of tile q-1 has left shared memory
+        }
+        __syncwarp();
+        issue(q + NST - 1);                                  // refill the stage of tile q-1
+    }
+    if (lane == 0) tma_store_wait_all<0>();
+    if (res != res) res = __longlong_as_double(0x7ff8000000000000LL);
+    res = warp_max_nonneg(res);
+    bad = __any_sync(0xffffffffu, bad);
+    if (lane == 0) {
+        atomic_max_nonneg(red, res);
+        if (bad) atomic_max_nonneg(red + 1, 1.0);
+    }
+}
+
+// Plain fallback (any nx, ny): thread per row, direct loads (u accesses are strided: correctness path for
+// odd or tiny grids, not a fast path).  uk may alias unew.
+__global__ void __launch_bounds__(32)
+xbwd2_plain_kernel(int nx, int ny, int mid, const double* __restrict__ alT, const double* __restrict__ beT,
+                   const double* __restrict__ zzT, const double* uk, double* unew, double* __restrict__ red)
+{
+    const int lane = threadIdx.x;
+    const int j = blockIdx.x * 32 + lane;
+    const int dir = blockIdx.y;
+    const bool rowok = j < ny;
+    const int jc = min(j, ny - 1);
+    double c12[12];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const size_t o = (size_t)(mid - 2 + k) * ny + jc;
+        c12[3 * k] = alT[o]; c12[3 * k + 1] = beT[o]; c12[3 * k + 2] = zzT[o];
+    }
+    const Join J = babe_join(c12);
+    double v1 = dir ? J.q : J.r, v2 = dir ? J.p : J.s;
+    double res = 0.0;
+    int bad = 0;
+    const int ncols = dir ? nx - mid : mid;
+    for (int k = 0; k < ncols; ++k) {
+        const int i = dir ? mid + k : mid - 1 - k;
+        const size_t o = (size_t)i * ny + jc;
+        const double v = fma(-alT[o], v1, fma(-beT[o], v2, zzT[o]));
+        const double uo = uk[(size_t)jc * nx + i];
+        const double un = uo + v;
+        const double rr = fabs(v) * rcp(uo);
+        if (rowok) {
+            res = fmax(res, rr);
+            bad |= !(un > 0.0 && un <= 1.7976931348623157e308) ? 1 : 0;
+            unew[(size_t)j * nx + i] = un;
+        }
+        v2 = v1; v1 = v;
+    }
     if (res != res) res = __longlong_as_double(0x7ff8000000000000LL);
     res = warp_max_nonneg(res);
     bad = __any_sync(0xffffffffu, bad);

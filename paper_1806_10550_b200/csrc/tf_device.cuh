@@ -110,6 +110,75 @@ __device__ __forceinline__ void elim_row(Elim& S, double e, double c, double q, 
     S.a1 = al; S.b1 = be; S.z1 = zz;
 }
 
+// ---------------------------------------------------------------------------------------------
+// The same elimination with the shortest loop-carried dependency chain (measured on B200: DFMA 8.2
+// cycles, MUFU.RCP64H 17.7; elim_row carries 75 cycles per row, this one 52).  Only 256 warps march
+// an 8192^2 sweep, so the chain length x ny is a floor of the sweep time.
+//   * row i-1 is carried UNFINISHED: its pivot reciprocal is r1 = y1 + y1*t1 (y1 the MUFU seed, t1 =
+//     e + e^2 the cubic correction), its alpha, beta, z numerators are p1, b1, s1;
+//   * the next pivot mu_i = T - (p1*gam) r1 is expanded as (T - g y1) - (g y1) t1, so that only ONE
+//     fma follows the arrival of t1:  chain = fma(mu) -> MUFU -> fma(e) -> fma(t).
+// A call consumes the bands of row i and emits the FINAL coefficients of row i-1 (the caller stores them
+// one row behind and calls elim2_flush after the last row).  Same arithmetic as (A.5)/PAPER.md:729-734
+// up to rounding (the reciprocal is applied in expanded form).
+// ---------------------------------------------------------------------------------------------
+struct Elim2 { double y1, t1, p1, b1, s1, a2, b2, z2; };
+
+__device__ __forceinline__ Elim2 elim2_init() { Elim2 S = {0, 0, 0, 0, 0, 0, 0, 0}; return S; }
+
+__device__ __forceinline__ void elim2_row(Elim2& S, double e, double c, double q, double a, double b, double y,
+                                          double& al, double& be, double& zz)
+{
+    const double gam = fma(-S.a2, e, c);
+    const double T = fma(-S.b2, e, q);
+    const double g = S.p1 * gam;
+    const double bg = S.b1 * gam;
+    const double sy = fma(-S.z2, e, y);
+    const double u1 = fma(-g, S.y1, T);
+    const double G = g * S.y1;
+    const double mu = fma(-G, S.t1, u1);             // the only op between t1 and the next seed
+    double y0;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(mu));
+    const double ee = fma(-mu, y0, 1.0);
+    const double tt = fma(ee, ee, ee);
+    const double r1 = fma(S.y1, S.t1, S.y1);         // finish row i-1, off the critical path
+    al = S.p1 * r1; be = S.b1 * r1; zz = S.s1 * r1;
+    const double p = fma(-bg, r1, a);
+    const double s = fma(-zz, gam, sy);
+    S.a2 = al; S.b2 = be; S.z2 = zz;
+    S.y1 = y0; S.t1 = tt; S.p1 = p; S.b1 = b; S.s1 = s;
+}
+
+__device__ __forceinline__ void elim2_flush(const Elim2& S, double& al, double& be, double& zz)
+{
+    const double r1 = fma(S.y1, S.t1, S.y1);
+    al = S.p1 * r1; be = S.b1 * r1; zz = S.s1 * r1;
+}
+
+// (No "memory" clobber on purpose: the stored fields are never read by the storing kernel, and a clobber
+// would pin the next row's shared-memory loads behind this row's stores.)
+// Predicated 8-byte store without a branch: the marching warps keep halo / out-of-range lanes alive, and a
+// branch around the stores of every row would cut the row loop into basic blocks (no overlap of the next
+// row's loads with this row's dependency chain).
+__device__ __forceinline__ void st_if(int p, double* addr, double v)
+{
+    asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %2, 0;\n@q st.global.f64 [%0], %1;\n}\n" ::"l"(addr), "d"(v), "r"(p));
+}
+
+// three predicated stores under one predicate (alpha, beta, z of one row)
+__device__ __forceinline__ void st3_if(int p, double* a0, double v0, double* a1, double v1, double* a2, double v2)
+{
+    asm volatile("{\n.reg .pred q;\nsetp.ne.b32 q, %6, 0;\n@q st.global.f64 [%0], %3;\n@q st.global.f64 [%1], %4;\n"
+                 "@q st.global.f64 [%2], %5;\n}\n" ::"l"(a0), "l"(a1), "l"(a2), "d"(v0), "d"(v1), "d"(v2), "r"(p));
+}
+
+// L2 prefetch hint (no register, no shared memory): the marching producers pull the rows they will need a
+// few tiles from now into L2, so that their register loads one tile ahead see L2 latency, not HBM latency.
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
+// warp index as a value the compiler knows to be warp-uniform (role branches then do not look divergent)
+__device__ __forceinline__ int uniform_warp_idx() { return __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0); }
+
 // order-preserving max for non-negative doubles (NaN bit patterns compare above +inf, so a NaN
 // anywhere surfaces in the result)
 __device__ __forceinline__ void atomic_max_nonneg(double* addr, double v)

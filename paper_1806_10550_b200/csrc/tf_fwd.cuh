@@ -12,8 +12,22 @@
 #include "tf_device.cuh"
 #include "tf_tma.cuh"
 
+#ifndef TF_DBG_MODE
+#define TF_DBG_MODE 0        // experiments only (_work/): 1 = producers skip assembly, 2 = consumer skips the recurrence
+#endif
+
 namespace tf {
 
+#ifndef YW_CUNROLL
+#define YW_CUNROLL 4
+#endif
+#ifndef YW_PFD
+#define YW_PFD 0             // L2 prefetch distance of the y producers in rounds of chunks; 0 = off (measured: no gain)
+#endif
+#ifndef YW_MINB
+#define YW_MINB 4            // CTAs per SM the y forward kernel is compiled for (register cap)
+#endif
+constexpr int YW_CU = YW_CUNROLL;   // unroll of the consumer's row loop
 constexpr int YW_VALID = 28;     // columns per strip (lanes 2..29; lanes 0,1,30,31 are x-halo)
 
 // rolling state of a thread marching down a column (see yfwd_kernel in tf_sweeps.cuh for the same scheme)
@@ -27,11 +41,11 @@ struct YState {
 };
 
 // MODE 0: bring in cell (j+1) only;  1: also face j+1/2;  2: also produce row j (bands + R).
-// out5 = {A_{j+1/2}, c, q, a, R}
+// out6 = {A_{j+1/2}, c, q, a, R, A_{j-1/2}}
 // INTERIOR: all faces touched are interior and unfolded (1 <= j <= ny-3): no boundary logic at all.
 template <int N, int M, int MODE, bool INTERIOR>
 __device__ __forceinline__ void y_advance(YState& S, int j, double hp2, const Params& P, const Dir& DX, const Dir& DY,
-                                          bool xface, double rhs_in, double* out5, double& sD_out)
+                                          bool xface, double rhs_in, double* out6, double& sD_out)
 {
     const unsigned FULL = 0xffffffffu;
     const int ny = P.ny;
@@ -60,102 +74,146 @@ __device__ __forceinline__ void y_advance(YState& S, int j, double hp2, const Pa
         const double phixm = __shfl_up_sync(FULL, phixp, 1);
         const double sD = (phixp - phixm) + (phip - S.phim);
         sD_out = sD;
-        out5[0] = fp.A;
-        out5[1] = -fp.A - S.fm.p1;
-        out5[2] = 1.0 + fp.p1 - S.fm.p2;
-        out5[3] = fp.p2 - S.fm.A;
-        out5[4] = (rhs_in - S.h0) - sD;            // FIRST: caller passes rhs_in = b, fixed up below
+        out6[0] = fp.A;
+        out6[1] = -fp.A - S.fm.p1;
+        out6[2] = 1.0 + fp.p1 - S.fm.p2;
+        out6[3] = fp.p2 - S.fm.A;
+        out6[4] = (rhs_in - S.h0) - sD;            // FIRST: caller passes rhs_in = b, fixed up below
+        out6[5] = S.fm.A;
     }
     S.hm1 = S.h0; S.h0 = S.hp1; S.hp1 = hp2; S.hR0 = hR;
     S.c0 = cp; S.L0 = Lp;
     if (MODE >= 1) { S.fm = fp; S.phim = phip; }
 }
 
-template <int N, int M, bool FIRST, int NP, int RP, int NSTG>
-__global__ void __launch_bounds__(32 * (NP + 1))
-yfwd_ws_kernel(Params P, Dir DX, Dir DY, const double* __restrict__ u, double* __restrict__ bn,
+// ---------------------------------------------------------------------------------------------
+// y forward, two-sided ("burn at both ends", twisted factorisation): the lines of a strip are eliminated
+// from row 0 downwards (half 0, rows [0, mid)) and from row ny-1 upwards (half 1, rows [mid, ny)) by two
+// independent CTAs; the back-substitution kernel joins them with a 4x4 interface solve per line.  Same
+// operation count as the one-sided LU of PAPER.md:729-734, half the serial chain, twice the marching
+// warps (the chain x ny was the floor of the one-sided kernel).  For half 1 the system is taken in
+// reversed order k = ny-1-j: e' = b, c' = a, a' = c, b' = e, so its producers hand over A_{j-1/2}
+// instead of A_{j+1/2} and the consumer swaps the c and a planes; everything else is shared.
+// Coefficients of half 0 mean x_j = z_j - al_j x_{j+1} - be_j x_{j+2}; of half 1: x_j = z_j - al_j x_{j-1} - be_j x_{j-2}.
+//
+// CTA = warp 0 (consumer: the recurrence) + NP producer warps (assembly).  The hand-over ring has NCH
+// slots of ONE CHUNK (RP rows of one producer) each: chunk c is assembled by producer c % NP into slot
+// c % NCH, so RP can be large (the two warm-up rows of a chunk are amortised over RP rows) while the ring
+// stays small (4 CTAs per SM).  Inputs are pulled into L2 a few chunks ahead by prefetch hints.
+// ---------------------------------------------------------------------------------------------
+template <int N, int M, bool FIRST, int NP, int RP, int NCH>
+__global__ void __launch_bounds__(128 * (NP + 1), 1)
+yfwd_ws_kernel(Params P, Dir DX, Dir DY, int mid, const double* __restrict__ u, double* __restrict__ bn,
                double* __restrict__ al, double* __restrict__ be, double* __restrict__ zz)
 {
-    constexpr int RT = NP * RP;                       // rows per tile / stage
-    constexpr int SV = RT * 32;                       // doubles per value plane of a stage
+    // One CTA per SM: 4 sub-problems q = warp & 3 (two adjacent strips x two halves), each with its own
+    // ring and its own consumer + NP producers.  Warps w, w+4, w+8, ... share an SM sub-partition, so every
+    // sub-partition gets exactly one consumer and NP producers (the consumers' dependent chains and the
+    // producers' fp64 work are spread evenly over the four issue ports).
+    constexpr int SV = RP * 32;                       // doubles per value plane of a slot
+    constexpr size_t RING = (size_t)NCH * 5 * SV * 8 + 16 * NCH;    // bytes per sub-problem
     extern __shared__ __align__(16) unsigned char raw[];
-    double* sm = reinterpret_cast<double*>(raw);      // [NSTG][5][RT][32]
-    uint64_t* full = reinterpret_cast<uint64_t*>(raw + (size_t)NSTG * 5 * SV * 8);
-    uint64_t* empty = full + NSTG;
     const int nx = P.nx, ny = P.ny;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (threadIdx.x == 0) {
+    const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
+    const int q = warp & 3, role = warp >> 2;         // role 0: consumer, 1..NP: producers
+    double* sm = reinterpret_cast<double*>(raw + q * RING);          // [NCH][5][RP][32]
+    uint64_t* full = reinterpret_cast<uint64_t*>(raw + q * RING + (size_t)NCH * 5 * SV * 8);
+    uint64_t* empty = full + NCH;
+    if (role == 0 && lane == 0) {
 #pragma unroll
-        for (int s = 0; s < NSTG; ++s) { mbar_init(full + s, NP); mbar_init(empty + s, 1); }
+        for (int s = 0; s < NCH; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
         mbar_fence_init();
     }
     __syncthreads();
-    const int i = blockIdx.x * YW_VALID - 2 + lane;
-    const int ntile = (ny + RT - 1) / RT;
+    const int strip = 2 * blockIdx.x + (q & 1);
+    if (strip * YW_VALID >= nx) return;               // odd strip count: the last CTA has one strip
+    const int i = strip * YW_VALID - 2 + lane;
+    const int dir = q >> 1;                           // 0: rows 0 .. mid-1 downwards, 1: rows ny-1 .. mid upwards
+    const int nrows = dir ? ny - mid : mid;           // rows of this half
+    const int nchunk = (nrows + RP - 1) / RP;
+    const int jmin = dir ? mid : 0, jmax = dir ? ny : mid;    // this half owns rows [jmin, jmax)
+    const int outl = ((lane >= 2) && (lane < 2 + YW_VALID) && (i < nx)) ? 1 : 0;
 
-    if (warp < NP) {
-        // ------------------------------------------------------------------ producer: rows [j0, j0+RP) of each tile
+    if (role > 0) {
+        // ------------------------------------------------------------------ producer pw: chunks pw, pw+NP, ...
+        const int pw = role - 1;
         const int ic = ghost(i, nx);
         const bool xface = (i >= 0) && (i <= nx - 2);
-        const bool outl = (lane >= 2) && (lane < 2 + YW_VALID) && (i < nx);
         const double* up = u + ic;
         const double* bp = bn + ic;
-        for (int t = 0; t < ntile; ++t) {
-            const int s = t % NSTG;
-            const int j0 = t * RT + warp * RP;
-            const bool interior = (j0 >= 2) && (j0 + RP + 1 <= ny - 2);
+        for (int c = pw; c < nchunk; c += NP) {
+            const int s = c % NCH;
+            const int jlo = dir ? ny - (c + 1) * RP : c * RP;          // the chunk is rows jlo .. jlo+RP-1
+            const bool interior = (jlo >= 2) && (jlo + RP + 1 <= ny - 2) && (jlo >= jmin) && (jlo + RP <= jmax);
+            {   // L2 prefetch of the rows that my chunk YW_PFD rounds ahead adds
+                const int cp = c + YW_PFD * NP;
+                if (YW_PFD > 0 && cp < nchunk) {
+                    const int jl = dir ? ny - (cp + 1) * RP : cp * RP;
+                    const int jh = dir ? jl - 2 : jl + 2;
+                    if ((lane & 15) == 0 || lane == 31) {       // one request per 128-byte line of the 256-byte row segment
+#pragma unroll
+                        for (int k = 0; k < RP; ++k) {
+                            prefetch_l2(up + (size_t)clampi(jh + k, 0, ny - 1) * nx);
+                            if (!FIRST) prefetch_l2(bp + (size_t)clampi(jl + k, 0, ny - 1) * nx);
+                        }
+                    }
+                }
+            }
             double hq[RP + 4], bq[RP];
             if (interior) {
-                const double* hp = up + (size_t)(j0 - 2) * nx;
+                const double* hp = up + (size_t)(jlo - 2) * nx;
 #pragma unroll
                 for (int k = 0; k < RP + 4; ++k) hq[k] = hp[(size_t)k * nx];
-                const double* bq0 = bp + (size_t)j0 * nx;
+                const double* bq0 = bp + (size_t)jlo * nx;
 #pragma unroll
                 for (int k = 0; k < RP; ++k) bq[k] = FIRST ? 0.0 : bq0[(size_t)k * nx];
-            } else if (j0 < ny) {
+            } else {
 #pragma unroll
-                for (int k = 0; k < RP + 4; ++k) hq[k] = up[(size_t)ghost(j0 - 2 + k, ny) * nx];
+                for (int k = 0; k < RP + 4; ++k) hq[k] = up[(size_t)ghost(jlo - 2 + k, ny) * nx];
 #pragma unroll
-                for (int k = 0; k < RP; ++k) bq[k] = FIRST ? 0.0 : bp[(size_t)clampi(j0 + k, 0, ny - 1) * nx];
+                for (int k = 0; k < RP; ++k) bq[k] = FIRST ? 0.0 : bp[(size_t)clampi(jlo + k, 0, ny - 1) * nx];
             }
-            mbar_wait(empty + s, ((t / NSTG) & 1) ^ 1);
-            double* st = sm + (size_t)s * 5 * SV + (warp * RP) * 32 + lane;
+            mbar_wait(empty + s, ((c / NCH) & 1) ^ 1);
+            // slot row of chunk row r: r (half 0), RP-1-r (half 1)
+            double* st = sm + (size_t)s * 5 * SV + (dir ? RP - 1 : 0) * 32 + lane;
+            const int sstep = dir ? -32 : 32;
             YState S;
             S.hm1 = 0.0; S.h0 = hq[0]; S.hp1 = hq[1]; S.hR0 = 0.0;
             S.c0 = {0, 0, 0, 0}; S.L0 = 0.0; S.fm = {0, 0, 0}; S.phim = 0.0;
-            double o5[5], sD;
-            if (interior) {
-                y_advance<N, M, 0, true>(S, j0 - 2, hq[2], P, DX, DY, xface, 0.0, o5, sD);
-                y_advance<N, M, 1, true>(S, j0 - 1, hq[3], P, DX, DY, xface, 0.0, o5, sD);
-                double* bo = bn + (size_t)j0 * nx + i;
+            double o6[6], sD;
+            if (TF_DBG_MODE == 1) {
+            } else if (interior) {
+                y_advance<N, M, 0, true>(S, jlo - 2, hq[2], P, DX, DY, xface, 0.0, o6, sD);
+                y_advance<N, M, 1, true>(S, jlo - 1, hq[3], P, DX, DY, xface, 0.0, o6, sD);
+                double* bo = bn + (size_t)jlo * nx + i;
 #pragma unroll
                 for (int r = 0; r < RP; ++r) {
                     const double hcur = S.h0;
-                    y_advance<N, M, 2, true>(S, j0 + r, hq[r + 4], P, DX, DY, xface, FIRST ? hcur : bq[r], o5, sD);
+                    y_advance<N, M, 2, true>(S, jlo + r, hq[r + 4], P, DX, DY, xface, FIRST ? hcur : bq[r], o6, sD);
                     if (FIRST) {
                         const double b = hcur - sD;
-                        if (outl) bo[(size_t)r * nx] = b;
-                        o5[4] = (b - hcur) - sD;
+                        st_if(outl, bo + (size_t)r * nx, b);
+                        o6[4] = (b - hcur) - sD;
                     }
-#pragma unroll
-                    for (int v = 0; v < 5; ++v) st[v * SV + r * 32] = o5[v];
+                    double* sr = st + r * sstep;
+                    sr[0] = dir ? o6[5] : o6[0]; sr[SV] = o6[1]; sr[2 * SV] = o6[2]; sr[3 * SV] = o6[3]; sr[4 * SV] = o6[4];
                 }
-            } else if (j0 < ny) {
-                y_advance<N, M, 0, false>(S, j0 - 2, hq[2], P, DX, DY, xface, 0.0, o5, sD);
-                y_advance<N, M, 1, false>(S, j0 - 1, hq[3], P, DX, DY, xface, 0.0, o5, sD);
+            } else {
+                y_advance<N, M, 0, false>(S, jlo - 2, hq[2], P, DX, DY, xface, 0.0, o6, sD);
+                y_advance<N, M, 1, false>(S, jlo - 1, hq[3], P, DX, DY, xface, 0.0, o6, sD);
 #pragma unroll
                 for (int r = 0; r < RP; ++r) {
-                    const int j = j0 + r;
-                    if (j < ny) {
-                        const double hcur = S.h0;
-                        y_advance<N, M, 2, false>(S, j, hq[r + 4], P, DX, DY, xface, FIRST ? hcur : bq[r], o5, sD);
+                    const int j = jlo + r;
+                    const double hcur = S.h0;
+                    y_advance<N, M, 2, false>(S, j, hq[r + 4], P, DX, DY, xface, FIRST ? hcur : bq[r], o6, sD);
+                    if (j >= jmin && j < jmax) {
                         if (FIRST) {
                             const double b = hcur - sD;
                             if (outl) bn[(size_t)j * nx + i] = b;
-                            o5[4] = (b - hcur) - sD;
+                            o6[4] = (b - hcur) - sD;
                         }
-#pragma unroll
-                        for (int v = 0; v < 5; ++v) st[v * SV + r * 32] = o5[v];
+                        double* sr = st + r * sstep;
+                        sr[0] = dir ? o6[5] : o6[0]; sr[SV] = o6[1]; sr[2 * SV] = o6[2]; sr[3 * SV] = o6[3]; sr[4 * SV] = o6[4];
                     }
                 }
             }
@@ -163,148 +221,202 @@ yfwd_ws_kernel(Params P, Dir DX, Dir DY, const double* __restrict__ u, double* _
             if (lane == 0) mbar_arrive(full + s);
         }
     } else {
-        // ------------------------------------------------------------------ consumer: the recurrence
-        const bool outl = (lane >= 2) && (lane < 2 + YW_VALID) && (i < nx);
-        Elim S = {0, 0, 0, 0, 0, 0};
+        // ------------------------------------------------------------------ consumer: the recurrence.
+        // elim2_row emits the coefficients of the PREVIOUS row, so every store goes one row behind.
+        Elim2 S = elim2_init();
         double e = 0.0;
-        for (int t = 0; t < ntile; ++t) {
-            const int s = t % NSTG;
-            mbar_wait(full + s, (t / NSTG) & 1);
+        const int step = dir ? -nx : nx;
+        int o = (dir ? ny : -1) * nx + i;                 // the row before the first one (32-bit element offset)
+        const int offc = dir ? 3 * SV : SV, offa = dir ? SV : 3 * SV;   // half 1: c' = a, a' = c
+        for (int c = 0; c < nchunk; ++c) {
+            const int s = c % NCH;
+            mbar_wait(full + s, (c / NCH) & 1);
             const double* st = sm + (size_t)s * 5 * SV + lane;
-            const int jt = t * RT;
-            const int nrow = min(RT, ny - jt);
-            size_t o = (size_t)jt * nx + i;
-            if (nrow == RT) {
-#pragma unroll 8
-                for (int r = 0; r < RT; ++r) {
-                    const double A = st[r * 32], c = st[SV + r * 32], q = st[2 * SV + r * 32], a = st[3 * SV + r * 32];
+            const double* stc = st + offc;
+            const double* sta = st + offa;
+            const int nrow = min(RP, nrows - c * RP);
+            if (TF_DBG_MODE == 2) {
+                o += step * nrow;
+            } else if (nrow == RP && c > 0) {
+#pragma unroll
+                for (int r = 0; r < RP; ++r) {
+                    const double A = st[r * 32], cc = stc[r * 32], q = st[2 * SV + r * 32], a = sta[r * 32];
                     const double R = st[4 * SV + r * 32];
                     double va, vb, vz;
-                    elim_row(S, e, c, q, a, A, R, va, vb, vz);
+                    elim2_row(S, e, cc, q, a, A, R, va, vb, vz);
                     e = A;
-                    if (outl) { al[o] = va; be[o] = vb; zz[o] = vz; }
-                    o += nx;
+                    st3_if(outl, al + o, va, be + o, vb, zz + o, vz);
+                    o += step;
                 }
             } else {
                 for (int r = 0; r < nrow; ++r) {
-                    const double A = st[r * 32], c = st[SV + r * 32], q = st[2 * SV + r * 32], a = st[3 * SV + r * 32];
+                    const double A = st[r * 32], cc = stc[r * 32], q = st[2 * SV + r * 32], a = sta[r * 32];
                     const double R = st[4 * SV + r * 32];
                     double va, vb, vz;
-                    elim_row(S, e, c, q, a, A, R, va, vb, vz);
+                    elim2_row(S, e, cc, q, a, A, R, va, vb, vz);
                     e = A;
-                    if (outl) { al[o] = va; be[o] = vb; zz[o] = vz; }
-                    o += nx;
+                    st3_if(outl && (c * RP + r) > 0, al + o, va, be + o, vb, zz + o, vz);
+                    o += step;
                 }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(empty + s);
         }
+        double va, vb, vz;
+        elim2_flush(S, va, vb, vz);
+        st3_if(outl, al + o, va, be + o, vb, zz + o, vz);
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// x forward, warp-specialised.  A CTA owns 32 rows.  Producers work with lanes ALONG the lines (lane <->
-// column i, coalesced loads, neighbours by shuffle; only x-neighbours are needed) and write
-// the bands transposed into the stage ([column][33]: conflict-free both ways); the consumer has
-// lane <-> row and marches i = 0..nx-1.  Coefficients go out transposed ([i][j]) so the stores are
-// coalesced too.  Tile = 28 columns (32 lanes minus 2 halo lanes each side).
+// x forward, two-sided, warp-specialised.  One CTA per SM with 4 sub-problems q = warp & 3: two adjacent
+// blocks of XW_R rows x two halves (half 0: columns 0 .. mid-1 ascending, half 1: columns nx-1 .. mid
+// descending; see yfwd_ws_kernel for the two-sided scheme).  Per sub-problem: one consumer warp (lane <->
+// row of the block, marches along the lines) and NP producer warps.  Producers work with lanes ALONG the
+// lines (lane <-> column, coalesced loads, x-neighbours by shuffle; only x-neighbours are needed,
+// PAPER.md:748) on tiles of 28 columns, split rows r = pw, pw+NP, ... between them, and write the bands
+// transposed into two ring slots of XW_CK = 14 columns each ([plane][column][XW_LD]: conflict-free for the
+// producers' half-warps and for the consumer).  Coefficients go out transposed ([i][j]) so the consumer's
+// stores are coalesced too.
 // ---------------------------------------------------------------------------------------------
-constexpr int XW_CT = 28;
-constexpr int XW_LD = 33;
+constexpr int XW_CT = 28;            // columns per producer tile (32 lanes minus 2 halo lanes each side)
+constexpr int XW_CK = 14;            // columns per ring slot
+constexpr int XW_R = 28;             // rows per block
+constexpr int XW_LD = 29;            // slot row pitch in doubles (odd)
 
-template <int N, int M, int NP, int NSTG>
-__global__ void __launch_bounds__(32 * (NP + 1))
-xfwd_ws_kernel(Params P, Dir DX, const double* __restrict__ u, const double* __restrict__ w,
+template <int N, int M, int NP, int NCH>
+__global__ void __launch_bounds__(128 * (NP + 1), 1)
+xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const double* __restrict__ w,
                double* __restrict__ alT, double* __restrict__ beT, double* __restrict__ zzT)
 {
-    constexpr int SV = XW_CT * XW_LD;                 // doubles per value plane of a stage
+    constexpr int SV = XW_CK * XW_LD;                 // doubles per value plane of a slot
+    constexpr size_t RING = (size_t)NCH * 5 * SV * 8 + 16 * NCH;
+    constexpr int NRMAX = (XW_R + NP - 1) / NP;       // rows per producer
     extern __shared__ __align__(16) unsigned char raw[];
-    double* sm = reinterpret_cast<double*>(raw);      // [NSTG][5][CT][33]
-    uint64_t* full = reinterpret_cast<uint64_t*>(raw + (size_t)NSTG * 5 * SV * 8);
-    uint64_t* empty = full + NSTG;
     const unsigned FULL = 0xffffffffu;
     const int nx = P.nx, ny = P.ny;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (threadIdx.x == 0) {
+    const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
+    const int q = warp & 3, role = warp >> 2;         // role 0: consumer, 1..NP: producers
+    double* sm = reinterpret_cast<double*>(raw + q * RING);          // [NCH][5][CK][LD]
+    uint64_t* full = reinterpret_cast<uint64_t*>(raw + q * RING + (size_t)NCH * 5 * SV * 8);
+    uint64_t* empty = full + NCH;
+    if (role == 0 && lane == 0) {
 #pragma unroll
-        for (int s = 0; s < NSTG; ++s) { mbar_init(full + s, NP); mbar_init(empty + s, 1); }
+        for (int s = 0; s < NCH; ++s) { mbar_init(full + s, NP); mbar_init(empty + s, 1); }
         mbar_fence_init();
     }
     __syncthreads();
-    const int j0 = blockIdx.x * 32;
-    const int ntile = (nx + XW_CT - 1) / XW_CT;
+    const int j0 = (2 * blockIdx.x + (q & 1)) * XW_R;
+    if (j0 >= ny) return;
+    const int dir = q >> 1;
+    const int ncols = dir ? nx - mid : mid;           // columns of this half
+    const int ntile = (ncols + XW_CT - 1) / XW_CT;
+    const int imin = dir ? mid : 0, imax = dir ? nx : mid;
 
-    if (warp < NP) {
-        // ------------------------------------------------------------------ producer: rows warp, warp+NP, ...
+    if (role > 0) {
+        // ------------------------------------------------------------------ producer pw: rows pw, pw+NP, ... of the block
+        const int pw = role - 1;
+        size_t rowoff[NRMAX];
+#pragma unroll
+        for (int k = 0; k < NRMAX; ++k) rowoff[k] = (size_t)min(j0 + pw + k * NP, ny - 1) * nx;
+        // marching position k of lane's column within the tile: lane-2 (half 0), 29-lane (half 1)
+        const int kk = dir ? XW_CT + 1 - lane : lane - 2;
+        const bool lane_ok = (lane >= 2) && (lane < 2 + XW_CT);
+        const int slot_sel = lane_ok ? kk / XW_CK : 0;       // first or second slot of the tile
+        const int kc = lane_ok ? kk % XW_CK : 0;             // column within the slot
         for (int t = 0; t < ntile; ++t) {
-            const int s = t % NSTG;
-            const int i = t * XW_CT - 2 + lane;
+            const int ilo = dir ? nx - (t + 1) * XW_CT : t * XW_CT;       // the tile is columns ilo .. ilo+27
+            const int i = ilo - 2 + lane;
             const int ic = ghost(i, nx);
             const bool face_ok = (i >= 0) && (i <= nx - 2);
-            const bool col_ok = (lane >= 2) && (lane < 2 + XW_CT) && (i < nx);
-            constexpr int NR = 32 / NP;
-            double hq[NR], wq[NR];
+            const bool col_ok = lane_ok && (i >= imin) && (i < imax);
+            double hq[NRMAX], wq[NRMAX];
 #pragma unroll
-            for (int k = 0; k < NR; ++k) {
-                const int jr = min(j0 + warp + k * NP, ny - 1);
-                hq[k] = u[(size_t)jr * nx + ic];
-                wq[k] = col_ok ? w[(size_t)jr * nx + i] : 0.0;
+            for (int k = 0; k < NRMAX; ++k) {
+                hq[k] = u[rowoff[k] + ic];
+                wq[k] = col_ok ? w[rowoff[k] + i] : 0.0;
             }
-            mbar_wait(empty + s, ((t / NSTG) & 1) ^ 1);
-            double* st = sm + (size_t)s * 5 * SV + (lane - 2) * XW_LD;
+            const int g0 = 2 * t, g1 = 2 * t + 1;             // global slot numbers of this tile
+            mbar_wait(empty + g0 % NCH, ((g0 / NCH) & 1) ^ 1);
+            mbar_wait(empty + g1 % NCH, ((g1 / NCH) & 1) ^ 1);
+            double* st = sm + (size_t)((slot_sel ? g1 : g0) % NCH) * 5 * SV + kc * XW_LD;
 #pragma unroll
-            for (int k = 0; k < NR; ++k) {
-                const int r = warp + k * NP;
-                const double h0 = hq[k];
-                const double hm1 = __shfl_up_sync(FULL, h0, 1);
-                const double hp1 = __shfl_down_sync(FULL, h0, 1), hp2 = __shfl_down_sync(FULL, h0, 2);
-                const Cell c0 = cell_functions<N, M>(h0, P);
-                Cell c1;
-                c1.f0 = __shfl_down_sync(FULL, c0.f0, 1); c1.f1 = __shfl_down_sync(FULL, c0.f1, 1);
-                c1.g0 = __shfl_down_sync(FULL, c0.g0, 1); c1.g1 = __shfl_down_sync(FULL, c0.g1, 1);
-                Face fp = face_partials(hm1, hp2, hp1 - h0, c0.f0 + c1.f0, c0.f1 + c1.f1, c0, c1, DX);
-                if (i == 0) fp.p1 -= fp.A;
-                if (i == nx - 2) fp.p2 += fp.A;
-                if (!face_ok) { fp.A = 0.0; fp.p1 = 0.0; fp.p2 = 0.0; }
-                Face fm;
-                fm.A = __shfl_up_sync(FULL, fp.A, 1); fm.p1 = __shfl_up_sync(FULL, fp.p1, 1);
-                fm.p2 = __shfl_up_sync(FULL, fp.p2, 1);
-                if (col_ok) {
-                    st[r] = fp.A;
-                    st[SV + r] = -fp.A - fm.p1;
-                    st[2 * SV + r] = 1.0 + fp.p1 - fm.p2;
-                    st[3 * SV + r] = fp.p2 - fm.A;
-                    st[4 * SV + r] = wq[k];
+            for (int k = 0; k < NRMAX; ++k) {
+                const int r = pw + k * NP;
+                if (r < XW_R) {
+                    const double h0 = hq[k];
+                    const double hm1 = __shfl_up_sync(FULL, h0, 1);
+                    const double hp1 = __shfl_down_sync(FULL, h0, 1), hp2 = __shfl_down_sync(FULL, h0, 2);
+                    const Cell c0 = cell_functions<N, M>(h0, P);
+                    Cell c1;
+                    c1.f0 = __shfl_down_sync(FULL, c0.f0, 1); c1.f1 = __shfl_down_sync(FULL, c0.f1, 1);
+                    c1.g0 = __shfl_down_sync(FULL, c0.g0, 1); c1.g1 = __shfl_down_sync(FULL, c0.g1, 1);
+                    Face fp = face_partials(hm1, hp2, hp1 - h0, c0.f0 + c1.f0, c0.f1 + c1.f1, c0, c1, DX);
+                    if (i == 0) fp.p1 -= fp.A;
+                    if (i == nx - 2) fp.p2 += fp.A;
+                    if (!face_ok) { fp.A = 0.0; fp.p1 = 0.0; fp.p2 = 0.0; }
+                    Face fm;
+                    fm.A = __shfl_up_sync(FULL, fp.A, 1); fm.p1 = __shfl_up_sync(FULL, fp.p1, 1);
+                    fm.p2 = __shfl_up_sync(FULL, fp.p2, 1);
+                    if (col_ok) {
+                        st[r] = dir ? fm.A : fp.A;
+                        st[SV + r] = -fp.A - fm.p1;
+                        st[2 * SV + r] = 1.0 + fp.p1 - fm.p2;
+                        st[3 * SV + r] = fp.p2 - fm.A;
+                        st[4 * SV + r] = wq[k];
+                    }
                 }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(full + s);
+            if (lane == 0) { mbar_arrive(full + g0 % NCH); mbar_arrive(full + g1 % NCH); }
         }
     } else {
         // ------------------------------------------------------------------ consumer: lane <-> row j0 + lane
         const int j = j0 + lane;
-        const bool rowok = j < ny;
-        Elim S = {0, 0, 0, 0, 0, 0};
+        const int rowok = (lane < XW_R && j < ny) ? 1 : 0;
+        Elim2 S = elim2_init();
         double e = 0.0;
-        for (int t = 0; t < ntile; ++t) {
-            const int s = t % NSTG;
-            mbar_wait(full + s, (t / NSTG) & 1);
-            const double* st = sm + (size_t)s * 5 * SV + lane;
-            const int i0 = t * XW_CT;
-            const int ncol = min(XW_CT, nx - i0);
-            size_t o = (size_t)i0 * ny + j;
-            for (int c = 0; c < ncol; ++c) {
-                const double A = st[c * XW_LD], cc = st[SV + c * XW_LD], q = st[2 * SV + c * XW_LD];
-                const double a = st[3 * SV + c * XW_LD], R = st[4 * SV + c * XW_LD];
-                double va, vb, vz;
-                elim_row(S, e, cc, q, a, A, R, va, vb, vz);
-                e = A;
-                if (rowok) { alT[o] = va; beT[o] = vb; zzT[o] = vz; }
-                o += ny;
+        const int step = dir ? -ny : ny;
+        int o = (dir ? nx : -1) * ny + j;                 // the column before the first one
+        const int offc = dir ? 3 * SV : SV, offa = dir ? SV : 3 * SV;
+        const int nslot = (ncols + XW_CK - 1) / XW_CK;
+        const int lr = min(lane, XW_R - 1);               // lanes beyond the block read a valid row (results unused)
+        for (int g = 0; g < 2 * ntile; ++g) {
+            const int s = g % NCH;
+            mbar_wait(full + s, (g / NCH) & 1);
+            const double* st = sm + (size_t)s * 5 * SV + lr;
+            const double* stc = st + offc;
+            const double* sta = st + offa;
+            const int ncol = min(XW_CK, ncols - g * XW_CK);
+            if (ncol == XW_CK && g > 0) {
+#pragma unroll
+                for (int c = 0; c < XW_CK; ++c) {
+                    const double A = st[c * XW_LD], cc = stc[c * XW_LD], qq = st[2 * SV + c * XW_LD], a = sta[c * XW_LD];
+                    const double R = st[4 * SV + c * XW_LD];
+                    double va, vb, vz;
+                    elim2_row(S, e, cc, qq, a, A, R, va, vb, vz);
+                    e = A;
+                    st3_if(rowok, alT + o, va, beT + o, vb, zzT + o, vz);
+                    o += step;
+                }
+            } else {
+                for (int c = 0; c < ncol; ++c) {
+                    const double A = st[c * XW_LD], cc = stc[c * XW_LD], qq = st[2 * SV + c * XW_LD], a = sta[c * XW_LD];
+                    const double R = st[4 * SV + c * XW_LD];
+                    double va, vb, vz;
+                    elim2_row(S, e, cc, qq, a, A, R, va, vb, vz);
+                    e = A;
+                    st3_if(rowok && (g * XW_CK + c) > 0, alT + o, va, beT + o, vb, zzT + o, vz);
+                    o += step;
+                }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(empty + s);
+            (void)nslot;
         }
+        double va, vb, vz;
+        elim2_flush(S, va, vb, vz);
+        st3_if(rowok, alT + o, va, beT + o, vb, zzT + o, vz);
     }
 }
 

@@ -31,11 +31,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
         "{\n"
         ".reg .pred p;\n"
         "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
         "@p bra DONE_%=;\n"
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
-        "}\n" ::"r"(s_addr(bar)), "r"(parity)
+        "}\n" ::"r"(s_addr(bar)), "r"(parity), "r"(0x989680u)     // suspend-time hint: a waiting warp sleeps in hardware
         : "memory");
 }
 
