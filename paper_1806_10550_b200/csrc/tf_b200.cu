@@ -232,7 +232,7 @@ cudaError_t launch_xbwd(int nx, int ny, const double* alT, const double* beT, co
 
 constexpr int YW_NP = 3, YW_RP = 8, YW_NSTG = 4;   // yfwd: consumer warp 0 + 3 producer warps, chunks of 8 rows, ring of 4 chunk slots (40 KiB)
 
-constexpr int XW_NP = 3, XW_NSTG = 3;              // xfwd: per sub-problem 1 consumer + 3 producer warps, ring of 3 slots of 14 columns (48 KiB)
+constexpr int XW_NP = 4, XW_NSTG = 3;              // xfwd: per sub-problem 1 consumer + 4 producer warps, ring of 3 slots of 14 columns (48 KiB)
 
 // one pseudo-Newton iteration k: reads src (u^n if k == 0 else uk), writes uk, red[2k..2k+1]
 template <int N, int M>

@@ -279,6 +279,9 @@ yfwd_ws_kernel(Params P, Dir DX, Dir DY, int mid, const double* __restrict__ u, 
 // producers' half-warps and for the consumer).  Coefficients go out transposed ([i][j]) so the consumer's
 // stores are coalesced too.
 // ---------------------------------------------------------------------------------------------
+#ifndef XW_RECOMPUTE_C1
+#define XW_RECOMPUTE_C1 1
+#endif
 constexpr int XW_CT = 28;            // columns per producer tile (32 lanes minus 2 halo lanes each side)
 constexpr int XW_CK = 14;            // columns per ring slot
 constexpr int XW_R = 28;             // rows per block
@@ -348,9 +351,13 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
                     const double hm1 = __shfl_up_sync(FULL, h0, 1);
                     const double hp1 = __shfl_down_sync(FULL, h0, 1), hp2 = __shfl_down_sync(FULL, h0, 2);
                     const Cell c0 = cell_functions<N, M>(h0, P);
+#if XW_RECOMPUTE_C1
+                    const Cell c1 = cell_functions<N, M>(hp1, P);   // cheaper than 8 shuffles: the LSU pipe, not fp64, bounds this kernel
+#else
                     Cell c1;
                     c1.f0 = __shfl_down_sync(FULL, c0.f0, 1); c1.f1 = __shfl_down_sync(FULL, c0.f1, 1);
                     c1.g0 = __shfl_down_sync(FULL, c0.g0, 1); c1.g1 = __shfl_down_sync(FULL, c0.g1, 1);
+#endif
                     Face fp = face_partials(hm1, hp2, hp1 - h0, c0.f0 + c1.f0, c0.f1 + c1.f1, c0, c1, DX);
                     if (i == 0) fp.p1 -= fp.A;
                     if (i == nx - 2) fp.p2 += fp.A;
