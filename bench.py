@@ -90,14 +90,22 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+NCU_SUMMARY = os.path.join("profiles", "r01_v4_ncu_full_summary.csv")
+NCU_KERNEL = {"y_forward": "yfwd_ws_kernel", "y_backward": "ybwd2_tma_kernel", "x_forward": "xfwd_ws_kernel",
+              "x_backward_update": "xbwd2_tma_kernel"}
+
+
 def ncu_traffic(kernel):
-    """dram bytes per launch of `kernel` from the committed ncu --set full summary, or None."""
-    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
-    if os.path.exists(p):
-        try:
-            return json.load(open(p)).get(kernel, {}).get("dram_bytes_per_launch")
-        except Exception:
-            return None
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` at 8192^2, from the committed
+    ncu --set full summary (profiles/r01_v4_ncu.md names the command), or None."""
+    import csv
+    p = os.path.join(ROOT, NCU_SUMMARY)
+    try:
+        for row in csv.DictReader(open(p)):
+            if row["kernel"].startswith(NCU_KERNEL[kernel]):
+                return int(round((float(row["dram_read_GB"]) + float(row["dram_write_GB"])) * 1e9))
+    except (OSError, KeyError, ValueError):
+        return None
     return None
 
 
@@ -140,6 +148,23 @@ def run_reference(args, cfg):
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------- multi-rank bookkeeping
+def max_over_ranks(seconds, world, device):
+    """The job's time is the slowest rank's device time (replicas: no data-path collective)."""
+    if world <= 1:
+        return float(seconds)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(npts, steps, world, seconds):
+    """grid-point steps per second over all ranks: every rank advances its own npts-point film `steps` times."""
+    return world * npts * steps / seconds
 
 
 # ----------------------------------------------------------------------------------------- B200 arm
@@ -196,10 +221,7 @@ def run_b200(args, cfg):
         barrier()
         w1 = time.time()
         sec = ev0.elapsed_time(ev1) / 1e3
-        if world > 1:
-            t = torch.tensor([sec], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            sec = float(t.item())
+        sec = max_over_ranks(sec, world, "cuda")
         return sec, iters, tf.kernel_launches() - l0, w0, w1
 
     sampler = ClockSampler(local) if rank == 0 else None
@@ -214,7 +236,7 @@ def run_b200(args, cfg):
     e2e = None
     if not args.no_e2e:
         esec, eiters, _, _, _ = timed_run(e2e=True)
-        e2e = {"value": world * npts * args.steps / esec, "unit": UNIT, "h2d_bytes_per_step": npts * 8,
+        e2e = {"value": whole_job_value(npts, args.steps, world, esec), "unit": UNIT, "h2d_bytes_per_step": npts * 8,
                "d2h_bytes_per_step": npts * 8, "ms_per_step": 1e3 * esec / args.steps, "newton_iters_total": eiters}
     if rank != 0:
         if world > 1:
@@ -233,11 +255,12 @@ def run_b200(args, cfg):
     if dom:
         a = kern[dom]["alg_gbs"]
         roofline = {"bound": "hbm", "kernel": dom, "achieved": a, "peak": peak, "unit": "GB/s", "frac": a / peak,
-                    "peak_source": peak_src, "traffic": ncu_traffic(dom),
+                    "peak_source": peak_src, "traffic": ncu_traffic(dom) if (nx, ny) == (8192, 8192) else None,
+                    "traffic_source": NCU_SUMMARY,
                     "alg_bytes_per_launch": kern[dom]["alg_bytes_per_launch"], "avg_launch_ms": kern[dom]["avg_ms"]}
     ksum = sum(k["avg_ms"] * k["launches"] for k in kern.values())
     line = {
-        "metric": METRIC, "value": world * npts * args.steps / sec, "unit": UNIT, "n_gpus": world,
+        "metric": METRIC, "value": whole_job_value(npts, args.steps, world, sec), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg["name"], "grid": [nx, ny], "dx": cfg["dx"], "dt": dt, "tol": cfg["tol"],

@@ -48,7 +48,8 @@ size_t tf_workspace_bytes(int nx, int ny);
 
 /*
  * Create a context (problem statement: PAPER.md:47 (1.1), 86-91 (1.7)-(1.8), 297-302 (2.28)).
- *   nx, ny >= 5; dx, dy, kappa, hstar > 0; integer exponents n > m >= 1; bc = TF_BC_NOFLUX
+ *   nx, ny >= 5 and (nx+1)*(ny+1) < 2^31 (the kernels index a field with 32-bit element offsets);
+ *   dx, dy, kappa, hstar > 0; integer exponents n > m >= 1; bc = TF_BC_NOFLUX
  *   (anything else: TF_ERR_UNSUPPORTED -- the paper defines no other boundary condition).
  * tf_create allocates tf_workspace_bytes() of device memory itself and uses the legacy
  * default stream.  tf_create_with_workspace borrows `dev_ws` (device pointer, 256-byte

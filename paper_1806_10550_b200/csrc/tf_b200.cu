@@ -115,7 +115,6 @@ bool make_map2d(CUtensorMap* m, const double* base, int inner, int outer, int bo
 
 // ---- ring-kernel launchers (dynamic shared memory above 48 KB needs the opt-in attribute once per kernel)
 constexpr int YB_NST = 8, YB_RS = 16;     // 8 stages x 16 rows x 3 arrays x 256 B = 96 KiB per warp
-constexpr int XB_NST = 6, XB_CS = 16;     // 6 stages x (3 x 16 x 256 B + 32 x 18 x 8 B) = 99 KiB per warp
 
 template <typename K>
 cudaError_t opt_in_smem(K kernel, size_t bytes)
@@ -125,19 +124,6 @@ cudaError_t opt_in_smem(K kernel, size_t bytes)
 
 constexpr int YT_NST = 6, YT_RS = 16;     // TMA ring: 6 stages x 3 boxes of 16 x 32 doubles = 72 KiB per warp
 constexpr int XT_NST = 6;                 // TMA ring: 6 stages x 16 KiB
-
-cudaError_t launch_ybwd_tma(const CUtensorMap* m, int nx, int ny, double* w, cudaStream_t st)
-{
-    constexpr size_t SM = (size_t)YT_NST * 3 * YT_RS * 32 * 8 + 8 * YT_NST + 1024;
-    static bool ready = false;
-    if (!ready) {
-        cudaError_t e = opt_in_smem(ybwd_tma_kernel<YT_NST, YT_RS>, SM);
-        if (e != cudaSuccess) return e;
-        ready = true;
-    }
-    ybwd_tma_kernel<YT_NST, YT_RS><<<(nx + 31) / 32, 32, SM, st>>>(m[0], m[1], m[2], nx, ny, w);
-    return cudaGetLastError();
-}
 
 // two-sided y back substitution (the y forward kernel is two-sided): TMA ring when the maps exist, else plain
 cudaError_t launch_ybwd2(const CUtensorMap* m, bool tma, int nx, int ny, int mid, const double* al, const double* be,
@@ -156,20 +142,6 @@ cudaError_t launch_ybwd2(const CUtensorMap* m, bool tma, int nx, int ny, int mid
         ready = true;
     }
     ybwd2_tma_kernel<YT_NST, YT_RS><<<g, 32, SM, st>>>(m[0], m[1], m[2], nx, ny, mid, al, be, zz, w);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_xbwd_tma(const CUtensorMap* m, const CUtensorMap& uin, const CUtensorMap& uout, int nx, int ny,
-                            double* red, cudaStream_t st)
-{
-    constexpr size_t SM = (size_t)XT_NST * 4 * 16 * 32 * 8 + 8 * XT_NST + 1024;
-    static bool ready = false;
-    if (!ready) {
-        cudaError_t e = opt_in_smem(xbwd_tma_kernel<XT_NST>, SM);
-        if (e != cudaSuccess) return e;
-        ready = true;
-    }
-    xbwd_tma_kernel<XT_NST><<<(ny + 31) / 32, 32, SM, st>>>(m[0], m[1], m[2], uin, uout, nx, ny, red);
     return cudaGetLastError();
 }
 
@@ -208,25 +180,6 @@ cudaError_t launch_ybwd(int nx, int ny, const double* al, const double* be, cons
     const int g = (nx + 31) / 32;
     if (nx % 2 == 0) ybwd_ring_kernel<YB_NST, YB_RS, true><<<g, 32, SM, st>>>(nx, ny, al, be, zz, w);
     else ybwd_ring_kernel<YB_NST, YB_RS, false><<<g, 32, SM, st>>>(nx, ny, al, be, zz, w);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_xbwd(int nx, int ny, const double* alT, const double* beT, const double* zzT, const double* uk,
-                        double* unew, double* red, cudaStream_t st)
-{
-    constexpr size_t SM = sizeof(double) * XB_NST * (3 * XB_CS * 32 + 32 * (XB_CS + 2));
-    static bool ready = false;
-    if (!ready) {
-        cudaError_t e = opt_in_smem(xbwd_ring_kernel<XB_NST, XB_CS, true>, SM);
-        if (e == cudaSuccess) e = opt_in_smem(xbwd_ring_kernel<XB_NST, XB_CS, false>, SM);
-        if (e != cudaSuccess) return e;
-        ready = true;
-    }
-    const int g = (ny + 31) / 32;
-    if (nx % 2 == 0 && ny % 2 == 0)
-        xbwd_ring_kernel<XB_NST, XB_CS, true><<<g, 32, SM, st>>>(nx, ny, alT, beT, zzT, uk, unew, red);
-    else
-        xbwd_ring_kernel<XB_NST, XB_CS, false><<<g, 32, SM, st>>>(nx, ny, alT, beT, zzT, uk, unew, red);
     return cudaGetLastError();
 }
 
@@ -309,6 +262,8 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
     if (!out) return fail(nullptr, TF_ERR_INVALID_ARG, "out is NULL");
     *out = nullptr;
     if (nx < 5 || ny < 5) return fail(nullptr, TF_ERR_INVALID_ARG, "nx, ny must be >= 5");
+    if (((long long)nx + 1) * ((long long)ny + 1) >= (1LL << 31))
+        return fail(nullptr, TF_ERR_INVALID_ARG, "(nx+1)*(ny+1) must be < 2^31 (32-bit element offsets)");
     if (!(dx > 0) || !(dy > 0) || !(kappa > 0) || !(hstar > 0) || !std::isfinite(dx) || !std::isfinite(dy) ||
         !std::isfinite(kappa) || !std::isfinite(hstar))
         return fail(nullptr, TF_ERR_INVALID_ARG, "dx, dy, kappa, hstar must be positive and finite");

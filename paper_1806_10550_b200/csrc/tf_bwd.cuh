@@ -1,9 +1,10 @@
-// tf_bwd.cuh -- back-substitution kernels with cp.async shared-memory rings (see tf_async.cuh).
-//   ybwd_ring : w_j = z_j - alpha_j w_{j+1} - beta_j w_{j+2}                    (S4)
-//   xbwd_ring : v_i likewise on the transposed coefficients, then u_{k+1} = u_k + v and
-//               res = max|v/u_k|                                              (S6+S7, (2.21)-(2.22))
-// One warp per CTA owns 32 lines; NST stages of RS (CS) line-elements each are in flight per warp,
-// so HBM latency is covered by (NST-1)*stage bytes per warp instead of by occupancy.
+// tf_bwd.cuh -- back-substitution kernels.
+//   ybwd2_* : two-sided y back substitution -> w                                   (S4)
+//   xbwd2_* : two-sided x back substitution on the transposed coefficients, then u_{k+1} = u_k + v and
+//             res = max|v/u_k|                                                   (S6+S7, (2.21)-(2.22))
+//   ybwd_ring_kernel : one-sided back substitution with a cp.async ring (isolated solver of config 4)
+// One warp per CTA owns 32 lines; NST stages of line-elements are in flight per warp (TMA boxes + mbarriers,
+// or cp.async), so HBM latency is covered by bytes in flight per warp instead of by occupancy.
 #pragma once
 #include "tf_async.cuh"
 #include "tf_tma.cuh"
@@ -53,159 +54,6 @@ ybwd_ring_kernel(int nx, int ny, const double* __restrict__ al, const double* __
                 w2 = w1; w1 = x;
             }
         }
-    }
-}
-
-template <int NST, int CS, bool VEC>
-__global__ void __launch_bounds__(32)
-xbwd_ring_kernel(int nx, int ny, const double* __restrict__ alT, const double* __restrict__ beT,
-                 const double* __restrict__ zzT, const double* uk, double* unew,   // uk may alias unew
-                 double* __restrict__ red)
-{
-    extern __shared__ __align__(16) double sm[];
-    constexpr int ULD = CS + 2;                              // u tile leading dimension (even: 16-byte rows)
-    constexpr int STAGE = 3 * CS * 32 + 32 * ULD;            // doubles per stage
-    const int lane = threadIdx.x;
-    const int j0 = blockIdx.x * 32;
-    const int rows_ok = min(32, ny - j0);                    // lines (rows j) this warp owns
-    const bool rowok = lane < rows_ok;
-    const int ntile = (nx + CS - 1) / CS;
-    const double* src[3] = {alT, beT, zzT};
-
-    auto issue = [&](int q) {
-        const int t = ntile - 1 - q;
-        if (t >= 0) {
-            const int i0 = t * CS, cols_ok = min(CS, nx - i0);
-            double* s = sm + (size_t)(q % NST) * STAGE;
-#pragma unroll
-            for (int a = 0; a < 3; ++a)
-                warp_copy_block<CS, 32, VEC>(s + a * CS * 32, 32, src[a] + (size_t)i0 * ny + j0, (size_t)ny,
-                                             cols_ok, rows_ok, lane);
-            warp_copy_block<32, CS, VEC>(s + 3 * CS * 32, ULD, uk + (size_t)j0 * nx + i0, (size_t)nx,
-                                         rows_ok, cols_ok, lane);
-        }
-        cp_async_commit();
-    };
-#pragma unroll
-    for (int q = 0; q < NST - 1; ++q) issue(q);
-    double v1 = 0.0, v2 = 0.0, res = 0.0;
-    int bad = 0;
-    for (int q = 0; q < ntile; ++q) {
-        cp_async_wait<NST - 2>();
-        __syncwarp();
-        issue(q + NST - 1);
-        const int i0 = (ntile - 1 - q) * CS, cols_ok = min(CS, nx - i0);
-        double* s = sm + (size_t)(q % NST) * STAGE;
-        double* su = s + 3 * CS * 32;
-#pragma unroll
-        for (int c = CS - 1; c >= 0; --c) {
-            if (c < cols_ok) {
-                const double v = fma(-s[c * 32 + lane], v1, fma(-s[CS * 32 + c * 32 + lane], v2, s[2 * CS * 32 + c * 32 + lane]));
-                const double uo = su[lane * ULD + c];
-                const double un = uo + v;
-                const double rr = fabs(v / uo);
-                if (rowok) {
-                    if (!(rr <= res)) res = rr;              // NaN sticks
-                    if (!(un > 0.0) || isinf(un)) bad = 1;
-                }
-                su[lane * ULD + c] = un;
-                v2 = v1; v1 = v;
-            }
-        }
-        __syncwarp();
-        // write the updated 32 x CS tile back, lanes along the contiguous index
-        if (VEC) {
-            constexpr int CPR = CS / 2;
-#pragma unroll
-            for (int k = 0; k < (32 * CPR + 31) / 32; ++k) {
-                const int idx = k * 32 + lane;
-                const int r = idx / CPR, c = (idx % CPR) * 2;
-                if (r < rows_ok && c < cols_ok)
-                    *reinterpret_cast<double2*>(unew + (size_t)(j0 + r) * nx + i0 + c) =
-                        *reinterpret_cast<const double2*>(su + r * ULD + c);
-            }
-        } else {
-#pragma unroll
-            for (int k = 0; k < (32 * CS + 31) / 32; ++k) {
-                const int idx = k * 32 + lane;
-                const int r = idx / CS, c = idx % CS;
-                if (r < rows_ok && c < cols_ok) unew[(size_t)(j0 + r) * nx + i0 + c] = su[r * ULD + c];
-            }
-        }
-    }
-    if (res != res) res = __longlong_as_double(0x7ff8000000000000LL);   // canonical +NaN for the bit-max
-    res = warp_max_nonneg(res);
-    bad = __any_sync(0xffffffffu, bad);
-    if (lane == 0) {
-        atomic_max_nonneg(red, res);
-        if (bad) atomic_max_nonneg(red + 1, 1.0);
-    }
-}
-
-// =============================================================================================
-// TMA variants (used whenever the row pitch is a multiple of 16 bytes, i.e. nx resp. ny even).
-// One instruction per [RS x 32] box, issued by lane 0; the other lanes only wait on the mbarrier.
-// =============================================================================================
-template <int NST, int RS>
-__global__ void __launch_bounds__(32)
-ybwd_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__ CUtensorMap mB,
-                const __grid_constant__ CUtensorMap mZ, int nx, int ny, double* __restrict__ w)
-{
-    extern __shared__ unsigned char raw[];
-    unsigned char* base = align1024(raw);
-    constexpr int BOX = RS * 32;                             // doubles per box
-    double* sm = reinterpret_cast<double*>(base);            // [NST][3][RS][32]
-    uint64_t* full = reinterpret_cast<uint64_t*>(base + (size_t)NST * 3 * BOX * 8);
-    const int lane = threadIdx.x;
-    const int i0 = blockIdx.x * 32, i = i0 + lane;
-    const int ntile = (ny + RS - 1) / RS;
-    if (lane == 0) {
-#pragma unroll
-        for (int s = 0; s < NST; ++s) mbar_init(full + s, 1);
-        mbar_fence_init();
-    }
-    __syncwarp();
-    auto issue = [&](int q) {
-        const int t = ntile - 1 - q;
-        if (t >= 0 && lane == 0) {
-            const int s = q % NST;
-            double* d = sm + (size_t)s * 3 * BOX;
-            mbar_expect_tx(full + s, 3 * BOX * 8);
-            tma_load_2d(d, &mA, i0, t * RS, full + s);
-            tma_load_2d(d + BOX, &mB, i0, t * RS, full + s);
-            tma_load_2d(d + 2 * BOX, &mZ, i0, t * RS, full + s);
-        }
-    };
-#pragma unroll
-    for (int q = 0; q < NST; ++q) issue(q);
-    double w1 = 0.0, w2 = 0.0;
-    for (int q = 0; q < ntile; ++q) {
-        const int s = q % NST;
-        mbar_wait(full + s, (q / NST) & 1);
-        const int j0 = (ntile - 1 - q) * RS;
-        const double* d = sm + (size_t)s * 3 * BOX + lane;
-        if (j0 + RS <= ny) {                                 // full tile: branch-free, one running pointer
-            double* wp = w + (size_t)(j0 + RS - 1) * nx + i;
-#pragma unroll
-            for (int r = RS - 1; r >= 0; --r) {
-                const double x = fma(-d[r * 32], w1, fma(-d[BOX + r * 32], w2, d[2 * BOX + r * 32]));
-                if (i < nx) *wp = x;
-                wp -= nx;
-                w2 = w1; w1 = x;
-            }
-        } else {
-            double* wp = w + (size_t)j0 * nx + i;
-#pragma unroll
-            for (int r = RS - 1; r >= 0; --r) {
-                if (j0 + r < ny) {
-                    const double x = fma(-d[r * 32], w1, fma(-d[BOX + r * 32], w2, d[2 * BOX + r * 32]));
-                    if (i < nx) wp[(size_t)r * nx] = x;
-                    w2 = w1; w1 = x;
-                }
-            }
-        }
-        __syncwarp();
-        issue(q + NST);
     }
 }
 
@@ -357,105 +205,6 @@ ybwd2_plain_kernel(int nx, int ny, int mid, const double* __restrict__ al, const
         const double x = fma(-al[o], w1, fma(-be[o], w2, zz[o]));
         w[o] = x;
         w2 = w1; w1 = x;
-    }
-}
-
-// byte offset of element (r, c) in a [32][16] fp64 tile written by TMA with CU_TENSOR_MAP_SWIZZLE_128B
-__device__ __forceinline__ int swz128(int r, int c) { return r * 128 + ((((c >> 1) ^ (r & 7))) << 4) + ((c & 1) << 3); }
-
-template <int NST>
-__global__ void __launch_bounds__(32)
-xbwd_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__ CUtensorMap mB,
-                const __grid_constant__ CUtensorMap mZ, const __grid_constant__ CUtensorMap mUin,
-                const __grid_constant__ CUtensorMap mUout, int nx, int ny, double* __restrict__ red)
-{
-    constexpr int CS = 16;                                   // columns per stage (= one 128-byte swizzled row)
-    constexpr int BOX = CS * 32;                             // doubles per coefficient box
-    constexpr int STAGE = 4 * BOX * 8;                       // bytes per stage: 3 coefficient boxes + the u tile
-    extern __shared__ unsigned char raw[];
-    unsigned char* base = align1024(raw);
-    uint64_t* full = reinterpret_cast<uint64_t*>(base + (size_t)NST * STAGE);
-    const int lane = threadIdx.x;
-    const int j0 = blockIdx.x * 32;
-    const bool rowok = j0 + lane < ny;
-    const int ntile = (nx + CS - 1) / CS;
-    if (lane == 0) {
-#pragma unroll
-        for (int s = 0; s < NST; ++s) mbar_init(full + s, 1);
-        mbar_fence_init();
-    }
-    __syncwarp();
-    auto issue = [&](int q) {
-        const int t = ntile - 1 - q;
-        if (t >= 0 && lane == 0) {
-            const int s = q % NST;
-            unsigned char* d = base + (size_t)s * STAGE;
-            mbar_expect_tx(full + s, STAGE);
-            tma_load_2d(d, &mA, j0, t * CS, full + s);
-            tma_load_2d(d + BOX * 8, &mB, j0, t * CS, full + s);
-            tma_load_2d(d + 2 * BOX * 8, &mZ, j0, t * CS, full + s);
-            tma_load_2d(d + 3 * BOX * 8, &mUin, t * CS, j0, full + s);
-        }
-    };
-#pragma unroll
-    for (int q = 0; q < NST - 1; ++q) issue(q);
-    double v1 = 0.0, v2 = 0.0, res = 0.0;
-    int bad = 0;
-    for (int q = 0; q < ntile; ++q) {
-        const int s = q % NST;
-        mbar_wait(full + s, (q / NST) & 1);
-        const int i0 = (ntile - 1 - q) * CS, cols_ok = min(CS, nx - i0);
-        unsigned char* d = base + (size_t)s * STAGE;
-        const double* cf = reinterpret_cast<const double*>(d) + lane;
-        unsigned char* su = d + 3 * BOX * 8;
-        unsigned char* sur = su + lane * 128;                // this lane's swizzled row
-        const int sx = (lane & 7) << 4;
-        if (cols_ok == CS) {                                 // full tile: branch-free
-#pragma unroll
-            for (int c = CS - 1; c >= 0; --c) {
-                const double v = fma(-cf[c * 32], v1, fma(-cf[BOX + c * 32], v2, cf[2 * BOX + c * 32]));
-                double* pu = reinterpret_cast<double*>(sur + ((((c >> 1) << 4) ^ sx) + ((c & 1) << 3)));
-                const double uo = *pu;
-                const double un = uo + v;
-                const double rr = fabs(v) * rcp(uo);
-                res = fmax(res, rowok ? rr : 0.0);           // a NaN/inf iterate is caught by `bad`
-                bad |= (rowok && !(un > 0.0 && un <= 1.7976931348623157e308)) ? 1 : 0;
-                *pu = un;
-                v2 = v1; v1 = v;
-            }
-        } else {
-#pragma unroll
-            for (int c = CS - 1; c >= 0; --c) {
-                if (c < cols_ok) {
-                    const double v = fma(-cf[c * 32], v1, fma(-cf[BOX + c * 32], v2, cf[2 * BOX + c * 32]));
-                    double* pu = reinterpret_cast<double*>(su + swz128(lane, c));
-                    const double uo = *pu;
-                    const double un = uo + v;
-                    const double rr = fabs(v) * rcp(uo);
-                    res = fmax(res, rowok ? rr : 0.0);
-                    bad |= (rowok && !(un > 0.0 && un <= 1.7976931348623157e308)) ? 1 : 0;
-                    *pu = un;
-                    v2 = v1; v1 = v;
-                }
-            }
-        }
-        fence_proxy_async();
-        __syncwarp();
-        if (lane == 0) {
-            tma_store_2d(&mUout, i0, j0, su);
-            tma_store_commit();
-            tma_store_wait_read<1>();                        // the store of tile q-1 has left shared memory
-        }
-        __syncwarp();
-        issue(q + NST - 1);                                  // refill the stage of tile q-1
-    }
-    if (lane == 0) tma_store_wait_all<0>();
-    if (res != res) res = __longlong_as_double(0x7ff8000000000000LL);
-    res = warp_max_nonneg(res);
-    bad = __any_sync(0xffffffffu, bad);
-    if (lane == 0) {
-        atomic_max_nonneg(red, res);
-        if (bad) atomic_max_nonneg(red + 1, 1.0);
     }
 }
 

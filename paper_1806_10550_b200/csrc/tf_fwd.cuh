@@ -30,7 +30,7 @@ namespace tf {
 constexpr int YW_CU = YW_CUNROLL;   // unroll of the consumer's row loop
 constexpr int YW_VALID = 28;     // columns per strip (lanes 2..29; lanes 0,1,30,31 are x-halo)
 
-// rolling state of a thread marching down a column (see yfwd_kernel in tf_sweeps.cuh for the same scheme)
+// rolling state of a thread marching down a column
 struct YState {
     double hm1, h0, hp1;         // h(j-1), h(j), h(j+1)
     double hR0;                  // h(j)[i+1]

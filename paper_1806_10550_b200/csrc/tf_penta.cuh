@@ -5,7 +5,7 @@
 //                              into padded shared memory and read transposed; the elimination
 //                              coefficients are stored transposed, x is written back through a tile.
 #pragma once
-#include "tf_sweeps.cuh"
+#include "tf_reduce.cuh"
 
 namespace tf {
 
@@ -38,7 +38,7 @@ penta_col_fwd_kernel(int nrow, int ncol, const double* __restrict__ e, const dou
         }
     }
 }
-// dir 1 backward == ybwd_kernel(nx = ncol, ny = nrow)
+// dir 1 backward == ybwd_ring_kernel(nx = ncol, ny = nrow)
 
 // ---- dir 0: forward.  ws arrays are TRANSPOSED: [c][r]
 constexpr int PT_ARR = 6;

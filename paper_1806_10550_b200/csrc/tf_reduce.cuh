@@ -1,0 +1,54 @@
+// tf_reduce.cuh -- reductions of a field (S9 mass of (3.2), and the validity check of a state).
+#pragma once
+#include "tf_device.cuh"
+
+namespace tf {
+
+constexpr int XT = 32;          // tile edge of the transposing kernels (tf_penta.cuh)
+constexpr int XTP = XT + 1;     // padded row length (doubles)
+constexpr int PF = 8;           // rows of register prefetch in the simple marching kernels
+
+// ---------------------------------------------------------------------------------------------
+// reductions (S9 mass, state validation): fixed grid, fixed order -> bitwise reproducible
+// ---------------------------------------------------------------------------------------------
+constexpr int RED_BLOCKS = 1184;   // 8 x 148 SMs
+constexpr int RED_THREADS = 256;
+
+// part[b] = sum over a fixed slice; flag[0] |= any non-finite or non-positive value
+__global__ void __launch_bounds__(RED_THREADS)
+sum_check_kernel(size_t n, const double* __restrict__ h, double* __restrict__ part, int* __restrict__ flag)
+{
+    __shared__ double sm[RED_THREADS / 32];
+    double acc = 0.0;
+    int bad = 0;
+    for (size_t p = (size_t)blockIdx.x * RED_THREADS + threadIdx.x; p < n; p += (size_t)RED_BLOCKS * RED_THREADS) {
+        const double v = h[p];
+        acc += v;
+        if (!(v > 0.0) || isinf(v)) bad = 1;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = acc;
+    if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(flag, 1);
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int k = 0; k < RED_THREADS / 32; ++k) t += sm[k];
+        part[blockIdx.x] = t;
+    }
+}
+
+__global__ void __launch_bounds__(1024)
+sum_final_kernel(const double* __restrict__ part, double scale, double* __restrict__ out)
+{
+    __shared__ double sm[1024];
+    const int t = threadIdx.x;
+    sm[t] = (t < RED_BLOCKS ? part[t] : 0.0) + (t + 1024 < RED_BLOCKS ? part[t + 1024] : 0.0);
+    __syncthreads();
+    for (int o = 512; o > 0; o >>= 1) {
+        if (t < o) sm[t] += sm[t + o];
+        __syncthreads();
+    }
+    if (t == 0) out[0] = scale * sm[0];
+}
+
+}  // namespace tf
