@@ -48,6 +48,8 @@ struct tf_ctx {
     bool tma_y, tma_x;                         // TMA rings usable (row pitch multiple of 16 B, grid >= one box)
     CUtensorMap mY[3], mX[3];                  // alpha,beta,z as [ny][nx] (box RS x 32) and as [nx][ny] (box CS x 32)
     CUtensorMap mU[2];                         // the two state buffers as [ny][nx], box 32 x 16, 128-byte swizzle
+    bool tma_yf;                               // y forward producers stage their inputs by TMA
+    CUtensorMap mUy[2], mBn;                   // state buffers / b^n as [ny][nx], boxes (RP+4) x 32 and RP x 32
     double* ubuf[2];                           // buffer addresses mU[0], mU[1] were encoded for
     bool profiling;
     cudaEvent_t ev[65 * 5];                    // 5 events per iteration, up to 65 iterations in flight
@@ -122,8 +124,8 @@ cudaError_t opt_in_smem(K kernel, size_t bytes)
     return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
-constexpr int YT_NST = 6, YT_RS = 16;     // TMA ring: 6 stages x 3 boxes of 16 x 32 doubles = 72 KiB per warp
-constexpr int XT_NST = 6;                 // TMA ring: 6 stages x 16 KiB
+constexpr int YT_NST = 4, YT_RS = 16;     // TMA ring: 4 stages x 3 boxes of 16 x 32 doubles = 48 KiB per warp: all 512 CTAs resident (4 per SM)
+constexpr int XT_NST = 3;                 // TMA ring: 3 stages x 16 KiB: all 512 CTAs resident (4 per SM)
 
 // two-sided y back substitution (the y forward kernel is two-sided): TMA ring when the maps exist, else plain
 cudaError_t launch_ybwd2(const CUtensorMap* m, bool tma, int nx, int ny, int mid, const double* al, const double* be,
@@ -198,7 +200,8 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
     cudaEvent_t* ev = (c->profiling && slot >= 0) ? c->ev + 5 * slot : nullptr;
     if (ev) cudaEventRecord(ev[0], c->stream);
     {
-        constexpr size_t SM = 4 * ((size_t)YW_NSTG * 5 * YW_RP * 32 * 8 + 16 * YW_NSTG);
+        constexpr size_t SM = 4 * (size_t)YW_NSTG * 5 * YW_RP * 32 * 8 + 4 * YW_NP * (size_t)(2 * YW_RP + 4) * 32 * 8 +
+                              (8 * YW_NSTG + 4 * YW_NP) * 8;
         static bool ready = false;
         if (!ready) {
             cudaError_t e = opt_in_smem(yfwd_ws_kernel<N, M, true, YW_NP, YW_RP, YW_NSTG>, SM);
@@ -207,10 +210,12 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
             ready = true;
         }
         const int nthr = 128 * (YW_NP + 1);
+        const CUtensorMap& mu = c->mUy[src == c->ubuf[0] ? 0 : 1];
+        const int tma = c->tma_yf ? 1 : 0;
         if (k == 0)
-            yfwd_ws_kernel<N, M, true, YW_NP, YW_RP, YW_NSTG><<<gy, nthr, SM, c->stream>>>(P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz);
+            yfwd_ws_kernel<N, M, true, YW_NP, YW_RP, YW_NSTG><<<gy, nthr, SM, c->stream>>>(mu, c->mBn, tma, P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz);
         else
-            yfwd_ws_kernel<N, M, false, YW_NP, YW_RP, YW_NSTG><<<gy, nthr, SM, c->stream>>>(P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz);
+            yfwd_ws_kernel<N, M, false, YW_NP, YW_RP, YW_NSTG><<<gy, nthr, SM, c->stream>>>(mu, c->mBn, tma, P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz);
     }
     if (ev) cudaEventRecord(ev[1], c->stream);
     cudaError_t le = launch_ybwd2(c->mY, c->tma_y, P.nx, P.ny, c->mid_y, c->al, c->be, c->zz, c->w, c->stream);
@@ -328,6 +333,12 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
         for (int k = 0; k < 3; ++k) c->tma_x = c->tma_x && make_map2d(&c->mX[k], f3[k], ny, nx, 32, 16, false);
         for (int k = 0; k < 2; ++k) c->tma_x = c->tma_x && make_map2d(&c->mU[k], c->ubuf[k], nx, ny, 16, 32, true);
     }
+    c->tma_yf = (nx % 2 == 0) && nx >= 32 && ny >= YW_RP + 4;
+    if (c->tma_yf) {
+        for (int k = 0; k < 2; ++k) c->tma_yf = c->tma_yf && make_map2d(&c->mUy[k], c->ubuf[k], nx, ny, 32, YW_RP + 4, false);
+        c->tma_yf = c->tma_yf && make_map2d(&c->mBn, c->bn, nx, ny, 32, YW_RP, false);
+    }
+    if (!c->tma_yf) { memset(&c->mUy, 0, sizeof(c->mUy)); memset(&c->mBn, 0, sizeof(c->mBn)); }
     c->profiling = false;
     for (auto& ev : c->ev) ev = nullptr;
     for (int q = 0; q < TF_PROFILE_SLOTS; ++q) { c->prof_ms[q] = 0.0; c->prof_n[q] = 0; }

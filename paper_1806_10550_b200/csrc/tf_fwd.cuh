@@ -103,25 +103,30 @@ __device__ __forceinline__ void y_advance(YState& S, int j, double hp2, const Pa
 // ---------------------------------------------------------------------------------------------
 template <int N, int M, bool FIRST, int NP, int RP, int NCH>
 __global__ void __launch_bounds__(128 * (NP + 1), 1)
-yfwd_ws_kernel(Params P, Dir DX, Dir DY, int mid, const double* __restrict__ u, double* __restrict__ bn,
+yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ CUtensorMap mB, int use_tma,
+               Params P, Dir DX, Dir DY, int mid, const double* __restrict__ u, double* __restrict__ bn,
                double* __restrict__ al, double* __restrict__ be, double* __restrict__ zz)
 {
     // One CTA per SM: 4 sub-problems q = warp & 3 (two adjacent strips x two halves), each with its own
     // ring and its own consumer + NP producers.  Warps w, w+4, w+8, ... share an SM sub-partition, so every
     // sub-partition gets exactly one consumer and NP producers (the consumers' dependent chains and the
     // producers' fp64 work are spread evenly over the four issue ports).
+    // Shared memory: 4 rings [NCH][5][RP][32] | 4*NP input stagings [(RP+4) + RP][32] | mbarriers.
     constexpr int SV = RP * 32;                       // doubles per value plane of a slot
-    constexpr size_t RING = (size_t)NCH * 5 * SV * 8 + 16 * NCH;    // bytes per sub-problem
-    extern __shared__ __align__(16) unsigned char raw[];
+    constexpr size_t RING = (size_t)NCH * 5 * SV * 8;                // bytes per sub-problem
+    constexpr size_t STG = (size_t)(2 * RP + 4) * 32 * 8;            // bytes per producer: rows of u, then rows of b^n
+    extern __shared__ __align__(128) unsigned char raw[];
     const int nx = P.nx, ny = P.ny;
     const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
     const int q = warp & 3, role = warp >> 2;         // role 0: consumer, 1..NP: producers
     double* sm = reinterpret_cast<double*>(raw + q * RING);          // [NCH][5][RP][32]
-    uint64_t* full = reinterpret_cast<uint64_t*>(raw + q * RING + (size_t)NCH * 5 * SV * 8);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(raw + 4 * RING + 4 * NP * STG);
+    uint64_t* full = bars + q * 2 * NCH;
     uint64_t* empty = full + NCH;
     if (role == 0 && lane == 0) {
 #pragma unroll
         for (int s = 0; s < NCH; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
+        for (int p = 0; p < NP; ++p) mbar_init(bars + 8 * NCH + q * NP + p, 1);
         mbar_fence_init();
     }
     __syncthreads();
@@ -141,26 +146,46 @@ yfwd_ws_kernel(Params P, Dir DX, Dir DY, int mid, const double* __restrict__ u, 
         const bool xface = (i >= 0) && (i <= nx - 2);
         const double* up = u + ic;
         const double* bp = bn + ic;
-        for (int c = pw; c < nchunk; c += NP) {
-            const int s = c % NCH;
-            const int jlo = dir ? ny - (c + 1) * RP : c * RP;          // the chunk is rows jlo .. jlo+RP-1
-            const bool interior = (jlo >= 2) && (jlo + RP + 1 <= ny - 2) && (jlo >= jmin) && (jlo + RP <= jmax);
-            {   // L2 prefetch of the rows that my chunk YW_PFD rounds ahead adds
-                const int cp = c + YW_PFD * NP;
-                if (YW_PFD > 0 && cp < nchunk) {
-                    const int jl = dir ? ny - (cp + 1) * RP : cp * RP;
-                    const int jh = dir ? jl - 2 : jl + 2;
-                    if ((lane & 15) == 0 || lane == 31) {       // one request per 128-byte line of the 256-byte row segment
-#pragma unroll
-                        for (int k = 0; k < RP; ++k) {
-                            prefetch_l2(up + (size_t)clampi(jh + k, 0, ny - 1) * nx);
-                            if (!FIRST) prefetch_l2(bp + (size_t)clampi(jl + k, 0, ny - 1) * nx);
-                        }
-                    }
+        // Input staging: one TMA box of RP+4 rows of u and one of RP rows of b^n per interior chunk, issued one
+        // chunk ahead (right after the previous chunk's rows were copied to registers), so that the chunk's
+        // global-memory latency overlaps the assembly of the chunk before it.  Boundary chunks, and grids whose
+        // row pitch is not a multiple of 16 bytes, load directly.
+        double* stg = reinterpret_cast<double*>(raw + 4 * RING + (size_t)(q * NP + pw) * STG);
+        uint64_t* sbar = bars + 8 * NCH + q * NP + pw;
+        const int col0 = strip * YW_VALID - 2;
+        const int srcl = lane + (ic - i);                      // lane holding my ghost column (edge strips)
+        const bool edge = (col0 < 0) || (col0 + 32 > nx);
+        auto chunk_lo = [&](int c) { return dir ? ny - (c + 1) * RP : c * RP; };
+        auto is_interior = [&](int jlo) { return (jlo >= 2) && (jlo + RP + 1 <= ny - 2) && (jlo >= jmin) && (jlo + RP <= jmax); };
+        auto issue_tma = [&](int c) {
+            if (use_tma && c < nchunk && lane == 0) {
+                const int jl = chunk_lo(c);
+                if (is_interior(jl)) {
+                    mbar_expect_tx(sbar, (uint32_t)((FIRST ? RP + 4 : 2 * RP + 4) * 32 * 8));
+                    tma_load_2d(stg, &mU, col0, jl - 2, sbar);
+                    if (!FIRST) tma_load_2d(stg + (RP + 4) * 32, &mB, col0, jl, sbar);
                 }
             }
+        };
+        issue_tma(pw);
+        unsigned ntma = 0;                                      // boxes consumed so far (staging barrier phase)
+        for (int c = pw; c < nchunk; c += NP) {
+            const int s = c % NCH;
+            const int jlo = chunk_lo(c);                        // the chunk is rows jlo .. jlo+RP-1
+            const bool interior = is_interior(jlo);
             double hq[RP + 4], bq[RP];
-            if (interior) {
+            if (interior && use_tma) {
+                mbar_wait(sbar, ntma & 1);
+                ++ntma;
+#pragma unroll
+                for (int k = 0; k < RP + 4; ++k) hq[k] = stg[k * 32 + lane];
+#pragma unroll
+                for (int k = 0; k < RP; ++k) bq[k] = FIRST ? 0.0 : stg[(RP + 4 + k) * 32 + lane];
+                if (edge) {                                     // reflect the ghost columns (TMA zero-fills them)
+#pragma unroll
+                    for (int k = 0; k < RP + 4; ++k) hq[k] = __shfl_sync(0xffffffffu, hq[k], srcl);
+                }
+            } else if (interior) {
                 const double* hp = up + (size_t)(jlo - 2) * nx;
 #pragma unroll
                 for (int k = 0; k < RP + 4; ++k) hq[k] = hp[(size_t)k * nx];
@@ -173,6 +198,8 @@ yfwd_ws_kernel(Params P, Dir DX, Dir DY, int mid, const double* __restrict__ u, 
 #pragma unroll
                 for (int k = 0; k < RP; ++k) bq[k] = FIRST ? 0.0 : bp[(size_t)clampi(jlo + k, 0, ny - 1) * nx];
             }
+            __syncwarp();
+            issue_tma(c + NP);                                  // staging is free again: fetch my next chunk
             mbar_wait(empty + s, ((c / NCH) & 1) ^ 1);
             // slot row of chunk row r: r (half 0), RP-1-r (half 1)
             double* st = sm + (size_t)s * 5 * SV + (dir ? RP - 1 : 0) * 32 + lane;
