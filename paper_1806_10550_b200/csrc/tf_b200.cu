@@ -160,11 +160,11 @@ cudaError_t launch_xbwd2(const CUtensorMap* m, const CUtensorMap& uin, const CUt
     constexpr size_t SM = (size_t)XT_NST * 4 * 16 * 32 * 8 + 8 * XT_NST + 1024;
     static bool ready = false;
     if (!ready) {
-        cudaError_t e = opt_in_smem(xbwd2_tma_kernel<XT_NST>, SM);
+        cudaError_t e = opt_in_smem(xbwd2_tma_kernel<XT_NST, true>, SM);
         if (e != cudaSuccess) return e;
         ready = true;
     }
-    xbwd2_tma_kernel<XT_NST><<<g, 32, SM, st>>>(m[0], m[1], m[2], uin, uout, nx, ny, mid, alT, beT, zzT, red);
+    xbwd2_tma_kernel<XT_NST, true><<<g, 32, SM, st>>>(m[0], m[1], m[2], uin, uout, nx, ny, mid, alT, beT, zzT, red);
     return cudaGetLastError();
 }
 
@@ -185,6 +185,8 @@ cudaError_t launch_ybwd(int nx, int ny, const double* al, const double* be, cons
     return cudaGetLastError();
 }
 
+constexpr int PC_NST = 3, PC_RS = 8;      // isolated solver, columns: 3 stages x 6 arrays x 8 rows x 256 B = 36 KiB per warp
+constexpr int PR_NST = 2;                 // isolated solver, rows: 2 stages x 6 arrays x 4 KiB = 48 KiB per warp
 constexpr int YW_NP = 3, YW_RP = 8, YW_NSTG = 4;   // yfwd: consumer warp 0 + 3 producer warps, chunks of 8 rows, ring of 4 chunk slots (40 KiB)
 
 constexpr int XW_NP = 4, XW_NSTG = 3;              // xfwd: per sub-problem 1 consumer + 4 producer warps, ring of 3 slots of 14 columns (48 KiB)
@@ -523,22 +525,74 @@ tf_status tf_penta_solve(int nrow, int ncol, int dir, const double* e, const dou
     double* al = (double*)dev_ws;
     double* be = (double*)((char*)dev_ws + fb);
     double* zz = (double*)((char*)dev_ws + 2 * fb);
+    const double* in6[6] = {e, c, d, a, b, rhs};
+    bool aligned = ((uintptr_t)dev_ws % 16 == 0) && ((uintptr_t)x % 16 == 0);
+    for (int k = 0; k < 6; ++k) aligned = aligned && ((uintptr_t)in6[k] % 16 == 0);
     if (dir == 1) {
-        const int g = (ncol + 31) / 32;
-        penta_col_fwd_kernel<<<g, 32, 0, st>>>(nrow, ncol, e, c, d, a, b, rhs, al, be, zz);
-        cudaError_t le = launch_ybwd(ncol, nrow, al, be, zz, x, st);
-        if (le != cudaSuccess) return cuda_fail(nullptr, le, "ybwd launch");
-    } else {
-        const int g = (nrow + XT - 1) / XT;
-        const size_t sm = sizeof(double) * PT_ARR * XT * XTP;
-        static bool attr_set = false;
-        if (!attr_set) {
-            cudaError_t ee = cudaFuncSetAttribute(penta_row_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-            if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
-            attr_set = true;
+        // systems along columns: nsys = ncol, length = nrow
+        const int mid = (nrow / 2) / 16 * 16;
+        bool fast = aligned && (ncol % 2 == 0) && ncol >= 32 && nrow >= 64;
+        Maps6 M;
+        CUtensorMap mw[3];
+        if (fast) {
+            for (int k = 0; k < 6; ++k) fast = fast && make_map2d(&M.m[k], in6[k], ncol, nrow, 32, PC_RS, false);
+            const double* w3[3] = {al, be, zz};
+            for (int k = 0; k < 3; ++k) fast = fast && make_map2d(&mw[k], w3[k], ncol, nrow, 32, YT_RS, false);
         }
-        penta_row_fwd_kernel<<<g, 32, sm, st>>>(nrow, ncol, e, c, d, a, b, rhs, al, be, zz);
-        penta_row_bwd_kernel<<<g, 32, 0, st>>>(nrow, ncol, al, be, zz, x);
+        if (fast) {
+            constexpr size_t SM = (size_t)PC_NST * 6 * PC_RS * 32 * 8 + 8 * PC_NST + 1024;
+            static bool ready = false;
+            if (!ready) {
+                cudaError_t ee = opt_in_smem(penta_col_fwd2_kernel<PC_NST, PC_RS>, SM);
+                if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
+                ready = true;
+            }
+            penta_col_fwd2_kernel<PC_NST, PC_RS><<<dim3((ncol + 31) / 32, 2), 32, SM, st>>>(M, nrow, ncol, mid, al, be, zz);
+            cudaError_t le = launch_ybwd2(mw, true, ncol, nrow, mid, al, be, zz, x, st);
+            if (le != cudaSuccess) return cuda_fail(nullptr, le, "ybwd2 launch");
+        } else {
+            const int g = (ncol + 31) / 32;
+            penta_col_fwd_kernel<<<g, 32, 0, st>>>(nrow, ncol, e, c, d, a, b, rhs, al, be, zz);
+            cudaError_t le = launch_ybwd(ncol, nrow, al, be, zz, x, st);
+            if (le != cudaSuccess) return cuda_fail(nullptr, le, "ybwd launch");
+        }
+    } else {
+        // systems along rows: nsys = nrow, length = ncol; coefficients transposed [col][row]
+        const int mid = (ncol / 2) / 16 * 16;
+        bool fast = aligned && (ncol % 2 == 0) && (nrow % 2 == 0) && ncol >= 64 && nrow >= 32;
+        Maps6 M;
+        CUtensorMap mw[3], mx;
+        if (fast) {
+            for (int k = 0; k < 6; ++k) fast = fast && make_map2d(&M.m[k], in6[k], ncol, nrow, 16, 32, true);
+            const double* w3[3] = {al, be, zz};
+            for (int k = 0; k < 3; ++k) fast = fast && make_map2d(&mw[k], w3[k], nrow, ncol, 32, 16, false);
+            fast = fast && make_map2d(&mx, x, ncol, nrow, 16, 32, true);
+        }
+        if (fast) {
+            constexpr size_t SMF = (size_t)PR_NST * 6 * 32 * 16 * 8 + 8 * PR_NST + 1024;
+            constexpr size_t SMB = (size_t)XT_NST * 4 * 16 * 32 * 8 + 8 * XT_NST + 1024;
+            static bool ready = false;
+            if (!ready) {
+                cudaError_t ee = opt_in_smem(penta_row_fwd2_kernel<PR_NST>, SMF);
+                if (ee == cudaSuccess) ee = opt_in_smem(xbwd2_tma_kernel<XT_NST, false>, SMB);
+                if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
+                ready = true;
+            }
+            const dim3 g((nrow + 31) / 32, 2);
+            penta_row_fwd2_kernel<PR_NST><<<g, 32, SMF, st>>>(M, nrow, ncol, mid, al, be, zz);
+            xbwd2_tma_kernel<XT_NST, false><<<g, 32, SMB, st>>>(mw[0], mw[1], mw[2], mx, mx, ncol, nrow, mid, al, be, zz, nullptr);
+        } else {
+            const int g = (nrow + XT - 1) / XT;
+            const size_t sm = sizeof(double) * PT_ARR * XT * XTP;
+            static bool attr_set = false;
+            if (!attr_set) {
+                cudaError_t ee = cudaFuncSetAttribute(penta_row_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+                if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
+                attr_set = true;
+            }
+            penta_row_fwd_kernel<<<g, 32, sm, st>>>(nrow, ncol, e, c, d, a, b, rhs, al, be, zz);
+            penta_row_bwd_kernel<<<g, 32, 0, st>>>(nrow, ncol, al, be, zz, x);
+        }
     }
     count_launch(2);
     cudaError_t ee = cudaGetLastError();

@@ -214,7 +214,9 @@ ybwd2_plain_kernel(int nx, int ny, int mid, const double* __restrict__ al, const
 // Half 0 marches columns mid-1 .. 0, half 1 columns mid .. nx-1; mid is a multiple of the tile width (16),
 // so the u tiles of the two halves (TMA load, in-place update, TMA store) never overlap.
 // ---------------------------------------------------------------------------------------------
-template <int NST>
+// UPDATE = true: the sweep's S7 (u tile loaded, updated in place, stored; residual reduced into red).
+// UPDATE = false: plain solve, the solution tile is stored through mUout (isolated solver, config 4).
+template <int NST, bool UPDATE>
 __global__ void __launch_bounds__(32)
 xbwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__ CUtensorMap mB,
                  const __grid_constant__ CUtensorMap mZ, const __grid_constant__ CUtensorMap mUin,
@@ -245,11 +247,11 @@ xbwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
             const int s = q % NST;
             unsigned char* d = base + (size_t)s * STAGE;
             const int i0 = tile_col(q);
-            mbar_expect_tx(full + s, STAGE);
+            mbar_expect_tx(full + s, UPDATE ? STAGE : 3 * BOX * 8);
             tma_load_2d(d, &mA, j0, i0, full + s);
             tma_load_2d(d + BOX * 8, &mB, j0, i0, full + s);
             tma_load_2d(d + 2 * BOX * 8, &mZ, j0, i0, full + s);
-            tma_load_2d(d + 3 * BOX * 8, &mUin, i0, j0, full + s);
+            if (UPDATE) tma_load_2d(d + 3 * BOX * 8, &mUin, i0, j0, full + s);
         }
     };
 #pragma unroll
@@ -278,12 +280,16 @@ xbwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
         auto column = [&](int c) {
             const double v = fma(-cf[c * 32], v1, fma(-cf[BOX + c * 32], v2, cf[2 * BOX + c * 32]));
             double* pu = reinterpret_cast<double*>(sur + ((((c >> 1) << 4) ^ sx) + ((c & 1) << 3)));
-            const double uo = *pu;
-            const double un = uo + v;
-            const double rr = fabs(v) * rcp(uo);
-            res = fmax(res, rowok ? rr : 0.0);               // a NaN/inf iterate is caught by `bad`
-            bad |= (rowok && !(un > 0.0 && un <= 1.7976931348623157e308)) ? 1 : 0;
-            *pu = un;
+            if (UPDATE) {
+                const double uo = *pu;
+                const double un = uo + v;
+                const double rr = fabs(v) * rcp(uo);
+                res = fmax(res, rowok ? rr : 0.0);           // a NaN/inf iterate is caught by `bad`
+                bad |= (rowok && !(un > 0.0 && un <= 1.7976931348623157e308)) ? 1 : 0;
+                *pu = un;
+            } else {
+                *pu = v;
+            }
             v2 = v1; v1 = v;
         };
         if (dir == 0) {                                      // always full tiles (mid is a multiple of CS)
@@ -308,6 +314,7 @@ xbwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
         issue(q + NST - 1);                                  // refill the stage of tile q-1
     }
     if (lane == 0) tma_store_wait_all<0>();
+    if (!UPDATE) return;
     if (res != res) res = __longlong_as_double(0x7ff8000000000000LL);
     res = warp_max_nonneg(res);
     bad = __any_sync(0xffffffffu, bad);

@@ -6,6 +6,7 @@
 //                              coefficients are stored transposed, x is written back through a tile.
 #pragma once
 #include "tf_reduce.cuh"
+#include "tf_tma.cuh"
 
 namespace tf {
 
@@ -125,6 +126,180 @@ penta_row_bwd_kernel(int nrow, int ncol, const double* __restrict__ alT, const d
                 if (r0 + rr < nrow) x[(size_t)(r0 + rr) * ncol + col] = sX[rr * XTP + lane];
         }
     }
+}
+
+// =============================================================================================
+// Fast path of the isolated solver (even pitches, lines long enough): the same two-sided elimination and TMA
+// rings as the sweeps, with the six band/right-hand-side arrays streamed by TMA instead of assembled.
+// Traffic per unknown: 48 B in + 24 B out forward, 24 B in + 8 B out backward = 104 B.
+// One warp per CTA; the elimination chain (52 cycles x N/2 rows) is far below the HBM time of these kernels,
+// so no producer warps are needed: the marching warp reads its rows straight from the TMA-filled stages.
+// =============================================================================================
+struct Maps6 { CUtensorMap m[6]; };      // e, c, d, a, b, rhs
+
+// ---- systems = columns (lanes along the contiguous index).  grid (ceil(ncol/32), 2), blockIdx.y = half:
+// half 0 eliminates rows 0 .. mid-1 downwards, half 1 rows nrow-1 .. mid upwards (reversed system: e<->b, c<->a).
+// Coefficients are stored [row][col] like the inputs; ybwd2_tma_kernel / ybwd2_plain_kernel finish the solve.
+template <int NST, int RS>
+__global__ void __launch_bounds__(32)
+penta_col_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int mid, double* __restrict__ al,
+                      double* __restrict__ be, double* __restrict__ zz)
+{
+    extern __shared__ unsigned char raw[];
+    unsigned char* base = align1024(raw);
+    constexpr int BOX = RS * 32;                             // doubles per box
+    double* sm = reinterpret_cast<double*>(base);            // [NST][6][RS][32]
+    uint64_t* full = reinterpret_cast<uint64_t*>(base + (size_t)NST * 6 * BOX * 8);
+    const int lane = threadIdx.x;
+    const int i0 = blockIdx.x * 32, i = i0 + lane;
+    const int dir = blockIdx.y;
+    const int colok = i < ncol ? 1 : 0;
+    const int jmin = dir ? mid : 0, jmax = dir ? nrow : mid;
+    const int nrows = jmax - jmin;
+    const int ntile = (nrows + RS - 1) / RS;
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < NST; ++s) mbar_init(full + s, 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+    auto box_row = [&](int q) { return dir ? nrow - (q + 1) * RS : q * RS; };
+    auto issue = [&](int q) {
+        if (q < ntile && lane == 0) {
+            const int s = q % NST;
+            double* d = sm + (size_t)s * 6 * BOX;
+            mbar_expect_tx(full + s, 6 * BOX * 8);
+#pragma unroll
+            for (int k = 0; k < 6; ++k) tma_load_2d(d + k * BOX, &M.m[k], i0, box_row(q), full + s);
+        }
+    };
+#pragma unroll
+    for (int q = 0; q < NST; ++q) issue(q);
+    Elim2 S = elim2_init();
+    const ptrdiff_t step = dir ? -(ptrdiff_t)ncol : (ptrdiff_t)ncol;
+    ptrdiff_t o = (ptrdiff_t)(dir ? nrow : -1) * ncol + i;   // the row before the first one
+    const int oe = dir ? 4 * BOX : 0, oc = dir ? 3 * BOX : BOX, oa = dir ? BOX : 3 * BOX, ob = dir ? 0 : 4 * BOX;
+    int k = 0;                                               // rows eliminated so far
+    for (int q = 0; q < ntile; ++q) {
+        const int s = q % NST;
+        mbar_wait(full + s, (q / NST) & 1);
+        const int jb = box_row(q);
+        const double* d = sm + (size_t)s * 6 * BOX + lane;
+        if (jb >= jmin && jb + RS <= jmax && q > 0) {
+#pragma unroll
+            for (int rr = 0; rr < RS; ++rr) {
+                const int r = dir ? RS - 1 - rr : rr;
+                double va, vb, vz;
+                elim2_row(S, d[oe + r * 32], d[oc + r * 32], d[2 * BOX + r * 32], d[oa + r * 32], d[ob + r * 32],
+                          d[5 * BOX + r * 32], va, vb, vz);
+                st3_if(colok, al + o, va, be + o, vb, zz + o, vz);
+                o += step;
+            }
+            k += RS;
+        } else {
+            for (int rr = 0; rr < RS; ++rr) {
+                const int r = dir ? RS - 1 - rr : rr;
+                const int j = jb + r;
+                if (j >= jmin && j < jmax) {
+                    double va, vb, vz;
+                    elim2_row(S, d[oe + r * 32], d[oc + r * 32], d[2 * BOX + r * 32], d[oa + r * 32], d[ob + r * 32],
+                              d[5 * BOX + r * 32], va, vb, vz);
+                    st3_if(colok && k > 0, al + o, va, be + o, vb, zz + o, vz);
+                    o += step;
+                    ++k;
+                }
+            }
+        }
+        __syncwarp();
+        issue(q + NST);
+    }
+    double va, vb, vz;
+    elim2_flush(S, va, vb, vz);
+    st3_if(colok, al + o, va, be + o, vb, zz + o, vz);
+}
+
+// ---- systems = rows (contiguous).  lane <-> row of a block of 32 rows, marching along the columns through
+// [32 rows x 16 cols] TMA boxes with the 128-byte swizzle (conflict-free column reads); coefficients are stored
+// TRANSPOSED [col][row] (coalesced).  grid (ceil(nrow/32), 2): half 0 columns 0 .. mid-1 ascending, half 1
+// columns ncol-1 .. mid descending.  xbwd2_tma_kernel<.., false> / penta_row_bwd2_plain_kernel finish the solve.
+template <int NST>
+__global__ void __launch_bounds__(32)
+penta_row_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int mid, double* __restrict__ alT,
+                      double* __restrict__ beT, double* __restrict__ zzT)
+{
+    constexpr int CS = 16;
+    constexpr int TILE = 32 * CS * 8;                        // bytes per array tile (4 KiB, 1024-aligned)
+    extern __shared__ unsigned char raw[];
+    unsigned char* base = align1024(raw);
+    uint64_t* full = reinterpret_cast<uint64_t*>(base + (size_t)NST * 6 * TILE);
+    const int lane = threadIdx.x;
+    const int r0 = blockIdx.x * 32;
+    const int dir = blockIdx.y;
+    const int rowok = r0 + lane < nrow ? 1 : 0;
+    const int imin = dir ? mid : 0, imax = dir ? ncol : mid;
+    const int ncols = imax - imin;
+    const int ntile = (ncols + CS - 1) / CS;
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < NST; ++s) mbar_init(full + s, 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+    auto tile_col = [&](int q) { return dir ? ncol - (q + 1) * CS : q * CS; };
+    auto issue = [&](int q) {
+        if (q < ntile && lane == 0) {
+            const int s = q % NST;
+            unsigned char* d = base + (size_t)s * 6 * TILE;
+            mbar_expect_tx(full + s, 6 * TILE);
+#pragma unroll
+            for (int k = 0; k < 6; ++k) tma_load_2d(d + k * TILE, &M.m[k], tile_col(q), r0, full + s);
+        }
+    };
+#pragma unroll
+    for (int q = 0; q < NST; ++q) issue(q);
+    Elim2 S = elim2_init();
+    const ptrdiff_t step = dir ? -(ptrdiff_t)nrow : (ptrdiff_t)nrow;
+    ptrdiff_t o = (ptrdiff_t)(dir ? ncol : -1) * nrow + r0 + lane;
+    const int oe = dir ? 4 * TILE : 0, oc = dir ? 3 * TILE : TILE, oa = dir ? TILE : 3 * TILE, ob = dir ? 0 : 4 * TILE;
+    const int sx = (lane & 7) << 4;
+    int k = 0;
+    for (int q = 0; q < ntile; ++q) {
+        const int s = q % NST;
+        mbar_wait(full + s, (q / NST) & 1);
+        const int ib = tile_col(q);
+        const unsigned char* d = base + (size_t)s * 6 * TILE + lane * 128;     // this lane's swizzled row
+        auto at = [&](int off, int c) {
+            return *reinterpret_cast<const double*>(d + off + ((((c >> 1) << 4) ^ sx) + ((c & 1) << 3)));
+        };
+        if (ib >= imin && ib + CS <= imax && q > 0) {
+#pragma unroll
+            for (int cc = 0; cc < CS; ++cc) {
+                const int c = dir ? CS - 1 - cc : cc;
+                double va, vb, vz;
+                elim2_row(S, at(oe, c), at(oc, c), at(2 * TILE, c), at(oa, c), at(ob, c), at(5 * TILE, c), va, vb, vz);
+                st3_if(rowok, alT + o, va, beT + o, vb, zzT + o, vz);
+                o += step;
+            }
+            k += CS;
+        } else {
+            for (int cc = 0; cc < CS; ++cc) {
+                const int c = dir ? CS - 1 - cc : cc;
+                const int i = ib + c;
+                if (i >= imin && i < imax) {
+                    double va, vb, vz;
+                    elim2_row(S, at(oe, c), at(oc, c), at(2 * TILE, c), at(oa, c), at(ob, c), at(5 * TILE, c), va, vb, vz);
+                    st3_if(rowok && k > 0, alT + o, va, beT + o, vb, zzT + o, vz);
+                    o += step;
+                    ++k;
+                }
+            }
+        }
+        __syncwarp();
+        issue(q + NST);
+    }
+    double va, vb, vz;
+    elim2_flush(S, va, vb, vz);
+    st3_if(rowok, alT + o, va, beT + o, vb, zzT + o, vz);
 }
 
 }  // namespace tf

@@ -209,7 +209,8 @@ def test_mass_is_bitwise_reproducible(tf):
 
 
 # ------------------------------------------------------------------ isolated pentadiagonal solve (config 4 shape)
-@pytest.mark.parametrize("nrow,ncol", [(64, 64), (33, 70), (130, 37), (3, 40), (40, 3), (257, 129)])
+@pytest.mark.parametrize("nrow,ncol", [(64, 64), (33, 70), (130, 37), (3, 40), (40, 3), (257, 129),
+                                       (96, 200), (130, 70), (66, 1000), (1000, 66), (250, 254)])   # even: TMA path, ragged tiles
 @pytest.mark.parametrize("direction", [0, 1])
 def test_penta_solve_parity(tf, tfo, nrow, ncol, direction):
     import torch
