@@ -36,7 +36,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (0-3); 3 is the headline")
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index; 3 is the headline, 4 the isolated solver (side measurement)")
     ap.add_argument("--fixed-iters", type=int, default=0, help="fixed Newton count per step (0: converge to tol)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -90,14 +90,14 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-NCU_SUMMARY = os.path.join("profiles", "r01_v4_ncu_full_summary.csv")
+NCU_SUMMARY = os.path.join("profiles", "r01_v5_ncu_full_summary.csv")
 NCU_KERNEL = {"y_forward": "yfwd_ws_kernel", "y_backward": "ybwd2_tma_kernel", "x_forward": "xfwd_ws_kernel",
               "x_backward_update": "xbwd2_tma_kernel"}
 
 
 def ncu_traffic(kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` at 8192^2, from the committed
-    ncu --set full summary (profiles/r01_v4_ncu.md names the command), or None."""
+    ncu --set full summary (profiles/r01_v5_ncu.md names the command), or None."""
     import csv
     p = os.path.join(ROOT, NCU_SUMMARY)
     try:
@@ -290,9 +290,51 @@ def run_b200(args, cfg):
         dist.destroy_process_group()
 
 
+# ----------------------------------------------------------------------------------------- config 4 (side measurement)
+def run_penta(args, cfg):
+    """Isolated batched pentadiagonal solve (BASELINE.json config 4), both directions, device-resident inputs of
+    the config's recipe drawn on the GPU (torch generator, seed 4): not the headline line, a kernel measurement."""
+    import torch
+    from paper_1806_10550_b200 import tf
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    n = cfg["nrow"]
+    gen = torch.Generator(device="cuda").manual_seed(cfg["seed"])
+    U = lambda lo, hi: torch.rand(n, n, dtype=torch.float64, device="cuda", generator=gen) * (hi - lo) + lo
+    e, c, a, b, y = U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1)
+    d = 1 + e.abs() + c.abs() + a.abs() + b.abs() + U(0, 1)
+    ws = torch.empty(tf.lib().tf_penta_workspace_bytes(n, n), dtype=torch.uint8, device="cuda")
+    out = torch.empty_like(e)
+    peak, peak_src = measured_peak()
+    res = {}
+    for direction, name in ((1, "along_columns_y"), (0, "along_rows_x")):
+        for _ in range(max(args.warmup, 3)):
+            tf.penta_solve(direction, e, c, d, a, b, y, out=out, workspace=ws)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        ev0.record()
+        for _ in range(args.steps):
+            tf.penta_solve(direction, e, c, d, a, b, y, out=out, workspace=ws)
+        ev1.record()
+        torch.cuda.synchronize()
+        ms = ev0.elapsed_time(ev1) / args.steps
+        res[name] = {"ms": ms, "unknowns_per_s": n * n / (ms * 1e-3), "alg_gbs": 104 * n * n / (ms * 1e-3) / 1e9,
+                     "frac_of_peak": 104 * n * n / (ms * 1e-3) / 1e9 / peak}
+    print(json.dumps({"metric": "pentadiagonal unknowns/s (fp64), isolated solve", "unit": "unknowns/s", "n_gpus": 1,
+                      "value": min(r["unknowns_per_s"] for r in res.values()), "steps": args.steps, "warmup": max(args.warmup, 3),
+                      "dtype": "f64", "data": "synthetic (config 4 recipe drawn on the GPU)", "higher_is_better": True,
+                      "config": {"workload": cfg["name"], "systems": n, "length": n, "alg_bytes_per_unknown": 104,
+                                 "l2": "inputs 6 x 2 GiB >> 126 MB L2"},
+                      "directions": res, "peak": peak, "peak_source": peak_src}), flush=True)
+
+
 def main():
     args = parse()
     cfg = inputs.config(args.config)
+    if args.config == 4:
+        return run_penta(args, cfg) if args.impl == "b200" else print(json.dumps(
+            {"impl": "reference", "unavailable": "config 4 is a side measurement of the B200 arm only"}))
     if args.impl == "reference":
         run_reference(args, cfg)
     else:
