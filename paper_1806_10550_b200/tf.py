@@ -178,6 +178,32 @@ class ThinFilm:
         return h.data_ptr(), (1 if h.is_cuda else 0), h
 
 
+def advance_adaptive(ctx, dt, n_accept, grow=1.1, shrink=0.5, dt_max=0.1, dt_min=1e-12, max_attempts=None):
+    """The adaptive time-stepping controller of Fig. 1 around tf_step: a step whose Newton
+    iteration does not converge within max_iter is rejected by the library (state unchanged) and retried with
+    dt*shrink; after an accepted step dt grows by `grow`, bounded by dt_max.  The factors are
+    BASELINE.json config 2's (the paper gives none).  Host logic only (S8); every step runs in the kernels.
+    Returns (t, dt_next, history) with history = [(dt, status, newton_iters, residual), ...]."""
+    t, hist, accepted = 0.0, [], 0
+    attempts = 0
+    max_attempts = max_attempts or 50 * n_accept
+    while accepted < n_accept:
+        attempts += 1
+        if attempts > max_attempts:
+            raise TfError(NOT_CONVERGED, "advance_adaptive", "too many attempts")
+        st, it, res = ctx.step(dt)
+        hist.append((dt, st, it, res))
+        if st == OK:
+            accepted += 1
+            t += dt
+            dt = min(dt * grow, dt_max)
+        else:
+            dt *= shrink
+            if dt < dt_min:
+                raise TfError(NOT_CONVERGED, "advance_adaptive", f"dt fell below {dt_min}")
+    return t, dt, hist
+
+
 def penta_solve(direction, e, c, d, a, b, rhs, out=None, workspace=None, stream=None):
     """tf_penta_solve on torch CUDA float64 tensors [nrow][ncol]; direction 0: rows are systems, 1: columns.
     Enqueues on the current stream and returns `out` without synchronising."""

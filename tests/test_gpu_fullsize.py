@@ -170,3 +170,48 @@ def test_penta_solve_full_length_systems(tf, tfo, direction):
     Ax[:, :-2] += b[:, :-2] * xs[:, 2:]
     normA = np.max(np.abs(e) + np.abs(c) + np.abs(d) + np.abs(a) + np.abs(b))
     assert np.max(np.abs(Ax - y)) / (normA * np.max(np.abs(xs)) + np.max(np.abs(y))) <= 1e-14
+
+
+# ------------------------------------------------------------------ config 2 at full size: adaptive controller
+def test_config2_4096_adaptive_run(tf, tfo):
+    """Config 2 (4096^2, uniform 0.12 film with 16 Gaussian depressions, adaptive dt from 1e-3): the controller of
+    Fig. 1 on the GPU path.  Physics of these parameters: Pi'(0.12) < 0, the depressions
+    heal, no step is rejected and dt climbs to its cap.  Checked: the accept sequence, dt growth, mass, healing;
+    and the field after three accepted steps (fixed iteration count) on sampled windows against the oracle."""
+    cfg = inputs.config(2)
+    n = cfg["nx"]
+    h = inputs.initial_condition(cfg)
+    assert h.min() > 0.06 and abs(h.max() - 0.12) < 1e-12
+    g = tf.ThinFilm(n, n, cfg["dx"], cfg["dy"], cfg["kappa"], cfg["hstar"], cfg["n"], cfg["m"])
+    # (a) sampled parity of the first three steps, dt = 1e-3 * 1.1^k, 5 fixed iterations each
+    g.set_newton(cfg["tol"], cfg["max_iter"], 5)
+    g.set_state(h)
+    dts = [cfg["dt"] * cfg["grow"] ** k for k in range(3)]
+    for dt in dts:
+        assert g.step(dt)[0] == 0
+    u3 = g.get_state()
+    jc, ic = np.unravel_index(np.argmin(h), h.shape)            # the deepest depression
+    o = tfo.ThinFilmOracle(W, W, cfg["dx"], cfg["dy"], cfg["kappa"], cfg["hstar"], cfg["n"], cfg["m"])
+    o.set_newton(cfg["tol"], cfg["max_iter"], 5)
+    for (j0, i0) in ((0, 0), (n - W, n - W), (min(max(jc - W // 2, 0), n - W), min(max(ic - W // 2, 0), n - W))):
+        o.set_state(np.ascontiguousarray(h[j0:j0 + W, i0:i0 + W]))
+        for dt in dts:
+            assert o.step(dt)[0] == 0
+        uo = o.get_state()
+        ja, jb = (0 if j0 == 0 else MARGIN), (W if j0 + W == n else W - MARGIN)
+        ia, ib = (0 if i0 == 0 else MARGIN), (W if i0 + W == n else W - MARGIN)
+        d = np.max(np.abs(u3[j0 + ja:j0 + jb, i0 + ia:i0 + ib] - uo[ja:jb, ia:ib])) / np.max(np.abs(uo))
+        assert d <= 1e-11, (j0, i0, d)
+    # (b) the adaptive run itself: 60 accepted steps from the initial film
+    g.set_newton(cfg["tol"], cfg["max_iter"], 0)
+    g.set_state(h)
+    m0 = g.mass()
+    t, dt_next, hist = tf.advance_adaptive(g, cfg["dt"], 60, cfg["grow"], cfg["shrink"], cfg["dt_max"], cfg["dt_min"])
+    assert all(st == 0 for _, st, _, _ in hist) and len(hist) == 60          # nothing rejected
+    assert all(it <= cfg["max_iter"] and res < cfg["tol"] for _, _, it, res in hist)
+    assert abs(hist[1][0] / hist[0][0] - cfg["grow"]) < 1e-12 and dt_next == cfg["dt_max"]   # 1e-3 * 1.1^49 > 0.1
+    assert abs(t - sum(x[0] for x in hist)) < 1e-12
+    u = g.get_state()
+    assert abs(g.mass() - m0) <= 1e-13 * m0
+    assert u.min() > h.min() and u.max() <= 0.12 + 1e-9                     # the depressions heal
+    g.close()
