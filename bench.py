@@ -110,10 +110,11 @@ def ncu_traffic(kernel):
 
 
 # ----------------------------------------------------------------------------------------- CPU oracle legs
-def oracle_sample_run(cfg, n, steps, warmup, fixed_iters):
-    """Times the CPU oracle AS IT STANDS (serial build) on an n x n cut of the config's recipe."""
+def oracle_sample_run(cfg, n, steps, warmup, fixed_iters, omp=False):
+    """Times the CPU oracle AS IT STANDS (serial build; omp=True: its OpenMP build, one thread per line) on an
+    n x n cut of the config's recipe."""
     from oracle import tfo
-    o = tfo.ThinFilmOracle(n, n, cfg["dx"], cfg["dy"], cfg["kappa"], cfg["hstar"], cfg["n"], cfg["m"])
+    o = tfo.ThinFilmOracle(n, n, cfg["dx"], cfg["dy"], cfg["kappa"], cfg["hstar"], cfg["n"], cfg["m"], omp=omp)
     o.set_newton(cfg["tol"], cfg["max_iter"], fixed_iters)
     o.set_state(inputs.initial_condition(cfg, n, n))
     for _ in range(warmup):
@@ -124,7 +125,7 @@ def oracle_sample_run(cfg, n, steps, warmup, fixed_iters):
         st, it, _ = o.step(cfg["dt"])
         iters += it
     dt = time.perf_counter() - t0
-    return dict(seconds=dt, iters=iters, pts=n * n, steps=steps, cores=tfo.num_threads(False))
+    return dict(seconds=dt, iters=iters, pts=n * n, steps=steps, cores=tfo.num_threads(omp))
 
 
 def run_reference(args, cfg):
@@ -284,6 +285,11 @@ def run_b200(args, cfg):
             "value": r["pts"] * r["steps"] / r["seconds"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
             "sample": f"{n}x{n} cut of {cfg['name']} (same dx, dt, IC recipe, seed), first step, {r['iters']} Newton "
                       f"iterations, {r['seconds']:.1f} s",
+            "point_iterations_per_s": r["pts"] * r["iters"] / r["seconds"]}
+        r = oracle_sample_run(cfg, n, 1, 0, args.fixed_iters, omp=True)      # same sample, the oracle's OpenMP build
+        line["cpu_baseline_all_cores"] = {
+            "value": r["pts"] * r["steps"] / r["seconds"], "unit": UNIT, "cores": r["cores"], "kind": "oracle (OpenMP build)",
+            "sample": f"{n}x{n} cut, first step, {r['iters']} Newton iterations, {r['seconds']:.1f} s",
             "point_iterations_per_s": r["pts"] * r["iters"] / r["seconds"]}
     print(json.dumps(line), flush=True)
     if world > 1:

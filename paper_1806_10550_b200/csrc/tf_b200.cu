@@ -45,6 +45,7 @@ struct tf_ctx {
     double *scal;                              // [8] : scal[0] mass, (int*)(scal+1) flag
     double *pinned;                            // [4] host pinned readback
     int mid_y, mid_x;                          // split rows / columns of the two-sided sweeps
+    int num_sms;
     bool tma_y, tma_x;                         // TMA rings usable (row pitch multiple of 16 B, grid >= one box)
     CUtensorMap mY[3], mX[3];                  // alpha,beta,z as [ny][nx] (box RS x 32) and as [nx][ny] (box CS x 32)
     CUtensorMap mU[2];                         // the two state buffers as [ny][nx], box 32 x 16, 128-byte swizzle
@@ -191,6 +192,39 @@ constexpr int YW_NP = 3, YW_RP = 8, YW_NSTG = 4;   // yfwd: consumer warp 0 + 3 
 
 constexpr int XW_NP = 4, XW_NSTG = 3;              // xfwd: per sub-problem 1 consumer + 4 producer warps, ring of 3 slots of 14 columns (48 KiB)
 
+// forward kernels: NSUB sub-problems per CTA (4: two strips/blocks x two halves; 2: one x two halves)
+template <int N, int M, bool FIRST, int NSUB>
+cudaError_t launch_yfwd(tf_ctx* c, const CUtensorMap& mu, int tma, const Params& P, const Dir& DX, const Dir& DY,
+                        const double* src, int grid)
+{
+    constexpr size_t SM = NSUB * (size_t)YW_NSTG * 5 * YW_RP * 32 * 8 + NSUB * YW_NP * (size_t)(2 * YW_RP + 4) * 32 * 8 +
+                          (2 * NSUB * YW_NSTG + NSUB * YW_NP) * 8;
+    auto kern = yfwd_ws_kernel<N, M, FIRST, YW_NP, YW_RP, YW_NSTG, NSUB>;
+    static bool ready = false;
+    if (!ready) {
+        cudaError_t e = opt_in_smem(kern, SM);
+        if (e != cudaSuccess) return e;
+        ready = true;
+    }
+    kern<<<grid, 32 * NSUB * (YW_NP + 1), SM, c->stream>>>(mu, c->mBn, tma, P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz);
+    return cudaGetLastError();
+}
+
+template <int N, int M, int NSUB>
+cudaError_t launch_xfwd(tf_ctx* c, const Params& P, const Dir& DX, const double* src, int grid)
+{
+    constexpr size_t SM = NSUB * ((size_t)XW_NSTG * 5 * XW_CK * XW_LD * 8 + 16 * XW_NSTG);
+    auto kern = xfwd_ws_kernel<N, M, XW_NP, XW_NSTG, NSUB>;
+    static bool ready = false;
+    if (!ready) {
+        cudaError_t e = opt_in_smem(kern, SM);
+        if (e != cudaSuccess) return e;
+        ready = true;
+    }
+    kern<<<grid, 32 * NSUB * (XW_NP + 1), SM, c->stream>>>(P, DX, c->mid_x, src, c->w, c->al, c->be, c->zz);
+    return cudaGetLastError();
+}
+
 // one pseudo-Newton iteration k: reads src (u^n if k == 0 else uk), writes uk, red[2k..2k+1]
 template <int N, int M>
 cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
@@ -198,41 +232,31 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
     const Params& P = c->P;
     const Dir DX = make_dir(s, P.dx), DY = make_dir(s, P.dy);
     const double* src = (k == 0) ? c->u : c->uk;
-    const int gy = ((P.nx + YW_VALID - 1) / YW_VALID + 1) / 2;     // one CTA = two strips x two halves
+    // one CTA = NSUB sub-problems: two strips x two halves, or one strip x two halves when that still leaves SMs idle
+    const int nstrip = (P.nx + YW_VALID - 1) / YW_VALID;
     cudaEvent_t* ev = (c->profiling && slot >= 0) ? c->ev + 5 * slot : nullptr;
     if (ev) cudaEventRecord(ev[0], c->stream);
     {
-        constexpr size_t SM = 4 * (size_t)YW_NSTG * 5 * YW_RP * 32 * 8 + 4 * YW_NP * (size_t)(2 * YW_RP + 4) * 32 * 8 +
-                              (8 * YW_NSTG + 4 * YW_NP) * 8;
-        static bool ready = false;
-        if (!ready) {
-            cudaError_t e = opt_in_smem(yfwd_ws_kernel<N, M, true, YW_NP, YW_RP, YW_NSTG>, SM);
-            if (e == cudaSuccess) e = opt_in_smem(yfwd_ws_kernel<N, M, false, YW_NP, YW_RP, YW_NSTG>, SM);
-            if (e != cudaSuccess) return e;
-            ready = true;
-        }
-        const int nthr = 128 * (YW_NP + 1);
         const CUtensorMap& mu = c->mUy[src == c->ubuf[0] ? 0 : 1];
         const int tma = c->tma_yf ? 1 : 0;
-        if (k == 0)
-            yfwd_ws_kernel<N, M, true, YW_NP, YW_RP, YW_NSTG><<<gy, nthr, SM, c->stream>>>(mu, c->mBn, tma, P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz);
+        cudaError_t e;
+        if (nstrip > c->num_sms)
+            e = k == 0 ? launch_yfwd<N, M, true, 4>(c, mu, tma, P, DX, DY, src, (nstrip + 1) / 2)
+                       : launch_yfwd<N, M, false, 4>(c, mu, tma, P, DX, DY, src, (nstrip + 1) / 2);
         else
-            yfwd_ws_kernel<N, M, false, YW_NP, YW_RP, YW_NSTG><<<gy, nthr, SM, c->stream>>>(mu, c->mBn, tma, P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz);
+            e = k == 0 ? launch_yfwd<N, M, true, 2>(c, mu, tma, P, DX, DY, src, nstrip)
+                       : launch_yfwd<N, M, false, 2>(c, mu, tma, P, DX, DY, src, nstrip);
+        if (e != cudaSuccess) return e;
     }
     if (ev) cudaEventRecord(ev[1], c->stream);
     cudaError_t le = launch_ybwd2(c->mY, c->tma_y, P.nx, P.ny, c->mid_y, c->al, c->be, c->zz, c->w, c->stream);
     if (le != cudaSuccess) return le;
     if (ev) cudaEventRecord(ev[2], c->stream);
-    const int gx = ((P.ny + XW_R - 1) / XW_R + 1) / 2;           // one CTA = two row blocks x two halves
     {
-        constexpr size_t SM = 4 * ((size_t)XW_NSTG * 5 * XW_CK * XW_LD * 8 + 16 * XW_NSTG);
-        static bool ready = false;
-        if (!ready) {
-            cudaError_t e = opt_in_smem(xfwd_ws_kernel<N, M, XW_NP, XW_NSTG>, SM);
-            if (e != cudaSuccess) return e;
-            ready = true;
-        }
-        xfwd_ws_kernel<N, M, XW_NP, XW_NSTG><<<gx, 128 * (XW_NP + 1), SM, c->stream>>>(P, DX, c->mid_x, src, c->w, c->al, c->be, c->zz);
+        const int nblk = (P.ny + XW_R - 1) / XW_R;
+        cudaError_t e = nblk > c->num_sms ? launch_xfwd<N, M, 4>(c, P, DX, src, (nblk + 1) / 2)
+                                          : launch_xfwd<N, M, 2>(c, P, DX, src, nblk);
+        if (e != cudaSuccess) return e;
     }
     if (ev) cudaEventRecord(ev[3], c->stream);
     le = launch_xbwd2(c->mX, c->mU[src == c->ubuf[0] ? 0 : 1], c->mU[c->uk == c->ubuf[0] ? 0 : 1], c->tma_x, P.nx, P.ny,
@@ -321,6 +345,11 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
         return fail(nullptr, TF_ERR_ALLOC, std::string("cudaMallocHost: ") + cudaGetErrorString(e));
     }
     c->ubuf[0] = c->u; c->ubuf[1] = c->uk;
+    {
+        int dev = 0, sms = 148;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        c->num_sms = sms;
+    }
     // split index of the two-sided sweeps: half the line, on a 16-row tile boundary when the line is long enough
     c->mid_y = ny >= 64 ? (ny / 2) / 16 * 16 : ny / 2;
     c->mid_x = nx >= 64 ? (nx / 2) / 16 * 16 : nx / 2;

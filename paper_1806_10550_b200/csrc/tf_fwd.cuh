@@ -101,16 +101,17 @@ __device__ __forceinline__ void y_advance(YState& S, int j, double hp2, const Pa
 // c % NCH, so RP can be large (the two warm-up rows of a chunk are amortised over RP rows) while the ring
 // stays small (4 CTAs per SM).  Inputs are pulled into L2 a few chunks ahead by prefetch hints.
 // ---------------------------------------------------------------------------------------------
-template <int N, int M, bool FIRST, int NP, int RP, int NCH>
-__global__ void __launch_bounds__(128 * (NP + 1), 1)
+template <int N, int M, bool FIRST, int NP, int RP, int NCH, int NSUB>
+__global__ void __launch_bounds__(32 * NSUB * (NP + 1), 1)
 yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ CUtensorMap mB, int use_tma,
                Params P, Dir DX, Dir DY, int mid, const double* __restrict__ u, double* __restrict__ bn,
                double* __restrict__ al, double* __restrict__ be, double* __restrict__ zz)
 {
-    // One CTA per SM: 4 sub-problems q = warp & 3 (two adjacent strips x two halves), each with its own
+    // One CTA per SM: NSUB = 4 sub-problems q = warp % 4 (two adjacent strips x two halves), each with its own
     // ring and its own consumer + NP producers.  Warps w, w+4, w+8, ... share an SM sub-partition, so every
     // sub-partition gets exactly one consumer and NP producers (the consumers' dependent chains and the
-    // producers' fp64 work are spread evenly over the four issue ports).
+    // producers' fp64 work are spread evenly over the four issue ports).  Grids with at most one strip per SM
+    // use NSUB = 2 (one strip x two halves per CTA) so that twice as many SMs work.
     // Shared memory: 4 rings [NCH][5][RP][32] | 4*NP input stagings [(RP+4) + RP][32] | mbarriers.
     constexpr int SV = RP * 32;                       // doubles per value plane of a slot
     constexpr size_t RING = (size_t)NCH * 5 * SV * 8;                // bytes per sub-problem
@@ -118,22 +119,22 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
     extern __shared__ __align__(128) unsigned char raw[];
     const int nx = P.nx, ny = P.ny;
     const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
-    const int q = warp & 3, role = warp >> 2;         // role 0: consumer, 1..NP: producers
+    const int q = warp % NSUB, role = warp / NSUB;    // role 0: consumer, 1..NP: producers
     double* sm = reinterpret_cast<double*>(raw + q * RING);          // [NCH][5][RP][32]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(raw + 4 * RING + 4 * NP * STG);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(raw + NSUB * RING + NSUB * NP * STG);
     uint64_t* full = bars + q * 2 * NCH;
     uint64_t* empty = full + NCH;
     if (role == 0 && lane == 0) {
 #pragma unroll
         for (int s = 0; s < NCH; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, 1); }
-        for (int p = 0; p < NP; ++p) mbar_init(bars + 8 * NCH + q * NP + p, 1);
+        for (int p = 0; p < NP; ++p) mbar_init(bars + 2 * NSUB * NCH + q * NP + p, 1);
         mbar_fence_init();
     }
     __syncthreads();
-    const int strip = 2 * blockIdx.x + (q & 1);
+    const int strip = (NSUB / 2) * blockIdx.x + (q % (NSUB / 2));
     if (strip * YW_VALID >= nx) return;               // odd strip count: the last CTA has one strip
     const int i = strip * YW_VALID - 2 + lane;
-    const int dir = q >> 1;                           // 0: rows 0 .. mid-1 downwards, 1: rows ny-1 .. mid upwards
+    const int dir = q / (NSUB / 2);                   // 0: rows 0 .. mid-1 downwards, 1: rows ny-1 .. mid upwards
     const int nrows = dir ? ny - mid : mid;           // rows of this half
     const int nchunk = (nrows + RP - 1) / RP;
     const int jmin = dir ? mid : 0, jmax = dir ? ny : mid;    // this half owns rows [jmin, jmax)
@@ -150,8 +151,8 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
         // chunk ahead (right after the previous chunk's rows were copied to registers), so that the chunk's
         // global-memory latency overlaps the assembly of the chunk before it.  Boundary chunks, and grids whose
         // row pitch is not a multiple of 16 bytes, load directly.
-        double* stg = reinterpret_cast<double*>(raw + 4 * RING + (size_t)(q * NP + pw) * STG);
-        uint64_t* sbar = bars + 8 * NCH + q * NP + pw;
+        double* stg = reinterpret_cast<double*>(raw + NSUB * RING + (size_t)(q * NP + pw) * STG);
+        uint64_t* sbar = bars + 2 * NSUB * NCH + q * NP + pw;
         const int col0 = strip * YW_VALID - 2;
         const int srcl = lane + (ic - i);                      // lane holding my ghost column (edge strips)
         const bool edge = (col0 < 0) || (col0 + 32 > nx);
@@ -314,8 +315,8 @@ constexpr int XW_CK = 14;            // columns per ring slot
 constexpr int XW_R = 28;             // rows per block
 constexpr int XW_LD = 29;            // slot row pitch in doubles (odd)
 
-template <int N, int M, int NP, int NCH>
-__global__ void __launch_bounds__(128 * (NP + 1), 1)
+template <int N, int M, int NP, int NCH, int NSUB>
+__global__ void __launch_bounds__(32 * NSUB * (NP + 1), 1)
 xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const double* __restrict__ w,
                double* __restrict__ alT, double* __restrict__ beT, double* __restrict__ zzT)
 {
@@ -326,7 +327,7 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
     const unsigned FULL = 0xffffffffu;
     const int nx = P.nx, ny = P.ny;
     const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
-    const int q = warp & 3, role = warp >> 2;         // role 0: consumer, 1..NP: producers
+    const int q = warp % NSUB, role = warp / NSUB;    // role 0: consumer, 1..NP: producers (NSUB: see yfwd_ws_kernel)
     double* sm = reinterpret_cast<double*>(raw + q * RING);          // [NCH][5][CK][LD]
     uint64_t* full = reinterpret_cast<uint64_t*>(raw + q * RING + (size_t)NCH * 5 * SV * 8);
     uint64_t* empty = full + NCH;
@@ -336,9 +337,9 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
         mbar_fence_init();
     }
     __syncthreads();
-    const int j0 = (2 * blockIdx.x + (q & 1)) * XW_R;
+    const int j0 = ((NSUB / 2) * blockIdx.x + (q % (NSUB / 2))) * XW_R;
     if (j0 >= ny) return;
-    const int dir = q >> 1;
+    const int dir = q / (NSUB / 2);
     const int ncols = dir ? nx - mid : mid;           // columns of this half
     const int ntile = (ncols + XW_CT - 1) / XW_CT;
     const int imin = dir ? mid : 0, imax = dir ? nx : mid;
