@@ -113,6 +113,9 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
     // producers' fp64 work are spread evenly over the four issue ports).  Grids with at most one strip per SM
     // use NSUB = 2 (one strip x two halves per CTA) so that twice as many SMs work.
     // Shared memory: 4 rings [NCH][5][RP][32] | 4*NP input stagings [(RP+4) + RP][32] | mbarriers.
+    // NCH >= NP keeps every producer less than one ring lap ahead of the consumer, which the parity waits need
+    // (a waiter two phases ahead would see the wrong parity as "done"; NP = 4, NCH = 3 hangs).
+    static_assert(NCH >= NP, "ring slots must not be fewer than producers");
     constexpr int SV = RP * 32;                       // doubles per value plane of a slot
     constexpr size_t RING = (size_t)NCH * 5 * SV * 8;                // bytes per sub-problem
     constexpr size_t STG = (size_t)(2 * RP + 4) * 32 * 8;            // bytes per producer: rows of u, then rows of b^n
