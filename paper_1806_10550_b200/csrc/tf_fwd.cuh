@@ -11,6 +11,7 @@
 #pragma once
 #include "tf_device.cuh"
 #include "tf_tma.cuh"
+#include <type_traits>
 
 #ifndef TF_DBG_MODE
 #define TF_DBG_MODE 0        // experiments only (_work/): 1 = producers skip assembly, 2 = consumer skips the recurrence
@@ -374,36 +375,48 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
             mbar_wait(empty + g0 % NCH, ((g0 / NCH) & 1) ^ 1);
             mbar_wait(empty + g1 % NCH, ((g1 / NCH) & 1) ^ 1);
             double* st = sm + (size_t)((slot_sel ? g1 : g0) % NCH) * 5 * SV + kc * XW_LD;
-#pragma unroll
-            for (int k = 0; k < NRMAX; ++k) {
+            // one row of the tile; INTERIOR: every face of the tile is an interior, unfolded face and every
+            // column belongs to this half -- no boundary selects (all tiles but the first, last and the split one)
+            auto row = [&](auto interior_tag, int k) {
+                constexpr bool INTERIOR = decltype(interior_tag)::value;
                 const int r = pw + k * NP;
-                if (r < XW_R) {
-                    const double h0 = hq[k];
-                    const double hm1 = __shfl_up_sync(FULL, h0, 1);
-                    const double hp1 = __shfl_down_sync(FULL, h0, 1), hp2 = __shfl_down_sync(FULL, h0, 2);
-                    const Cell c0 = cell_functions<N, M>(h0, P);
+                const double h0 = hq[k];
+                const double hm1 = __shfl_up_sync(FULL, h0, 1);
+                const double hp1 = __shfl_down_sync(FULL, h0, 1), hp2 = __shfl_down_sync(FULL, h0, 2);
+                const Cell c0 = cell_functions<N, M>(h0, P);
 #if XW_RECOMPUTE_C1
-                    const Cell c1 = cell_functions<N, M>(hp1, P);   // cheaper than 8 shuffles: the LSU pipe, not fp64, bounds this kernel
+                const Cell c1 = cell_functions<N, M>(hp1, P);   // cheaper than 8 shuffles: the LSU pipe, not fp64, bounds this kernel
 #else
-                    Cell c1;
-                    c1.f0 = __shfl_down_sync(FULL, c0.f0, 1); c1.f1 = __shfl_down_sync(FULL, c0.f1, 1);
-                    c1.g0 = __shfl_down_sync(FULL, c0.g0, 1); c1.g1 = __shfl_down_sync(FULL, c0.g1, 1);
+                Cell c1;
+                c1.f0 = __shfl_down_sync(FULL, c0.f0, 1); c1.f1 = __shfl_down_sync(FULL, c0.f1, 1);
+                c1.g0 = __shfl_down_sync(FULL, c0.g0, 1); c1.g1 = __shfl_down_sync(FULL, c0.g1, 1);
 #endif
-                    Face fp = face_partials(hm1, hp2, hp1 - h0, c0.f0 + c1.f0, c0.f1 + c1.f1, c0, c1, DX);
+                Face fp = face_partials(hm1, hp2, hp1 - h0, c0.f0 + c1.f0, c0.f1 + c1.f1, c0, c1, DX);
+                if (!INTERIOR) {
                     if (i == 0) fp.p1 -= fp.A;
                     if (i == nx - 2) fp.p2 += fp.A;
                     if (!face_ok) { fp.A = 0.0; fp.p1 = 0.0; fp.p2 = 0.0; }
-                    Face fm;
-                    fm.A = __shfl_up_sync(FULL, fp.A, 1); fm.p1 = __shfl_up_sync(FULL, fp.p1, 1);
-                    fm.p2 = __shfl_up_sync(FULL, fp.p2, 1);
-                    if (col_ok) {
-                        st[r] = dir ? fm.A : fp.A;
-                        st[SV + r] = -fp.A - fm.p1;
-                        st[2 * SV + r] = 1.0 + fp.p1 - fm.p2;
-                        st[3 * SV + r] = fp.p2 - fm.A;
-                        st[4 * SV + r] = wq[k];
-                    }
                 }
+                Face fm;
+                fm.A = __shfl_up_sync(FULL, fp.A, 1); fm.p1 = __shfl_up_sync(FULL, fp.p1, 1);
+                fm.p2 = __shfl_up_sync(FULL, fp.p2, 1);
+                if (INTERIOR ? lane_ok : col_ok) {
+                    st[r] = dir ? fm.A : fp.A;
+                    st[SV + r] = -fp.A - fm.p1;
+                    st[2 * SV + r] = 1.0 + fp.p1 - fm.p2;
+                    st[3 * SV + r] = fp.p2 - fm.A;
+                    st[4 * SV + r] = wq[k];
+                }
+            };
+            const bool interior = (ilo >= 3) && (ilo + XW_CT + 2 <= nx - 2) && (ilo >= imin) && (ilo + XW_CT <= imax);
+            if (interior) {
+#pragma unroll
+                for (int k = 0; k < NRMAX; ++k)
+                    if (pw + k * NP < XW_R) row(std::true_type{}, k);
+            } else {
+#pragma unroll
+                for (int k = 0; k < NRMAX; ++k)
+                    if (pw + k * NP < XW_R) row(std::false_type{}, k);
             }
             __syncwarp();
             if (lane == 0) { mbar_arrive(full + g0 % NCH); mbar_arrive(full + g1 % NCH); }
