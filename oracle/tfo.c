@@ -17,8 +17,9 @@
  * 13-point Crank-Nicolson solve of the linear model (1.6), finite-difference
  * Jacobian, column sums, mass conservation, dispersion relation (1.4), dt-halving
  * order, G(u)=0 at convergence, fixed point, transpose symmetry.
- * Parity unpinned: nothing in this file (NLC elastic term / polymer model are not
- * implemented; they are out of scope).
+ * The NLC (1.8)-(1.9) and polymer (1.12) disjoining pressures are pinned by finite
+ * differences of Pi(h) as the paper defines it, the finite-difference Jacobian, G(u) = 0 and the dispersion
+ * relation (tests/test_oracle_models.py).  Parity unpinned: nothing in this file.
  *
  * The optional "#pragma omp parallel for" lines are no-ops unless compiled with
  * -fopenmp (second build, used only for the all-core timed baseline).
@@ -33,8 +34,12 @@ enum { TFO_OK = 0, TFO_NOT_CONVERGED = 1, TFO_ERR_INVALID_ARG = -1,
 typedef struct tfo_ctx {
     int nx, ny;
     double dx, dy;
-    /* model: 0 = thin film (1.7) with power-law Pi (K-term of (1.8)); 1 = linear (1.6) */
+    /* model: 0 = thin film (1.7) with power-law Pi (K-term of (1.8)); 1 = linear (1.6);
+     *        2 = thin film (1.7) with Pi_NLC (1.8)-(1.9); 3 = thin film (1.7) with Pi_POL (1.12) */
     int model;
+    double cap0, cap1;               /* models 2,3: f0 = cap0 h^3, f1 = cap1 h^3 Pi'(h)  (reading R19)      */
+    double pk, pb, pn, pbeta, pw;    /* NLC: K, b, N, beta, w of (1.8)-(1.9), (1.11)                      */
+    double qc, qa1, qa2, qd;         /* polymer: C, A_SiOx, A_Si, d of (1.12)-(1.13)                      */
     double kappa, hstar; int n, m;   /* Pi(h) = kappa[(hstar/h)^n - (hstar/h)^m]   */
     double c0, c1;                   /* linear model f0 = c0, f1 = c1  */
     double tol; int max_iter, fixed_iters;
@@ -56,9 +61,69 @@ static double ipow(double x, int p) { double r = 1.0; for (int k = 0; k < p; ++k
  *   Pi''(h) = kappa[ n(n+1) h*^n / h^(n+2) - m(m+1) h*^m / h^(m+2) ].
  * Linear model (1.6): f0 = c0, f1 = c1, derivatives 0.
  */
+
+#define TFO_PI 3.14159265358979323846
+
+/* Pi(h) exactly as the paper defines it -- used by the pins to difference, never by the solver.
+ *   NLC, (1.8)-(1.9):  Pi = K[(b/h)^3 - (b/h)^2] + (N/2) [m(h)/h]^2,
+ *        m = g h^2/(h^2 + beta^2),  g = (1/2)[1 + tanh((h - 2b)/w)];
+ *   polymer, (1.12):    Pi = -d psi/dh,  psi = C/h^8 - A1/(12 pi h^2) + (A1 - A2)/(12 pi (h+d)^2). */
+static double pressure(const tfo_ctx *c, double h)
+{
+    if (c->model == 2) {
+        double r = c->pb / h;
+        double g = 0.5 * (1.0 + tanh((h - 2.0 * c->pb) / c->pw));
+        double m = g * h * h / (h * h + c->pbeta * c->pbeta);
+        return c->pk * (r * r * r - r * r) + 0.5 * c->pn * (m / h) * (m / h);
+    }
+    if (c->model == 3) {
+        double hd = h + c->qd;
+        return 8.0 * c->qc / pow(h, 9) - c->qa1 / (6.0 * TFO_PI * h * h * h) + (c->qa1 - c->qa2) / (6.0 * TFO_PI * hd * hd * hd);
+    }
+    double r = c->hstar / h;
+    return c->kappa * (ipow(r, c->n) - ipow(r, c->m));
+}
+
+/* Pi'(h) and Pi''(h) of the NLC and polymer pressures, by the chain and quotient rules on the definitions above:
+ *   NLC: with D = h^2 + beta^2, M = m/h = g h/D, x = (h - 2b)/w, t = tanh x:
+ *        g' = (1 - t^2)/(2w),  g'' = -t (1 - t^2)/w^2,
+ *        M' = g' h/D + g (beta^2 - h^2)/D^2,
+ *        M'' = g'' h/D + 2 g' (beta^2 - h^2)/D^2 + g (2h^3 - 6 h beta^2)/D^3,
+ *        Pi' = K[-3 b^3/h^4 + 2 b^2/h^3] + N M M',   Pi'' = K[12 b^3/h^5 - 6 b^2/h^4] + N (M'^2 + M M'');
+ *   polymer: Pi' = -72 C/h^10 + A1/(2 pi h^4) - (A1 - A2)/(2 pi (h+d)^4),
+ *            Pi'' = 720 C/h^11 - 2 A1/(pi h^5) + 2 (A1 - A2)/(pi (h+d)^5). */
+static void pressure_derivatives(const tfo_ctx *c, double h, double *P1, double *P2)
+{
+    if (c->model == 2) {
+        double b = c->pb, w = c->pw, be2 = c->pbeta * c->pbeta;
+        double t = tanh((h - 2.0 * b) / w);
+        double g = 0.5 * (1.0 + t), g1 = (1.0 - t * t) / (2.0 * w), g2 = -t * (1.0 - t * t) / (w * w);
+        double D = h * h + be2;
+        double M = g * h / D;
+        double M1 = g1 * h / D + g * (be2 - h * h) / (D * D);
+        double M2 = g2 * h / D + 2.0 * g1 * (be2 - h * h) / (D * D) + g * (2.0 * h * h * h - 6.0 * h * be2) / (D * D * D);
+        double r = 1.0 / h;
+        *P1 = c->pk * (-3.0 * b * b * b * ipow(r, 4) + 2.0 * b * b * ipow(r, 3)) + c->pn * M * M1;
+        *P2 = c->pk * (12.0 * b * b * b * ipow(r, 5) - 6.0 * b * b * ipow(r, 4)) + c->pn * (M1 * M1 + M * M2);
+        return;
+    }
+    double r = 1.0 / h, rd = 1.0 / (h + c->qd), da = c->qa1 - c->qa2;
+    *P1 = -72.0 * c->qc * ipow(r, 10) + c->qa1 * ipow(r, 4) / (2.0 * TFO_PI) - da * ipow(rd, 4) / (2.0 * TFO_PI);
+    *P2 = 720.0 * c->qc * ipow(r, 11) - 2.0 * c->qa1 * ipow(r, 5) / TFO_PI + 2.0 * da * ipow(rd, 5) / TFO_PI;
+}
+
 static void model_functions(const tfo_ctx *c, double h, double *f0, double *f1, double *g0, double *g1)
 {
     if (c->model == 1) { *f0 = c->c0; *f1 = c->c1; *g0 = 0.0; *g1 = 0.0; return; }
+    if (c->model >= 2) {
+        /* (1.7), with caller-supplied prefactors (reading R19): f0 = cap0 h^3, f1 = cap1 h^3 Pi' */
+        double P1, P2;
+        pressure_derivatives(c, h, &P1, &P2);
+        double h2 = h * h, h3 = h2 * h;
+        *f0 = c->cap0 * h3; *g0 = c->cap0 * 3.0 * h2;
+        *f1 = c->cap1 * h3 * P1; *g1 = c->cap1 * (3.0 * h2 * P1 + h3 * P2);
+        return;
+    }
     double r = 1.0 / h;
     double hn = ipow(c->hstar, c->n), hm = ipow(c->hstar, c->m);
     double P1 = c->kappa * (c->m * hm * ipow(r, c->m + 1) - c->n * hn * ipow(r, c->n + 1));
@@ -262,6 +327,33 @@ int tfo_create(tfo_ctx **out, int nx, int ny, double dx, double dy,
 int tfo_set_model_linear(tfo_ctx *c, double c0, double c1)
 { if (!c) return TFO_ERR_INVALID_ARG; c->model = 1; c->c0 = c0; c->c1 = c1; return TFO_OK; }
 
+/* Disjoining pressure of SURVEY.md 8(f) row f-1.  kind 2: NLC, p = {cap0, cap1, K, b, N, beta, w};
+ * kind 3: polymer, p = {cap0, cap1, C, A_SiOx, A_Si, d}. */
+int tfo_set_pressure(tfo_ctx *c, int kind, const double *p, int np)
+{
+    if (!c || !p) return TFO_ERR_INVALID_ARG;
+    if (kind == 2 && np == 7) {
+        c->cap0 = p[0]; c->cap1 = p[1]; c->pk = p[2]; c->pb = p[3]; c->pn = p[4]; c->pbeta = p[5]; c->pw = p[6];
+        if (!(c->pb > 0) || !(c->pw > 0)) return TFO_ERR_INVALID_ARG;
+    } else if (kind == 3 && np == 6) {
+        c->cap0 = p[0]; c->cap1 = p[1]; c->qc = p[2]; c->qa1 = p[3]; c->qa2 = p[4]; c->qd = p[5];
+        if (!(c->qd > 0)) return TFO_ERR_INVALID_ARG;
+    } else return TFO_ERR_INVALID_ARG;
+    if (!(c->cap0 > 0) || !(c->cap1 > 0)) return TFO_ERR_INVALID_ARG;
+    c->model = kind;
+    return TFO_OK;
+}
+
+/* pins only: Pi(h) as defined by the paper, and the four cell functions, at n points */
+int tfo_pressure(tfo_ctx *c, int n, const double *h, double *Pi)
+{ if (!c || !h || !Pi) return TFO_ERR_INVALID_ARG; for (int k = 0; k < n; ++k) Pi[k] = pressure(c, h[k]); return TFO_OK; }
+int tfo_cell_functions(tfo_ctx *c, int n, const double *h, double *f0, double *f1, double *g0, double *g1)
+{
+    if (!c || !h || !f0 || !f1 || !g0 || !g1) return TFO_ERR_INVALID_ARG;
+    for (int k = 0; k < n; ++k) model_functions(c, h[k], f0 + k, f1 + k, g0 + k, g1 + k);
+    return TFO_OK;
+}
+
 int tfo_set_newton(tfo_ctx *c, double tol, int max_iter, int fixed_iters)
 {
     if (!c || !(tol >= 1e-14) || max_iter < 1 || fixed_iters < 0) return TFO_ERR_INVALID_ARG; /* PAPER.md:338 */
@@ -274,7 +366,7 @@ int tfo_set_state(tfo_ctx *c, const double *h)
     if (!c || !h) return TFO_ERR_INVALID_ARG;
     size_t N = (size_t)c->nx * c->ny;
     for (size_t p = 0; p < N; ++p)
-        if (!isfinite(h[p]) || (c->model == 0 && !(h[p] > 0))) return TFO_ERR_INVALID_ARG;
+        if (!isfinite(h[p]) || (c->model != 1 && !(h[p] > 0))) return TFO_ERR_INVALID_ARG;
     memcpy(c->u, h, N * sizeof(double));
     c->have_state = 1;
     return TFO_OK;
@@ -320,7 +412,7 @@ int tfo_step(tfo_ctx *c, double dt, int *newton_iters, double *residual)
             double r = fabs(c->v[p] / c->uk[p]);           /* (2.22), denominator u_(k) */
             if (!(r <= res)) res = r;                      /* NaN propagates into res   */
             c->uk[p] += c->v[p];                           /* (2.21) */
-            if (!isfinite(c->uk[p]) || (c->model == 0 && !(c->uk[p] > 0))) bad = 1;
+            if (!isfinite(c->uk[p]) || (c->model != 1 && !(c->uk[p] > 0))) bad = 1;
         }
         ++k;
         if (c->fixed_iters > 0) { if (k == kmax) status = TFO_OK; continue; }

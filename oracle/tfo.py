@@ -39,6 +39,9 @@ def lib(omp=False):
                                  ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
                                  ctypes.c_int]
         L.tfo_set_model_linear.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_double]
+        L.tfo_set_pressure.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, ctypes.c_int]
+        L.tfo_pressure.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, _dp]
+        L.tfo_cell_functions.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, _dp, _dp, _dp, _dp]
         L.tfo_set_newton.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_int, ctypes.c_int]
         L.tfo_set_state.argtypes = [ctypes.c_void_p, _dp]
         L.tfo_get_state.argtypes = [ctypes.c_void_p, _dp]
@@ -87,6 +90,24 @@ class ThinFilmOracle:
 
     def set_model_linear(self, c0, c1):
         _chk(self.L.tfo_set_model_linear(self._h, c0, c1), "tfo_set_model_linear")
+
+    def set_pressure(self, kind, params):
+        """kind 2: NLC (1.8)-(1.9), params (cap0, cap1, K, b, N, beta, w); kind 3: polymer (1.12), params
+        (cap0, cap1, C, A_SiOx, A_Si, d).  f0 = cap0 h^3, f1 = cap1 h^3 Pi'(h)."""
+        p = np.ascontiguousarray(params, dtype=np.float64)
+        _chk(self.L.tfo_set_pressure(self._h, int(kind), _p(p), int(p.size)), "tfo_set_pressure")
+
+    def pressure(self, h):
+        h = np.ascontiguousarray(h, dtype=np.float64).ravel()
+        out = np.empty_like(h)
+        _chk(self.L.tfo_pressure(self._h, h.size, _p(h), _p(out)), "tfo_pressure")
+        return out
+
+    def cell_functions(self, h):
+        h = np.ascontiguousarray(h, dtype=np.float64).ravel()
+        outs = [np.empty_like(h) for _ in range(4)]
+        _chk(self.L.tfo_cell_functions(self._h, h.size, _p(h), *[_p(o) for o in outs]), "tfo_cell_functions")
+        return outs   # f0, f1, f0', f1'
 
     def set_newton(self, tol=1e-10, max_iter=10, fixed_iters=0):
         _chk(self.L.tfo_set_newton(self._h, tol, max_iter, fixed_iters), "tfo_set_newton")
