@@ -38,6 +38,9 @@ def parse():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index; 3 is the headline, 4 the isolated solver (side measurement)")
     ap.add_argument("--fixed-iters", type=int, default=0, help="fixed Newton count per step (0: converge to tol)")
+    ap.add_argument("--pressure", default="power", choices=["power", "nlc"],
+                    help="power: BASELINE.json's Pi (headline); nlc: the paper's NLC pressure (1.8)-(1.9) with (1.11), on the "
+                         "same grid with the paper's spacing 0.05 and a 0.2 film (side measurement, row f-1)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -190,9 +193,17 @@ def run_b200(args, cfg):
 
     nx, ny, dt = cfg["nx"], cfg["ny"], cfg["dt"]
     npts = nx * ny
-    h_host = torch.from_numpy(inputs.initial_condition(cfg)).pin_memory()     # every rank: its own replica
+    if args.pressure == "nlc":
+        # the paper's own model and scales (PAPER.md:99-105 (1.11), 453: spacing 0.05), film 0.2 (1 + 0.01 U[-1,1])
+        cfg = dict(cfg, dx=0.05, dy=0.05, name=cfg["name"] + "_nlc")
+        dt = 1e-3
+        h_host = torch.from_numpy(0.2 * inputs.noise_ic(nx, ny, cfg["seed"])).pin_memory()
+    else:
+        h_host = torch.from_numpy(inputs.initial_condition(cfg)).pin_memory()     # every rank: its own replica
     h_dev = h_host.cuda(non_blocking=True)
     ctx = tf.ThinFilm(nx, ny, cfg["dx"], cfg["dy"], cfg["kappa"], cfg["hstar"], cfg["n"], cfg["m"])
+    if args.pressure == "nlc":
+        ctx.set_pressure(tf.PI_NLC, (0.0857, 1.0 / 0.0857, 36.0, 0.01, 1.67, 1.0, 0.05))
     ctx.set_newton(cfg["tol"], cfg["max_iter"], args.fixed_iters)
 
     def timed_run(e2e):
@@ -265,7 +276,7 @@ def run_b200(args, cfg):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg["name"], "grid": [nx, ny], "dx": cfg["dx"], "dt": dt, "tol": cfg["tol"],
-                   "max_iter": cfg["max_iter"], "fixed_iters": args.fixed_iters,
+                   "max_iter": cfg["max_iter"], "fixed_iters": args.fixed_iters, "pressure": args.pressure,
                    "ic": "1 + 0.01 U[-1,1] seeded noise", "parallelism": f"replicas x{world} (no exchange step)",
                    "l2": "working set 7 fields x 512 MiB >> 126 MB L2: every launch streams from HBM, no flush needed"},
         "newton_iters_total": iters, "newton_iters_per_step": iters / args.steps,
@@ -278,7 +289,7 @@ def run_b200(args, cfg):
         "roofline": roofline, "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
         "mass_rel_drift": mass_drift,
     }
-    if world == 1 and not args.no_cpu_baseline:
+    if world == 1 and not args.no_cpu_baseline and args.pressure == "power":
         n = 2048 if min(nx, ny) >= 2048 else min(nx, ny)
         r = oracle_sample_run(cfg, n, 1, 0, args.fixed_iters)
         line["cpu_baseline"] = {

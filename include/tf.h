@@ -63,6 +63,20 @@ tf_status tf_create_with_workspace(tf_ctx** out, int nx, int ny, double dx, doub
                                    void* dev_ws, size_t bytes, void* cuda_stream);
 void tf_destroy(tf_ctx* ctx);
 
+/* Disjoining pressure behind the same sweep.  With (1.7), in the form
+ * f0 = cap0 h^3, f1 = cap1 h^3 Pi'(h) (the printed placement of the capillary number is cap0 = C, cap1 = 1/C;
+ * both prefactors are the caller's):
+ *   TF_PI_POWER    Pi = kappa[(hstar/h)^n - (hstar/h)^m] of tf_create, cap0 = cap1 = 1 (default; params ignored)
+ *   TF_PI_NLC      (1.8)-(1.9): Pi = K[(b/h)^3 - (b/h)^2] + (N/2)[m(h)/h]^2,
+ *                  m = g h^2/(h^2 + beta^2), g = (1 + tanh((h - 2b)/w))/2;
+ *                  params[7] = {cap0, cap1, K, b, N, beta, w}   (host pointer; (1.11) lists the paper's values)
+ *   TF_PI_POLYMER  (1.12): Pi = -d psi/dh, psi = C/h^8 - A_SiOx/(12 pi h^2) + (A_SiOx - A_Si)/(12 pi (h+d)^2);
+ *                  params[6] = {cap0, cap1, C, A_SiOx, A_Si, d}
+ * Takes effect from the next tf_step; the state is kept.  TF_ERR_INVALID_ARG for a wrong count, non-finite values or
+ * non-positive cap0, cap1, b, w, d; TF_ERR_UNSUPPORTED for another kind. */
+typedef enum { TF_PI_POWER = 0, TF_PI_NLC = 2, TF_PI_POLYMER = 3 } tf_pressure;
+tf_status tf_set_pressure(tf_ctx* ctx, tf_pressure kind, const double* params, int nparams);
+
 /* Newton controls, (2.22) and Notes 1-2.  Defaults: tol = 1e-10,
  * max_iter = 10, fixed_iters = 0 (off).  tol >= 1e-14;
  * 1 <= max_iter <= 4096; 0 <= fixed_iters <= 4096.  fixed_iters = K > 0: exactly K

@@ -34,6 +34,7 @@ constexpr int NFIELDS = 7;   // u, uk, bn, w, alpha, beta, z
 struct tf_ctx {
     Params P;
     double kappa, hstar;
+    int model;                                 // tf_pressure: TF_PI_POWER (create-time kappa, h*, n, m), TF_PI_NLC, TF_PI_POLYMER
     double tol;
     int max_iter, fixed_iters;
     bool have_state, owns_ws;
@@ -269,6 +270,8 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
 
 cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
 {
+    if (c->model == TF_PI_NLC) return launch_iteration<MODEL_NLC, 0>(c, s, k, slot);
+    if (c->model == TF_PI_POLYMER) return launch_iteration<MODEL_POLYMER, 0>(c, s, k, slot);
     if (c->P.n == 3 && c->P.m == 2) return launch_iteration<3, 2>(c, s, k, slot);
     return launch_iteration<0, 0>(c, s, k, slot);
 }
@@ -315,6 +318,8 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
     for (int k = 0; k < n; ++k) hn *= hstar;
     P.cm = kappa * m * hm; P.cn = kappa * n * hn;
     c->kappa = kappa; c->hstar = hstar;
+    c->model = TF_PI_POWER;
+    for (double& v : P.mp) v = 0.0;
     c->tol = 1e-10; c->max_iter = 10; c->fixed_iters = 0;
     c->have_state = false; c->owns_ws = own;
     c->stream = (cudaStream_t)stream;
@@ -433,6 +438,38 @@ tf_status tf_set_newton(tf_ctx* c, double tol, int max_iter, int fixed_iters)
     if (max_iter < 1 || max_iter > MAX_ITERS || fixed_iters < 0 || fixed_iters > MAX_ITERS)
         return fail(c, TF_ERR_INVALID_ARG, "max_iter in [1,4096], fixed_iters in [0,4096]");
     c->tol = tol; c->max_iter = max_iter; c->fixed_iters = fixed_iters;
+    return TF_OK;
+}
+
+tf_status tf_set_pressure(tf_ctx* c, tf_pressure kind, const double* p, int np)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    double* mp = c->P.mp;
+    const double PI = 3.14159265358979323846;
+    auto finite_pos = [](double v) { return v > 0 && std::isfinite(v); };
+    if (kind == TF_PI_POWER) {
+        c->model = TF_PI_POWER;
+        return TF_OK;
+    }
+    if (!p) return fail(c, TF_ERR_INVALID_ARG, "params is NULL");
+    for (int k = 0; k < np; ++k)
+        if (!std::isfinite(p[k])) return fail(c, TF_ERR_INVALID_ARG, "non-finite parameter");
+    if (kind == TF_PI_NLC) {
+        if (np != 7) return fail(c, TF_ERR_INVALID_ARG, "NLC takes 7 parameters: cap0, cap1, K, b, N, beta, w");
+        if (!finite_pos(p[0]) || !finite_pos(p[1]) || !finite_pos(p[3]) || !finite_pos(p[6]))
+            return fail(c, TF_ERR_INVALID_ARG, "cap0, cap1, b, w must be positive");
+        const double K = p[2], b = p[3];
+        mp[0] = p[0]; mp[1] = p[1]; mp[2] = K * b * b * b; mp[3] = K * b * b; mp[4] = p[4]; mp[5] = p[5] * p[5];
+        mp[6] = 1.0 / p[6]; mp[7] = 2.0 * b;
+    } else if (kind == TF_PI_POLYMER) {
+        if (np != 6) return fail(c, TF_ERR_INVALID_ARG, "polymer takes 6 parameters: cap0, cap1, C, A_SiOx, A_Si, d");
+        if (!finite_pos(p[0]) || !finite_pos(p[1]) || !finite_pos(p[5]))
+            return fail(c, TF_ERR_INVALID_ARG, "cap0, cap1, d must be positive");
+        mp[0] = p[0]; mp[1] = p[1]; mp[2] = p[2]; mp[3] = p[3] / (2.0 * PI); mp[4] = (p[3] - p[4]) / (2.0 * PI); mp[5] = p[5];
+    } else {
+        return fail(c, TF_ERR_UNSUPPORTED, "unknown pressure kind");
+    }
+    c->model = kind;
     return TF_OK;
 }
 

@@ -20,7 +20,11 @@ struct Params {
     double rdx2, rdy2;      // 1/dx^2, 1/dy^2
     int n, m;               // Pi exponents, n > m >= 1
     double cm, cn;          // kappa*m*hstar^m, kappa*n*hstar^n
+    double mp[10];          // constants of the NLC / polymer pressures (tf_set_pressure), see cell_functions
 };
+
+// model selectors carried in the kernels' <N, M> template pair (N > 0: power law with exponents N, M; 0: runtime n, m)
+constexpr int MODEL_NLC = -2, MODEL_POLYMER = -3;
 
 // per-direction constants for one dt:  ca = s/(2 d^4),  cb = s/(2 d^2)
 struct Dir { double ca, cb; };
@@ -55,12 +59,46 @@ __device__ __forceinline__ double ipow_rh(double r, double h, int k)
 
 // Cell-centre functions.  With r = 1/h:  h^3 Pi'(h) = cm r^(m-2) - cn r^(n-2)  and its derivative
 // (2-m) cm r^(m-1) + (n-2) cn r^(n-1)  (the same polynomials as 3h^2 Pi' + h^3 Pi'', summed exactly).
+// NLC (1.8)-(1.9): Pi = K[(b/h)^3 - (b/h)^2] + (N/2) M^2, M = m(h)/h = g h/(h^2 + beta^2),
+//   g = (1 + tanh((h - 2b)/w))/2.  mp = {cap0, cap1, K b^3, K b^2, N, beta^2, 1/w, 2b}.
+// polymer (1.12): Pi = 8C/h^9 - A1/(6 pi h^3) + (A1 - A2)/(6 pi (h+d)^3).
+//   mp = {cap0, cap1, C, A1/(2 pi), (A1 - A2)/(2 pi), d}.
+// Both: f0 = cap0 h^3, f1 = cap1 h^3 Pi'(h) (1.7); the derivatives Pi', Pi'' are written out by hand below.
 template <int N, int M>
 __device__ __forceinline__ Cell cell_functions(double h, const Params& P)
 {
     Cell c;
     const double r = rcp(h);
     const double h2 = h * h;
+    if (N == MODEL_NLC || N == MODEL_POLYMER) {
+        double P1, P2;
+        if (N == MODEL_NLC) {
+            const double Kb3 = P.mp[2], Kb2 = P.mp[3], Nn = P.mp[4], be2 = P.mp[5], iw = P.mp[6];
+            const double t = tanh((h - P.mp[7]) * iw);
+            const double s2 = fma(-t, t, 1.0);
+            const double g = fma(0.5, t, 0.5), g1 = 0.5 * s2 * iw, g2 = -t * s2 * iw * iw;
+            const double rD = rcp(h2 + be2), bh = be2 - h2;
+            const double Mm = g * h * rD;
+            const double M1 = fma(g1, h, g * bh * rD) * rD;
+            const double M2 = fma(g2, h, fma(2.0 * g1, bh, g * h * fma(2.0, h2, -6.0 * be2) * rD) * rD) * rD;
+            const double r2 = r * r, r3 = r2 * r;
+            P1 = fma(-3.0 * Kb3, r, 2.0 * Kb2) * r3 + Nn * Mm * M1;
+            P2 = fma(12.0 * Kb3, r, -6.0 * Kb2) * r3 * r + Nn * fma(M1, M1, Mm * M2);
+        } else {
+            const double Cc = P.mp[2], a1 = P.mp[3], da = P.mp[4];
+            const double rd = rcp(h + P.mp[5]);
+            const double r2 = r * r, r4 = r2 * r2, r5 = r4 * r, r10 = r5 * r5;
+            const double rd2 = rd * rd, rd4 = rd2 * rd2;
+            P1 = fma(-72.0 * Cc, r10, fma(a1, r4, -da * rd4));
+            P2 = fma(720.0 * Cc, r10 * r, fma(-4.0 * a1, r5, 4.0 * da * rd4 * rd));
+        }
+        const double h3 = h2 * h;
+        c.f0 = P.mp[0] * h3;
+        c.g0 = 3.0 * P.mp[0] * h2;
+        c.f1 = P.mp[1] * h3 * P1;
+        c.g1 = P.mp[1] * fma(3.0 * h2, P1, h3 * P2);
+        return c;
+    }
     c.f0 = h2 * h;
     c.g0 = 3.0 * h2;
     if (N == 3 && M == 2) {

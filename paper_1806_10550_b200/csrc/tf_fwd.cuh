@@ -384,13 +384,15 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
                 const double hm1 = __shfl_up_sync(FULL, h0, 1);
                 const double hp1 = __shfl_down_sync(FULL, h0, 1), hp2 = __shfl_down_sync(FULL, h0, 2);
                 const Cell c0 = cell_functions<N, M>(h0, P);
-#if XW_RECOMPUTE_C1
-                const Cell c1 = cell_functions<N, M>(hp1, P);   // cheaper than 8 shuffles: the LSU pipe, not fp64, bounds this kernel
-#else
                 Cell c1;
-                c1.f0 = __shfl_down_sync(FULL, c0.f0, 1); c1.f1 = __shfl_down_sync(FULL, c0.f1, 1);
-                c1.g0 = __shfl_down_sync(FULL, c0.g0, 1); c1.g1 = __shfl_down_sync(FULL, c0.g1, 1);
-#endif
+                if (XW_RECOMPUTE_C1 && N >= 0) {
+                    // power-law Pi: recomputing the neighbour's cell (10 fp64) is cheaper than 8 shuffles -- the LSU
+                    // pipe, not fp64, bounds this kernel; the NLC / polymer cells (tanh, high powers) are shuffled
+                    c1 = cell_functions<N, M>(hp1, P);
+                } else {
+                    c1.f0 = __shfl_down_sync(FULL, c0.f0, 1); c1.f1 = __shfl_down_sync(FULL, c0.f1, 1);
+                    c1.g0 = __shfl_down_sync(FULL, c0.g0, 1); c1.g1 = __shfl_down_sync(FULL, c0.g1, 1);
+                }
                 Face fp = face_partials(hm1, hp2, hp1 - h0, c0.f0 + c1.f0, c0.f1 + c1.f1, c0, c1, DX);
                 if (!INTERIOR) {
                     if (i == 0) fp.p1 -= fp.A;

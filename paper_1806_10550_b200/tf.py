@@ -14,6 +14,7 @@ from . import build as _build
 OK, NOT_CONVERGED = 0, 1
 ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_ALLOC, ERR_STATE = -1, -2, -3, -4, -5
 BC_NOFLUX = 0
+PI_POWER, PI_NLC, PI_POLYMER = 0, 2, 3
 
 _dp = ctypes.POINTER(ctypes.c_double)
 _vp = ctypes.c_void_p
@@ -29,6 +30,7 @@ SYMBOLS = {
                                                 ctypes.c_int, ctypes.c_int, _vp, ctypes.c_size_t, _vp]),
     "tf_destroy": (None, [_vp]),
     "tf_set_newton": (ctypes.c_int, [_vp, ctypes.c_double, ctypes.c_int, ctypes.c_int]),
+    "tf_set_pressure": (ctypes.c_int, [_vp, ctypes.c_int, _dp, ctypes.c_int]),
     "tf_set_state": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
     "tf_get_state": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
     "tf_step": (ctypes.c_int, [_vp, ctypes.c_double, ctypes.POINTER(ctypes.c_int), _dp]),
@@ -112,6 +114,13 @@ class ThinFilm:
         st = lib().tf_set_newton(self._h, tol, max_iter, fixed_iters)
         if st != OK:
             _err(self._h, st, "tf_set_newton")
+
+    def set_pressure(self, kind, params=()):
+        """tf_set_pressure: PI_POWER (), PI_NLC (cap0, cap1, K, b, N, beta, w), PI_POLYMER (cap0, cap1, C, A_SiOx, A_Si, d)."""
+        arr = (ctypes.c_double * max(len(params), 1))(*[float(v) for v in params])
+        st = lib().tf_set_pressure(self._h, int(kind), arr, len(params))
+        if st != OK:
+            _err(self._h, st, "tf_set_pressure")
 
     def set_state(self, h):
         """h: torch CUDA float64 tensor [ny][nx] (device copy) or numpy / CPU tensor (host copy)."""
