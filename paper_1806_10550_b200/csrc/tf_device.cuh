@@ -74,9 +74,13 @@ __device__ __forceinline__ Cell cell_functions(double h, const Params& P)
         double P1, P2;
         if (N == MODEL_NLC) {
             const double Kb3 = P.mp[2], Kb2 = P.mp[3], Nn = P.mp[4], be2 = P.mp[5], iw = P.mp[6];
-            const double t = tanh((h - P.mp[7]) * iw);
-            const double s2 = fma(-t, t, 1.0);
-            const double g = fma(0.5, t, 0.5), g1 = 0.5 * s2 * iw, g2 = -t * s2 * iw * iw;
+            // g = (1 + tanh x)/2 = 1/(1 + e^(-2x)); 1 - tanh^2 = 4 g (1 - g); tanh = 2g - 1 (one exp and one
+            // reciprocal instead of the library tanh; x clamped so that e^(-2x) stays finite)
+            const double x = fmin(fmax((h - P.mp[7]) * iw, -300.0), 300.0);
+            const double g = rcp(1.0 + exp(-2.0 * x));
+            const double t = fma(2.0, g, -1.0);
+            const double s2 = 4.0 * g * (1.0 - g);
+            const double g1 = 0.5 * s2 * iw, g2 = -t * s2 * iw * iw;
             const double rD = rcp(h2 + be2), bh = be2 - h2;
             const double Mm = g * h * rD;
             const double M1 = fma(g1, h, g * bh * rD) * rD;
