@@ -1,34 +1,24 @@
 // tf_fwd.cuh -- warp-specialised forward kernels (assembly + LU forward elimination), S1-S6 forward halves.
 //
 // Why: a sweep has only nx (ny) independent lines = 256 warps at 8192^2 for 592 SM sub-partitions, and the
-// assembly of one matrix row costs ~100 fp64 instructions against ~20 for the elimination recurrence.  If
-// the thread that carries the recurrence also assembles, under half of the fp64 pipes are ever busy and
-// the serial chain is 5x longer than it must be.  So a CTA owns one strip of lines and splits the work:
-//   * NP producer warps assemble rows (bands A,c,q,a and right-hand side R) for disjoint row chunks of a
-//     tile -- embarrassingly parallel -- and hand them over through a shared-memory ring;
-//   * 1 consumer warp runs the pentadiagonal recurrence and streams alpha,beta,z out.
-// Hand-over is by mbarriers (full/empty per stage), no __syncthreads in the steady state.
+// assembly of one matrix row costs ~55 fp64 instructions against 17 for the elimination recurrence, which is
+// a serial chain (52 cycles per row).  If the thread that carries the recurrence also assembles, most fp64
+// pipes idle.  So the work of a strip of lines is split:
+//   * NP producer warps assemble rows (bands A,c,q,a and right-hand side R) for disjoint chunks --
+//     embarrassingly parallel -- and hand them over through a shared-memory ring;
+//   * 1 consumer warp runs the pentadiagonal recurrence and streams alpha,beta,z out;
+//   * every line is eliminated from both ends by two such teams (two-sided / twisted factorisation), and one
+//     CTA per SM hosts four teams, one per SM sub-partition.
+// Hand-over is by mbarriers (full/empty per slot), no __syncthreads in the steady state.
+// has the measurements behind each of these choices (register reallocation between the consumer and producer
+// warpgroups with setmaxnreg was also measured: no gain).
 #pragma once
 #include "tf_device.cuh"
 #include "tf_tma.cuh"
 #include <type_traits>
 
-#ifndef TF_DBG_MODE
-#define TF_DBG_MODE 0        // experiments only (_work/): 1 = producers skip assembly, 2 = consumer skips the recurrence
-#endif
-
 namespace tf {
 
-#ifndef YW_CUNROLL
-#define YW_CUNROLL 4
-#endif
-#ifndef YW_PFD
-#define YW_PFD 0             // L2 prefetch distance of the y producers in rounds of chunks; 0 = off (measured: no gain)
-#endif
-#ifndef YW_MINB
-#define YW_MINB 4            // CTAs per SM the y forward kernel is compiled for (register cap)
-#endif
-constexpr int YW_CU = YW_CUNROLL;   // unroll of the consumer's row loop
 constexpr int YW_VALID = 28;     // columns per strip (lanes 2..29; lanes 0,1,30,31 are x-halo)
 
 // rolling state of a thread marching down a column
@@ -100,7 +90,7 @@ __device__ __forceinline__ void y_advance(YState& S, int j, double hp2, const Pa
 // CTA = warp 0 (consumer: the recurrence) + NP producer warps (assembly).  The hand-over ring has NCH
 // slots of ONE CHUNK (RP rows of one producer) each: chunk c is assembled by producer c % NP into slot
 // c % NCH, so RP can be large (the two warm-up rows of a chunk are amortised over RP rows) while the ring
-// stays small (4 CTAs per SM).  Inputs are pulled into L2 a few chunks ahead by prefetch hints.
+// stays small.  Inputs arrive by TMA, one box per chunk, issued a chunk ahead (see the producer loop).
 // ---------------------------------------------------------------------------------------------
 template <int N, int M, bool FIRST, int NP, int RP, int NCH, int NSUB>
 __global__ void __launch_bounds__(32 * NSUB * (NP + 1), 1)
@@ -213,8 +203,7 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
             S.hm1 = 0.0; S.h0 = hq[0]; S.hp1 = hq[1]; S.hR0 = 0.0;
             S.c0 = {0, 0, 0, 0}; S.L0 = 0.0; S.fm = {0, 0, 0}; S.phim = 0.0;
             double o6[6], sD;
-            if (TF_DBG_MODE == 1) {
-            } else if (interior) {
+            if (interior) {
                 y_advance<N, M, 0, true>(S, jlo - 2, hq[2], P, DX, DY, xface, 0.0, o6, sD);
                 y_advance<N, M, 1, true>(S, jlo - 1, hq[3], P, DX, DY, xface, 0.0, o6, sD);
                 double* bo = bn + (size_t)jlo * nx + i;
@@ -267,9 +256,7 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
             const double* stc = st + offc;
             const double* sta = st + offa;
             const int nrow = min(RP, nrows - c * RP);
-            if (TF_DBG_MODE == 2) {
-                o += step * nrow;
-            } else if (nrow == RP && c > 0) {
+            if (nrow == RP && c > 0) {
 #pragma unroll
                 for (int r = 0; r < RP; ++r) {
                     const double A = st[r * 32], cc = stc[r * 32], q = st[2 * SV + r * 32], a = sta[r * 32];
