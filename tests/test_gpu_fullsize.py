@@ -215,3 +215,32 @@ def test_config2_4096_adaptive_run(tf, tfo):
     assert abs(g.mass() - m0) <= 1e-13 * m0
     assert u.min() > h.min() and u.max() <= 0.12 + 1e-9                     # the depressions heal
     g.close()
+
+
+# ------------------------------------------------------------------ large non-square grids (ragged strips, tiles, splits)
+@pytest.mark.parametrize("nx,ny", [(12010, 3002), (2050, 9998), (16384, 4100)])
+def test_large_nonsquare_grids_sampled(tf, tfo, nx, ny):
+    """Grid sides that are multiples of neither 28 (strips), 16 (tiles) nor 32 (blocks); more strips than SMs in one
+    direction and fewer in the other (both CTA layouts of the forward kernels); dx != dy."""
+    cfg = inputs.config(3)
+    dx, dy = cfg["dx"], 1.07 * cfg["dx"]
+    h = inputs.noise_ic(nx, ny, seed=nx + ny)
+    g = tf.ThinFilm(nx, ny, dx, dy)
+    g.set_newton(1e-10, 64, 3)
+    g.set_state(h)
+    m0 = g.mass()
+    assert g.step(cfg["dt"])[:2] == (0, 3)
+    u = g.get_state()
+    assert abs(g.mass() - m0) <= 1e-13 * m0
+    g.close()
+    midx, midy = (nx // 2) // 16 * 16, (ny // 2) // 16 * 16
+    o = tfo.ThinFilmOracle(W, W, dx, dy)
+    o.set_newton(1e-10, 64, 3)
+    for (j0, i0) in ((0, 0), (ny - W, nx - W), (midy - W // 2, midx - W // 2), (0, nx - W), (midy - W // 2, 0)):
+        o.set_state(np.ascontiguousarray(h[j0:j0 + W, i0:i0 + W]))
+        assert o.step(cfg["dt"])[:2] == (0, 3)
+        uo = o.get_state()
+        ja, jb = (0 if j0 == 0 else MARGIN), (W if j0 + W == ny else W - MARGIN)
+        ia, ib = (0 if i0 == 0 else MARGIN), (W if i0 + W == nx else W - MARGIN)
+        d = np.max(np.abs(u[j0 + ja:j0 + jb, i0 + ia:i0 + ib] - uo[ja:jb, ia:ib])) / np.max(np.abs(uo))
+        assert d <= 1e-11, (nx, ny, j0, i0, d)
