@@ -120,6 +120,14 @@ bool make_map2d(CUtensorMap* m, const double* base, int inner, int outer, int bo
 // ---- ring-kernel launchers (dynamic shared memory above 48 KB needs the opt-in attribute once per kernel)
 constexpr int YB_NST = 8, YB_RS = 16;     // 8 stages x 16 rows x 3 arrays x 256 B = 96 KiB per warp
 
+// "has this kernel's shared-memory opt-in been done on the current device" (function attributes are per device)
+struct DevOnce {
+    unsigned long long mask = 0;
+    static int dev() { int d = 0; cudaGetDevice(&d); return d & 63; }
+    bool done() const { return (mask >> dev()) & 1ull; }
+    void mark() { mask |= 1ull << dev(); }
+};
+
 template <typename K>
 cudaError_t opt_in_smem(K kernel, size_t bytes)
 {
@@ -145,11 +153,11 @@ cudaError_t launch_ybwd2_n(const CUtensorMap* m, dim3 g, int nx, int ny, int mid
                            const double* zz, double* w, cudaStream_t st)
 {
     constexpr size_t SM = (size_t)NST * 3 * YT_RS * 32 * 8 + 8 * NST + 1024;
-    static bool ready = false;
-    if (!ready) {
+    static DevOnce ready;
+    if (!ready.done()) {
         cudaError_t e = opt_in_smem(ybwd2_tma_kernel<NST, YT_RS>, SM);
         if (e != cudaSuccess) return e;
-        ready = true;
+        ready.mark();
     }
     ybwd2_tma_kernel<NST, YT_RS><<<g, 32, SM, st>>>(m[0], m[1], m[2], nx, ny, mid, al, be, zz, w);
     return cudaGetLastError();
@@ -160,11 +168,11 @@ cudaError_t launch_xbwd2_n(const CUtensorMap* m, const CUtensorMap& uin, const C
                            int mid, const double* alT, const double* beT, const double* zzT, double* red, cudaStream_t st)
 {
     constexpr size_t SM = (size_t)NST * 4 * 16 * 32 * 8 + 8 * NST + 1024;
-    static bool ready = false;
-    if (!ready) {
+    static DevOnce ready;
+    if (!ready.done()) {
         cudaError_t e = opt_in_smem(xbwd2_tma_kernel<NST, UPDATE>, SM);
         if (e != cudaSuccess) return e;
-        ready = true;
+        ready.mark();
     }
     xbwd2_tma_kernel<NST, UPDATE><<<g, 32, SM, st>>>(m[0], m[1], m[2], uin, uout, nx, ny, mid, alT, beT, zzT, red);
     return cudaGetLastError();
@@ -203,12 +211,12 @@ cudaError_t launch_ybwd(int nx, int ny, const double* al, const double* be, cons
                         cudaStream_t st)
 {
     constexpr size_t SM = sizeof(double) * YB_NST * 3 * YB_RS * 32;
-    static bool ready = false;
-    if (!ready) {
+    static DevOnce ready;
+    if (!ready.done()) {
         cudaError_t e = opt_in_smem(ybwd_ring_kernel<YB_NST, YB_RS, true>, SM);
         if (e == cudaSuccess) e = opt_in_smem(ybwd_ring_kernel<YB_NST, YB_RS, false>, SM);
         if (e != cudaSuccess) return e;
-        ready = true;
+        ready.mark();
     }
     const int g = (nx + 31) / 32;
     if (nx % 2 == 0) ybwd_ring_kernel<YB_NST, YB_RS, true><<<g, 32, SM, st>>>(nx, ny, al, be, zz, w);
@@ -230,11 +238,11 @@ cudaError_t launch_yfwd(tf_ctx* c, const CUtensorMap& mu, int tma, const Params&
     constexpr size_t SM = NSUB * (size_t)YW_NSTG * 5 * YW_RP * 32 * 8 + NSUB * YW_NP * (size_t)(2 * YW_RP + 4) * 32 * 8 +
                           (2 * NSUB * YW_NSTG + NSUB * YW_NP) * 8;
     auto kern = yfwd_ws_kernel<N, M, FIRST, YW_NP, YW_RP, YW_NSTG, NSUB>;
-    static bool ready = false;
-    if (!ready) {
+    static DevOnce ready;
+    if (!ready.done()) {
         cudaError_t e = opt_in_smem(kern, SM);
         if (e != cudaSuccess) return e;
-        ready = true;
+        ready.mark();
     }
     kern<<<grid, 32 * NSUB * (YW_NP + 1), SM, c->stream>>>(mu, c->mBn, tma, P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz);
     return cudaGetLastError();
@@ -245,11 +253,11 @@ cudaError_t launch_xfwd(tf_ctx* c, const Params& P, const Dir& DX, const double*
 {
     constexpr size_t SM = NSUB * ((size_t)XW_NSTG * 5 * XW_CK * XW_LD * 8 + 16 * XW_NSTG);
     auto kern = xfwd_ws_kernel<N, M, XW_NP, XW_NSTG, NSUB>;
-    static bool ready = false;
-    if (!ready) {
+    static DevOnce ready;
+    if (!ready.done()) {
         cudaError_t e = opt_in_smem(kern, SM);
         if (e != cudaSuccess) return e;
-        ready = true;
+        ready.mark();
     }
     kern<<<grid, 32 * NSUB * (XW_NP + 1), SM, c->stream>>>(P, DX, c->mid_x, src, c->w, c->al, c->be, c->zz);
     return cudaGetLastError();
@@ -636,11 +644,11 @@ tf_status tf_penta_solve(int nrow, int ncol, int dir, const double* e, const dou
         }
         if (fast) {
             constexpr size_t SM = (size_t)PC_NST * 6 * PC_RS * 32 * 8 + 8 * PC_NST + 1024;
-            static bool ready = false;
-            if (!ready) {
+            static DevOnce ready;
+            if (!ready.done()) {
                 cudaError_t ee = opt_in_smem(penta_col_fwd2_kernel<PC_NST, PC_RS>, SM);
                 if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
-                ready = true;
+                ready.mark();
             }
             penta_col_fwd2_kernel<PC_NST, PC_RS><<<dim3((ncol + 31) / 32, 2), 32, SM, st>>>(M, nrow, ncol, mid, al, be, zz);
             cudaError_t le = launch_ybwd2(mw, true, ncol, nrow, mid, al, be, zz, x, st);
@@ -665,11 +673,11 @@ tf_status tf_penta_solve(int nrow, int ncol, int dir, const double* e, const dou
         }
         if (fast) {
             constexpr size_t SMF = (size_t)PR_NST * 6 * 32 * 16 * 8 + 8 * PR_NST + 1024;
-            static bool ready = false;
-            if (!ready) {
+            static DevOnce ready;
+            if (!ready.done()) {
                 cudaError_t ee = opt_in_smem(penta_row_fwd2_kernel<PR_NST>, SMF);
                 if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
-                ready = true;
+                ready.mark();
             }
             const dim3 g((nrow + 31) / 32, 2);
             penta_row_fwd2_kernel<PR_NST><<<g, 32, SMF, st>>>(M, nrow, ncol, mid, al, be, zz);
@@ -678,11 +686,11 @@ tf_status tf_penta_solve(int nrow, int ncol, int dir, const double* e, const dou
         } else {
             const int g = (nrow + XT - 1) / XT;
             const size_t sm = sizeof(double) * PT_ARR * XT * XTP;
-            static bool attr_set = false;
-            if (!attr_set) {
+            static DevOnce attr_set;
+            if (!attr_set.done()) {
                 cudaError_t ee = cudaFuncSetAttribute(penta_row_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
                 if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
-                attr_set = true;
+                attr_set.mark();
             }
             penta_row_fwd_kernel<<<g, 32, sm, st>>>(nrow, ncol, e, c, d, a, b, rhs, al, be, zz);
             penta_row_bwd_kernel<<<g, 32, 0, st>>>(nrow, ncol, al, be, zz, x);
