@@ -41,6 +41,9 @@ def parse():
     ap.add_argument("--pressure", default="power", choices=["power", "nlc"],
                     help="power: BASELINE.json's Pi (headline); nlc: the paper's NLC pressure (1.8)-(1.9) with (1.11), on the "
                          "same grid with the paper's spacing 0.05 and a 0.2 film (side measurement, row f-1)")
+    ap.add_argument("--nsys", type=int, default=0, help="config 4 only: number of systems (0: the config's 16384)")
+    ap.add_argument("--variant", default="lu", choices=["lu", "partition"], help="config 4 only: tf_penta_solve_ex variant")
+    ap.add_argument("--nparts", type=int, default=0, help="config 4 only: chunks per system of the partition variant (0: automatic)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -317,33 +320,56 @@ def run_penta(args, cfg):
         return
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
     n = cfg["nrow"]
+    nsys = args.nsys or n
+    variant = tf.PENTA_PARTITION if args.variant == "partition" else tf.PENTA_LU
     gen = torch.Generator(device="cuda").manual_seed(cfg["seed"])
-    U = lambda lo, hi: torch.rand(n, n, dtype=torch.float64, device="cuda", generator=gen) * (hi - lo) + lo
-    e, c, a, b, y = U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1)
-    d = 1 + e.abs() + c.abs() + a.abs() + b.abs() + U(0, 1)
-    ws = torch.empty(tf.lib().tf_penta_workspace_bytes(n, n), dtype=torch.uint8, device="cuda")
-    out = torch.empty_like(e)
     peak, peak_src = measured_peak()
+    small = 7 * nsys * n * 8 < 4 * 126e6          # working set not far above L2: flush between timed solves
+    flush = torch.empty(64 * 1024 * 1024, dtype=torch.float64, device="cuda") if small else None
     res = {}
     for direction, name in ((1, "along_columns_y"), (0, "along_rows_x")):
+        nrow, ncol = (nsys, n) if direction == 0 else (n, nsys)
+        U = lambda lo, hi: torch.rand(nrow, ncol, dtype=torch.float64, device="cuda", generator=gen) * (hi - lo) + lo
+        e, c, a, b, y = U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1)
+        d = 1 + e.abs() + c.abs() + a.abs() + b.abs() + U(0, 1)
+        ws = torch.empty(tf.lib().tf_penta_workspace_bytes_ex(nrow, ncol, direction, variant, args.nparts),
+                         dtype=torch.uint8, device="cuda")
+        out = torch.empty_like(e)
+        chunks = tf.penta_partition_chunks(nrow, ncol, direction, args.nparts) if variant == tf.PENTA_PARTITION else 1
+        solve = lambda: tf.penta_solve(direction, e, c, d, a, b, y, out=out, workspace=ws, variant=variant, nparts=args.nparts)
         for _ in range(max(args.warmup, 3)):
-            tf.penta_solve(direction, e, c, d, a, b, y, out=out, workspace=ws)
-        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            solve()
         torch.cuda.synchronize()
-        ev0.record()
-        for _ in range(args.steps):
-            tf.penta_solve(direction, e, c, d, a, b, y, out=out, workspace=ws)
-        ev1.record()
-        torch.cuda.synchronize()
-        ms = ev0.elapsed_time(ev1) / args.steps
-        res[name] = {"ms": ms, "unknowns_per_s": n * n / (ms * 1e-3), "alg_gbs": 104 * n * n / (ms * 1e-3) / 1e9,
-                     "frac_of_peak": 104 * n * n / (ms * 1e-3) / 1e9 / peak}
+        if small:
+            evs = []
+            for _ in range(args.steps):
+                flush.fill_(0.0)
+                ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                ev0.record()
+                solve()
+                ev1.record()
+                evs.append((ev0, ev1))
+            torch.cuda.synchronize()
+            ms = sum(a0.elapsed_time(a1) for a0, a1 in evs) / args.steps
+        else:
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ev0.record()
+            for _ in range(args.steps):
+                solve()
+            ev1.record()
+            torch.cuda.synchronize()
+            ms = ev0.elapsed_time(ev1) / args.steps
+        bpu = 104 if chunks == 1 else 200          # partition: 2 x 48 B interface pass + 104 B chunk solves
+        res[name] = {"ms": ms, "chunks": chunks, "unknowns_per_s": nsys * n / (ms * 1e-3), "alg_bytes_per_unknown": bpu,
+                     "alg_gbs": bpu * nsys * n / (ms * 1e-3) / 1e9, "frac_of_peak": bpu * nsys * n / (ms * 1e-3) / 1e9 / peak}
+        del e, c, a, b, y, d, ws, out
     print(json.dumps({"metric": "pentadiagonal unknowns/s (fp64), isolated solve", "unit": "unknowns/s", "n_gpus": 1,
                       "value": min(r["unknowns_per_s"] for r in res.values()), "steps": args.steps, "warmup": max(args.warmup, 3),
                       "dtype": "f64", "data": "synthetic (config 4 recipe drawn on the GPU)", "higher_is_better": True,
-                      "config": {"workload": cfg["name"], "systems": n, "length": n, "alg_bytes_per_unknown": 104,
-                                 "l2": "inputs 6 x 2 GiB >> 126 MB L2"},
-                      "directions": res, "peak": peak, "peak_source": peak_src}), flush=True)
+                      "config": {"workload": cfg["name"], "systems": nsys, "length": n, "variant": args.variant,
+                                 "l2": "256 MiB flush write between timed solves" if small else "inputs 6 x 2 GiB >> 126 MB L2"},
+                      "directions": res, "peak": peak, "peak_source": peak_src,
+                      "gpu_launches": (4 if variant == tf.PENTA_PARTITION else 2) * 2 * args.steps}), flush=True)
 
 
 def main():

@@ -122,6 +122,29 @@ tf_status tf_penta_solve(int nrow, int ncol, int dir,
                          const double* a, const double* b, const double* rhs, double* x,
                          void* dev_ws, void* cuda_stream);
 
+/*
+ * The same solve with a selectable algorithm (PAPER.md:647 names "the SPIKE method or
+ * cyclical reduction" as the way to parallelise a single system):
+ *   TF_PENTA_LU         one thread per system, two-sided LU (what tf_penta_solve runs);
+ *   TF_PENTA_PARTITION  every system is cut into nparts chunks of rows (nparts = 0: chosen from the shape so that
+ *                       about four marching warps per SM exist): (1) per chunk, elimination from both ends with the
+ *                       two coupling columns as extra right-hand sides gives exact relations between the chunk's
+ *                       four end unknowns and the four unknowns outside it, (2) the reduced system of 4*nparts end
+ *                       unknowns per system is solved, (3) all chunks are solved independently with corrected
+ *                       right-hand sides.  Same solution up to rounding; for few, long systems (nsys << 20 000).
+ * tf_penta_partition_chunks returns the chunk count that will be used (1 = the shape falls back to TF_PENTA_LU:
+ * odd nrow or ncol, fewer than 32 systems, or systems shorter than 192); 0 for invalid arguments.
+ * dev_ws needs tf_penta_workspace_bytes_ex(nrow, ncol, dir, variant, nparts) bytes.  Arrays must be 16-byte
+ * aligned for TF_PENTA_PARTITION (TF_ERR_UNSUPPORTED otherwise).
+ */
+typedef enum { TF_PENTA_LU = 0, TF_PENTA_PARTITION = 1 } tf_penta_variant;
+int       tf_penta_partition_chunks(int nrow, int ncol, int dir, int nparts);
+size_t    tf_penta_workspace_bytes_ex(int nrow, int ncol, int dir, int variant, int nparts);
+tf_status tf_penta_solve_ex(int nrow, int ncol, int dir, int variant, int nparts,
+                            const double* e, const double* c, const double* d,
+                            const double* a, const double* b, const double* rhs, double* x,
+                            void* dev_ws, void* cuda_stream);
+
 /* Text of the last error on this context ("" if none); ctx == NULL: last error of a failed
  * tf_create* / tf_penta_solve on this thread.  Valid until the next call. */
 const char* tf_last_error(const tf_ctx* ctx);

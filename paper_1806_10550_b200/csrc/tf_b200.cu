@@ -7,6 +7,7 @@
 #include "tf_bwd.cuh"
 #include "tf_fwd.cuh"
 
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdio>
@@ -436,6 +437,78 @@ tf_status reduce_field(tf_ctx* c, const double* dev_field, double scale, double*
     return TF_OK;
 }
 
+// ---- partition variant of the isolated solver (tf_partition.cuh): interface pass, reduced system, chunk solves
+constexpr int PART_MIN_LEN = 96;          // shortest admitted line length per chunk (chunks keep >= 81 rows)
+constexpr int PART_MAX = 256;             // the reduced system is solved serially per line
+constexpr int PI_NST = 4;                 // interface pass, columns: 4 stages x 12 KiB
+constexpr int PJ_NST = 3;                 // interface pass, rows: 3 stages x 24 KiB
+
+tf_status penta_partition(int nrow, int ncol, int dir, int P, const double* e, const double* c, const double* d,
+                          const double* a, const double* b, const double* rhs, double* x, char* ws, size_t fb,
+                          cudaStream_t st)
+{
+    double* al = (double*)ws;
+    double* be = (double*)(ws + fb);
+    double* zz = (double*)(ws + 2 * fb);
+    const size_t nsys = (size_t)(dir ? ncol : nrow);
+    double* iface = (double*)(ws + 3 * fb);
+    double* rc = iface + (size_t)P * 2 * IF_VALS * nsys;
+    double* X = rc + (size_t)P * RC_VALS * nsys;
+    const double* in6[6] = {e, c, d, a, b, rhs};
+    bool ok = ((uintptr_t)ws % 16 == 0) && ((uintptr_t)x % 16 == 0);
+    for (int k = 0; k < 6; ++k) ok = ok && ((uintptr_t)in6[k] % 16 == 0);
+    Maps6 M;
+    CUtensorMap mw[3], mx;
+    const double* w3[3] = {al, be, zz};
+    if (dir == 1) {
+        for (int k = 0; k < 6; ++k) ok = ok && make_map2d(&M.m[k], in6[k], ncol, nrow, 32, PC_RS, false);
+        for (int k = 0; k < 3; ++k) ok = ok && make_map2d(&mw[k], w3[k], ncol, nrow, 32, YT_RS, false);
+    } else {
+        for (int k = 0; k < 6; ++k) ok = ok && make_map2d(&M.m[k], in6[k], ncol, nrow, 16, 32, true);
+        for (int k = 0; k < 3; ++k) ok = ok && make_map2d(&mw[k], w3[k], nrow, ncol, 32, 16, false);
+        ok = ok && make_map2d(&mx, x, ncol, nrow, 16, 32, true);
+    }
+    if (!ok) return fail(nullptr, TF_ERR_UNSUPPORTED, "partition variant: 16-byte aligned arrays and TMA tensor maps required");
+    const dim3 g((unsigned)((nsys + 31) / 32), 2, (unsigned)P);
+    if (dir == 1) {
+        constexpr size_t SMI = (size_t)PI_NST * 6 * PC_RS * 32 * 8 + 8 * PI_NST + 1024;
+        constexpr size_t SMF = (size_t)PC_NST * 6 * PC_RS * 32 * 8 + 8 * PC_NST + 1024;
+        constexpr size_t SMB = (size_t)YT_NST * 3 * YT_RS * 32 * 8 + 8 * YT_NST + 1024;
+        static DevOnce ready;
+        if (!ready.done()) {
+            cudaError_t ee = opt_in_smem(penta_col_iface_kernel<PI_NST, PC_RS>, SMI);
+            if (ee == cudaSuccess) ee = opt_in_smem(penta_col_fwd2_kernel<PC_NST, PC_RS>, SMF);
+            if (ee == cudaSuccess) ee = opt_in_smem(ybwd2_tma_kernel<YT_NST, YT_RS, true>, SMB);
+            if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
+            ready.mark();
+        }
+        penta_col_iface_kernel<PI_NST, PC_RS><<<g, 32, SMI, st>>>(M, nrow, ncol, P, iface);
+        penta_reduced_kernel<<<(unsigned)((nsys + 127) / 128), 128, 0, st>>>((int)nsys, P, iface, rc, X);
+        penta_col_fwd2_kernel<PC_NST, PC_RS><<<g, 32, SMF, st>>>(M, nrow, ncol, 0, al, be, zz, P, X);
+        ybwd2_tma_kernel<YT_NST, YT_RS, true><<<g, 32, SMB, st>>>(mw[0], mw[1], mw[2], ncol, nrow, 0, al, be, zz, x, P);
+    } else {
+        constexpr size_t SMI = (size_t)PJ_NST * 6 * 32 * 16 * 8 + 8 * PJ_NST + 1024;
+        constexpr size_t SMF = (size_t)PR_NST * 6 * 32 * 16 * 8 + 8 * PR_NST + 1024;
+        constexpr size_t SMB = (size_t)XT_NST * 4 * 16 * 32 * 8 + 8 * XT_NST + 1024;
+        static DevOnce ready;
+        if (!ready.done()) {
+            cudaError_t ee = opt_in_smem(penta_row_iface_kernel<PJ_NST>, SMI);
+            if (ee == cudaSuccess) ee = opt_in_smem(penta_row_fwd2_kernel<PR_NST>, SMF);
+            if (ee == cudaSuccess) ee = opt_in_smem(xbwd2_tma_kernel<XT_NST, false, true>, SMB);
+            if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
+            ready.mark();
+        }
+        penta_row_iface_kernel<PJ_NST><<<g, 32, SMI, st>>>(M, nrow, ncol, P, iface);
+        penta_reduced_kernel<<<(unsigned)((nsys + 127) / 128), 128, 0, st>>>((int)nsys, P, iface, rc, X);
+        penta_row_fwd2_kernel<PR_NST><<<g, 32, SMF, st>>>(M, nrow, ncol, 0, al, be, zz, P, X);
+        xbwd2_tma_kernel<XT_NST, false, true><<<g, 32, SMB, st>>>(mw[0], mw[1], mw[2], mx, mx, ncol, nrow, 0, al, be, zz, nullptr, P);
+    }
+    count_launch(4);
+    cudaError_t ee = cudaGetLastError();
+    if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "tf_penta_solve_ex (partition) launch");
+    return TF_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -616,15 +689,51 @@ size_t tf_penta_workspace_bytes(int nrow, int ncol)
     return 3 * align_up((size_t)nrow * ncol * sizeof(double));
 }
 
+int tf_penta_partition_chunks(int nrow, int ncol, int dir, int nparts)
+{
+    if (nrow < 1 || ncol < 1 || (dir != 0 && dir != 1) || nparts < 0) return 0;
+    const int len = dir ? nrow : ncol, nsys = dir ? ncol : nrow;
+    const int pmax = std::min(len / PART_MIN_LEN, PART_MAX);          // every chunk keeps >= PART_MIN_LEN - 16 rows
+    if (pmax < 2 || nsys < 32 || nrow % 2 || ncol % 2) return 1;      // the chunked kernels are the TMA ones only
+    if (nparts > 0) return std::min(nparts, pmax);
+    // auto: enough marching warps (2 per chunk and strip of 32 lines) for ~4 per SM, chunks not shorter than 256 rows
+    const int strips = (nsys + 31) / 32;
+    const int want = (2 * num_sms() + strips - 1) / strips;
+    if (want < 6) return 1;               // >= ~1600 lines: thread-per-line is already HBM-bound (measured crossover ~2048)
+    return std::max(1, std::min(std::min(want, len / 256), pmax));
+}
+
+size_t tf_penta_workspace_bytes_ex(int nrow, int ncol, int dir, int variant, int nparts)
+{
+    const size_t lu = tf_penta_workspace_bytes(nrow, ncol);
+    if (lu == 0 || variant != TF_PENTA_PARTITION) return lu;
+    const int P = tf_penta_partition_chunks(nrow, ncol, dir, nparts);
+    const size_t nsys = (size_t)(dir ? ncol : nrow);
+    return lu + align_up((size_t)P * (2 * IF_VALS + RC_VALS + 4) * nsys * sizeof(double));
+}
+
 tf_status tf_penta_solve(int nrow, int ncol, int dir, const double* e, const double* c, const double* d,
                          const double* a, const double* b, const double* rhs, double* x, void* dev_ws,
                          void* cuda_stream)
 {
+    return tf_penta_solve_ex(nrow, ncol, dir, TF_PENTA_LU, 0, e, c, d, a, b, rhs, x, dev_ws, cuda_stream);
+}
+
+tf_status tf_penta_solve_ex(int nrow, int ncol, int dir, int variant, int nparts, const double* e, const double* c,
+                            const double* d, const double* a, const double* b, const double* rhs, double* x,
+                            void* dev_ws, void* cuda_stream)
+{
     if (nrow < 1 || ncol < 1 || (dir != 0 && dir != 1)) return fail(nullptr, TF_ERR_INVALID_ARG, "bad shape or dir");
     if ((dir ? nrow : ncol) < 3) return fail(nullptr, TF_ERR_INVALID_ARG, "system length must be >= 3");
     if (!e || !c || !d || !a || !b || !rhs || !x || !dev_ws) return fail(nullptr, TF_ERR_INVALID_ARG, "NULL pointer");
+    if (variant != TF_PENTA_LU && variant != TF_PENTA_PARTITION) return fail(nullptr, TF_ERR_UNSUPPORTED, "unknown variant");
+    if (nparts < 0) return fail(nullptr, TF_ERR_INVALID_ARG, "nparts < 0");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t fb = align_up((size_t)nrow * ncol * sizeof(double));
+    if (variant == TF_PENTA_PARTITION) {
+        const int P = tf_penta_partition_chunks(nrow, ncol, dir, nparts);
+        if (P > 1) return penta_partition(nrow, ncol, dir, P, e, c, d, a, b, rhs, x, (char*)dev_ws, fb, st);
+    }
     double* al = (double*)dev_ws;
     double* be = (double*)((char*)dev_ws + fb);
     double* zz = (double*)((char*)dev_ws + 2 * fb);
@@ -650,7 +759,7 @@ tf_status tf_penta_solve(int nrow, int ncol, int dir, const double* e, const dou
                 if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
                 ready.mark();
             }
-            penta_col_fwd2_kernel<PC_NST, PC_RS><<<dim3((ncol + 31) / 32, 2), 32, SM, st>>>(M, nrow, ncol, mid, al, be, zz);
+            penta_col_fwd2_kernel<PC_NST, PC_RS><<<dim3((ncol + 31) / 32, 2), 32, SM, st>>>(M, nrow, ncol, mid, al, be, zz, 1, nullptr);
             cudaError_t le = launch_ybwd2(mw, true, ncol, nrow, mid, al, be, zz, x, st);
             if (le != cudaSuccess) return cuda_fail(nullptr, le, "ybwd2 launch");
         } else {
@@ -680,7 +789,7 @@ tf_status tf_penta_solve(int nrow, int ncol, int dir, const double* e, const dou
                 ready.mark();
             }
             const dim3 g((nrow + 31) / 32, 2);
-            penta_row_fwd2_kernel<PR_NST><<<g, 32, SMF, st>>>(M, nrow, ncol, mid, al, be, zz);
+            penta_row_fwd2_kernel<PR_NST><<<g, 32, SMF, st>>>(M, nrow, ncol, mid, al, be, zz, 1, nullptr);
             cudaError_t le = launch_xbwd2_n<XT_NST, false>(mw, mx, mx, g, ncol, nrow, mid, al, be, zz, nullptr, st);
             if (le != cudaSuccess) return cuda_fail(nullptr, le, "xbwd2 launch");
         } else {

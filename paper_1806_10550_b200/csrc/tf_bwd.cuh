@@ -9,6 +9,7 @@
 #include "tf_async.cuh"
 #include "tf_tma.cuh"
 #include "tf_device.cuh"
+#include "tf_partition.cuh"
 
 namespace tf {
 
@@ -84,11 +85,13 @@ __device__ __forceinline__ Join babe_join(const double* c)
 }
 
 // y direction: coefficient fields [ny][nx], lane <-> column.  grid (ceil(nx/32), 2): blockIdx.y = half.
-template <int NST, int RS>
+// CH (partition variant of the isolated solver, tf_partition.cuh step 3): gridDim.z = P chunks, each an independent
+// system over rows [lo, hi) split at its own mid; CH = false is the sweep's kernel (lo = 0, hi = ny).
+template <int NST, int RS, bool CH = false>
 __global__ void __launch_bounds__(32)
 ybwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__ CUtensorMap mB,
-                 const __grid_constant__ CUtensorMap mZ, int nx, int ny, int mid, const double* __restrict__ al,
-                 const double* __restrict__ be, const double* __restrict__ zz, double* __restrict__ w)
+                 const __grid_constant__ CUtensorMap mZ, int nx, int ny, int mid_arg, const double* __restrict__ al,
+                 const double* __restrict__ be, const double* __restrict__ zz, double* __restrict__ w, int P = 1)
 {
     extern __shared__ unsigned char raw[];
     unsigned char* base = align1024(raw);
@@ -99,7 +102,9 @@ ybwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
     const int i0 = blockIdx.x * 32, i = i0 + lane;
     const int dir = blockIdx.y;
     const bool colok = i < nx;
-    const int nrows = dir ? ny - mid : mid;
+    const int lo = CH ? chunk_lo(blockIdx.z, P, ny) : 0, hi = CH ? chunk_lo(blockIdx.z + 1, P, ny) : ny;
+    const int mid = CH ? chunk_mid(lo, hi) : mid_arg;
+    const int nrows = dir ? hi - mid : mid - lo;
     const int ntile = (nrows + RS - 1) / RS;
     if (lane == 0) {
 #pragma unroll
@@ -138,7 +143,7 @@ ybwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
         const int jb = box_row(q);
         const double* d = sm + (size_t)s * 3 * BOX + lane;
         if (dir == 0) {
-            if (jb >= 0) {                                   // full tile: branch-free, one running pointer
+            if (jb >= lo) {                                  // full tile: branch-free, one running pointer
                 double* wp = w + (size_t)(jb + RS - 1) * nx + i;
 #pragma unroll
                 for (int r = RS - 1; r >= 0; --r) {
@@ -150,7 +155,7 @@ ybwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
             } else {
 #pragma unroll
                 for (int r = RS - 1; r >= 0; --r) {
-                    if (jb + r >= 0) {
+                    if (jb + r >= lo) {
                         const double x = fma(-d[r * 32], w1, fma(-d[BOX + r * 32], w2, d[2 * BOX + r * 32]));
                         if (colok) w[(size_t)(jb + r) * nx + i] = x;
                         w2 = w1; w1 = x;
@@ -158,7 +163,7 @@ ybwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
                 }
             }
         } else {
-            if (jb + RS <= ny) {
+            if (jb + RS <= hi) {
                 double* wp = w + (size_t)jb * nx + i;
 #pragma unroll
                 for (int r = 0; r < RS; ++r) {
@@ -170,7 +175,7 @@ ybwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
             } else {
 #pragma unroll
                 for (int r = 0; r < RS; ++r) {
-                    if (jb + r < ny) {
+                    if (jb + r < hi) {
                         const double x = fma(-d[r * 32], w1, fma(-d[BOX + r * 32], w2, d[2 * BOX + r * 32]));
                         if (colok) w[(size_t)(jb + r) * nx + i] = x;
                         w2 = w1; w1 = x;
@@ -216,12 +221,14 @@ ybwd2_plain_kernel(int nx, int ny, int mid, const double* __restrict__ al, const
 // ---------------------------------------------------------------------------------------------
 // UPDATE = true: the sweep's S7 (u tile loaded, updated in place, stored; residual reduced into red).
 // UPDATE = false: plain solve, the solution tile is stored through mUout (isolated solver, config 4).
-template <int NST, bool UPDATE>
+// CH: chunks of columns [lo, hi) as independent systems (see ybwd2_tma_kernel); interior chunk bounds and every mid
+// are multiples of the tile width, so tiles of different CTAs stay disjoint.
+template <int NST, bool UPDATE, bool CH = false>
 __global__ void __launch_bounds__(32)
 xbwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__ CUtensorMap mB,
                  const __grid_constant__ CUtensorMap mZ, const __grid_constant__ CUtensorMap mUin,
-                 const __grid_constant__ CUtensorMap mUout, int nx, int ny, int mid, const double* __restrict__ alT,
-                 const double* __restrict__ beT, const double* __restrict__ zzT, double* __restrict__ red)
+                 const __grid_constant__ CUtensorMap mUout, int nx, int ny, int mid_arg, const double* __restrict__ alT,
+                 const double* __restrict__ beT, const double* __restrict__ zzT, double* __restrict__ red, int P = 1)
 {
     constexpr int CS = 16;                                   // columns per stage (= one 128-byte swizzled row)
     constexpr int BOX = CS * 32;                             // doubles per coefficient box
@@ -233,7 +240,9 @@ xbwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
     const int j0 = blockIdx.x * 32;
     const int dir = blockIdx.y;
     const bool rowok = j0 + lane < ny;
-    const int ncols = dir ? nx - mid : mid;
+    const int lo = CH ? chunk_lo(blockIdx.z, P, nx) : 0, hi = CH ? chunk_lo(blockIdx.z + 1, P, nx) : nx;
+    const int mid = CH ? chunk_mid(lo, hi) : mid_arg;
+    const int ncols = dir ? hi - mid : mid - lo;
     const int ntile = (ncols + CS - 1) / CS;
     if (lane == 0) {
 #pragma unroll
@@ -271,7 +280,7 @@ xbwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
     for (int q = 0; q < ntile; ++q) {
         const int s = q % NST;
         mbar_wait(full + s, (q / NST) & 1);
-        const int i0 = tile_col(q), cols_ok = min(CS, nx - i0);
+        const int i0 = tile_col(q), cols_ok = min(CS, hi - i0);
         unsigned char* d = base + (size_t)s * STAGE;
         const double* cf = reinterpret_cast<const double*>(d) + lane;
         unsigned char* su = d + 3 * BOX * 8;

@@ -7,6 +7,7 @@
 #pragma once
 #include "tf_reduce.cuh"
 #include "tf_tma.cuh"
+#include "tf_partition.cuh"
 
 namespace tf {
 
@@ -135,15 +136,15 @@ penta_row_bwd_kernel(int nrow, int ncol, const double* __restrict__ alT, const d
 // One warp per CTA; the elimination chain (52 cycles x N/2 rows) is far below the HBM time of these kernels,
 // so no producer warps are needed: the marching warp reads its rows straight from the TMA-filled stages.
 // =============================================================================================
-struct Maps6 { CUtensorMap m[6]; };      // e, c, d, a, b, rhs
-
 // ---- systems = columns (lanes along the contiguous index).  grid (ceil(ncol/32), 2), blockIdx.y = half:
 // half 0 eliminates rows 0 .. mid-1 downwards, half 1 rows nrow-1 .. mid upwards (reversed system: e<->b, c<->a).
 // Coefficients are stored [row][col] like the inputs; ybwd2_tma_kernel / ybwd2_plain_kernel finish the solve.
+// Partition variant (tf_partition.cuh step 3): gridDim.z = P chunks, each an independent system over rows [lo, hi)
+// whose first two right-hand sides of either march are corrected by the outside unknowns X ([P][4][ncol]).
 template <int NST, int RS>
 __global__ void __launch_bounds__(32)
-penta_col_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int mid, double* __restrict__ al,
-                      double* __restrict__ be, double* __restrict__ zz)
+penta_col_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int mid_arg, double* __restrict__ al,
+                      double* __restrict__ be, double* __restrict__ zz, int P, const double* __restrict__ X)
 {
     extern __shared__ unsigned char raw[];
     unsigned char* base = align1024(raw);
@@ -152,10 +153,18 @@ penta_col_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int m
     uint64_t* full = reinterpret_cast<uint64_t*>(base + (size_t)NST * 6 * BOX * 8);
     const int lane = threadIdx.x;
     const int i0 = blockIdx.x * 32, i = i0 + lane;
-    const int dir = blockIdx.y;
+    const int dir = blockIdx.y, p = blockIdx.z;
     const int colok = i < ncol ? 1 : 0;
-    const int jmin = dir ? mid : 0, jmax = dir ? nrow : mid;
+    const int lo = chunk_lo(p, P, nrow), hi = chunk_lo(p + 1, P, nrow);
+    const int mid = P > 1 ? chunk_mid(lo, hi) : mid_arg;
+    const int jmin = dir ? mid : lo, jmax = dir ? hi : mid;
     const int nrows = jmax - jmin;
+    double xfar = 0.0, xnear = 0.0;                          // known unknowns just outside this march's first row
+    if (P > 1 && (dir ? p < P - 1 : p > 0)) {
+        const double* xo = X + (size_t)(dir ? (p + 1) * 4 : (p - 1) * 4 + 2) * ncol + min(i, ncol - 1);
+        xfar = dir ? xo[ncol] : xo[0];
+        xnear = dir ? xo[0] : xo[ncol];
+    }
     const int ntile = (nrows + RS - 1) / RS;
     if (lane == 0) {
 #pragma unroll
@@ -163,7 +172,7 @@ penta_col_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int m
         mbar_fence_init();
     }
     __syncwarp();
-    auto box_row = [&](int q) { return dir ? nrow - (q + 1) * RS : q * RS; };
+    auto box_row = [&](int q) { return dir ? hi - (q + 1) * RS : lo + q * RS; };
     auto issue = [&](int q) {
         if (q < ntile && lane == 0) {
             const int s = q % NST;
@@ -177,7 +186,7 @@ penta_col_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int m
     for (int q = 0; q < NST; ++q) issue(q);
     Elim2 S = elim2_init();
     const ptrdiff_t step = dir ? -(ptrdiff_t)ncol : (ptrdiff_t)ncol;
-    ptrdiff_t o = (ptrdiff_t)(dir ? nrow : -1) * ncol + i;   // the row before the first one
+    ptrdiff_t o = (ptrdiff_t)(dir ? hi : lo - 1) * ncol + i;   // the row before the first one
     const int oe = dir ? 4 * BOX : 0, oc = dir ? 3 * BOX : BOX, oa = dir ? BOX : 3 * BOX, ob = dir ? 0 : 4 * BOX;
     int k = 0;                                               // rows eliminated so far
     for (int q = 0; q < ntile; ++q) {
@@ -202,8 +211,11 @@ penta_col_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int m
                 const int j = jb + r;
                 if (j >= jmin && j < jmax) {
                     double va, vb, vz;
-                    elim2_row(S, d[oe + r * 32], d[oc + r * 32], d[2 * BOX + r * 32], d[oa + r * 32], d[ob + r * 32],
-                              d[5 * BOX + r * 32], va, vb, vz);
+                    const double ve = d[oe + r * 32], vc = d[oc + r * 32];
+                    double vy = d[5 * BOX + r * 32];
+                    if (k == 0) vy -= ve * xfar + vc * xnear;
+                    if (k == 1) vy -= ve * xnear;
+                    elim2_row(S, ve, vc, d[2 * BOX + r * 32], d[oa + r * 32], d[ob + r * 32], vy, va, vb, vz);
                     st3_if(colok && k > 0, al + o, va, be + o, vb, zz + o, vz);
                     o += step;
                     ++k;
@@ -222,10 +234,11 @@ penta_col_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int m
 // [32 rows x 16 cols] TMA boxes with the 128-byte swizzle (conflict-free column reads); coefficients are stored
 // TRANSPOSED [col][row] (coalesced).  grid (ceil(nrow/32), 2): half 0 columns 0 .. mid-1 ascending, half 1
 // columns ncol-1 .. mid descending.  xbwd2_tma_kernel<.., false> / penta_row_bwd2_plain_kernel finish the solve.
+// Partition variant: gridDim.z = P chunks of columns [lo, hi), X = [P][4][nrow] (see penta_col_fwd2_kernel).
 template <int NST>
 __global__ void __launch_bounds__(32)
-penta_row_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int mid, double* __restrict__ alT,
-                      double* __restrict__ beT, double* __restrict__ zzT)
+penta_row_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int mid_arg, double* __restrict__ alT,
+                      double* __restrict__ beT, double* __restrict__ zzT, int P, const double* __restrict__ X)
 {
     constexpr int CS = 16;
     constexpr int TILE = 32 * CS * 8;                        // bytes per array tile (4 KiB, 1024-aligned)
@@ -234,9 +247,17 @@ penta_row_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int m
     uint64_t* full = reinterpret_cast<uint64_t*>(base + (size_t)NST * 6 * TILE);
     const int lane = threadIdx.x;
     const int r0 = blockIdx.x * 32;
-    const int dir = blockIdx.y;
+    const int dir = blockIdx.y, p = blockIdx.z;
     const int rowok = r0 + lane < nrow ? 1 : 0;
-    const int imin = dir ? mid : 0, imax = dir ? ncol : mid;
+    const int lo = chunk_lo(p, P, ncol), hi = chunk_lo(p + 1, P, ncol);
+    const int mid = P > 1 ? chunk_mid(lo, hi) : mid_arg;
+    const int imin = dir ? mid : lo, imax = dir ? hi : mid;
+    double xfar = 0.0, xnear = 0.0;
+    if (P > 1 && (dir ? p < P - 1 : p > 0)) {
+        const double* xo = X + (size_t)(dir ? (p + 1) * 4 : (p - 1) * 4 + 2) * nrow + min(r0 + lane, nrow - 1);
+        xfar = dir ? xo[nrow] : xo[0];
+        xnear = dir ? xo[0] : xo[nrow];
+    }
     const int ncols = imax - imin;
     const int ntile = (ncols + CS - 1) / CS;
     if (lane == 0) {
@@ -245,7 +266,7 @@ penta_row_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int m
         mbar_fence_init();
     }
     __syncwarp();
-    auto tile_col = [&](int q) { return dir ? ncol - (q + 1) * CS : q * CS; };
+    auto tile_col = [&](int q) { return dir ? hi - (q + 1) * CS : lo + q * CS; };
     auto issue = [&](int q) {
         if (q < ntile && lane == 0) {
             const int s = q % NST;
@@ -259,7 +280,7 @@ penta_row_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int m
     for (int q = 0; q < NST; ++q) issue(q);
     Elim2 S = elim2_init();
     const ptrdiff_t step = dir ? -(ptrdiff_t)nrow : (ptrdiff_t)nrow;
-    ptrdiff_t o = (ptrdiff_t)(dir ? ncol : -1) * nrow + r0 + lane;
+    ptrdiff_t o = (ptrdiff_t)(dir ? hi : lo - 1) * nrow + r0 + lane;
     const int oe = dir ? 4 * TILE : 0, oc = dir ? 3 * TILE : TILE, oa = dir ? TILE : 3 * TILE, ob = dir ? 0 : 4 * TILE;
     const int sx = (lane & 7) << 4;
     int k = 0;
@@ -287,7 +308,11 @@ penta_row_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int m
                 const int i = ib + c;
                 if (i >= imin && i < imax) {
                     double va, vb, vz;
-                    elim2_row(S, at(oe, c), at(oc, c), at(2 * TILE, c), at(oa, c), at(ob, c), at(5 * TILE, c), va, vb, vz);
+                    const double ve = at(oe, c), vc = at(oc, c);
+                    double vy = at(5 * TILE, c);
+                    if (k == 0) vy -= ve * xfar + vc * xnear;
+                    if (k == 1) vy -= ve * xnear;
+                    elim2_row(S, ve, vc, at(2 * TILE, c), at(oa, c), at(ob, c), vy, va, vb, vz);
                     st3_if(rowok && k > 0, alT + o, va, beT + o, vb, zzT + o, vz);
                     o += step;
                     ++k;

@@ -105,3 +105,24 @@ def penta_system(nrow, ncol, seed, rows=None):
         for arr, v in zip(out, (e, c, d, a, b, rhs)):
             arr[k] = v
     return out  # e, c, d, a, b, rhs
+
+
+def penta_system_bending(nsys, n, seed, sigma):
+    """Weakly dominant test systems for the partition variant of the isolated solver: A = diag(1 + U[0,1]) +
+    sigma * D2^T diag(w) D2 with D2 the interior second differences of a line of n points and w ~ U[0.5, 1.5]
+    (symmetric positive definite, the structure of I + s J of the sweeps with f0 = w; couples rows over
+    ~ sigma^(1/4) neighbours, unlike the strictly dominant config-4 systems whose coupling dies within a few rows).
+    Six [nsys][n] arrays e, c, d, a, b, rhs with system s = row s."""
+    rng = np.random.default_rng([seed, 77])
+    w = rng.uniform(0.5, 1.5, (nsys, n))
+    w[:, 0] = 0.0
+    w[:, -1] = 0.0
+    wm = np.concatenate([np.zeros((nsys, 1)), w[:, :-1]], axis=1)      # w_{i-1}
+    wp = np.concatenate([w[:, 1:], np.zeros((nsys, 1))], axis=1)       # w_{i+1}
+    e = sigma * wm
+    b = sigma * wp
+    c = -2.0 * sigma * (wm + w)
+    a = -2.0 * sigma * (w + wp)
+    d = 1.0 + rng.uniform(0.0, 1.0, (nsys, n)) + sigma * (wm + 4.0 * w + wp)
+    rhs = rng.uniform(-1.0, 1.0, (nsys, n))
+    return [np.ascontiguousarray(t) for t in (e, c, d, a, b, rhs)]

@@ -37,6 +37,9 @@ SYMBOLS = {
     "tf_mass": (ctypes.c_int, [_vp, _dp]),
     "tf_penta_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int, ctypes.c_int]),
     "tf_penta_solve": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int] + [_vp] * 9),
+    "tf_penta_partition_chunks": (ctypes.c_int, [ctypes.c_int] * 4),
+    "tf_penta_workspace_bytes_ex": (ctypes.c_size_t, [ctypes.c_int] * 5),
+    "tf_penta_solve_ex": (ctypes.c_int, [ctypes.c_int] * 5 + [_vp] * 9),
     "tf_set_profiling": (ctypes.c_int, [_vp, ctypes.c_int]),
     "tf_get_profile": (ctypes.c_int, [_vp, _dp, ctypes.POINTER(ctypes.c_ulonglong)]),
     "tf_last_error": (ctypes.c_char_p, [_vp]),
@@ -213,8 +216,17 @@ def advance_adaptive(ctx, dt, n_accept, grow=1.1, shrink=0.5, dt_max=0.1, dt_min
     return t, dt, hist
 
 
-def penta_solve(direction, e, c, d, a, b, rhs, out=None, workspace=None, stream=None):
-    """tf_penta_solve on torch CUDA float64 tensors [nrow][ncol]; direction 0: rows are systems, 1: columns.
+PENTA_LU, PENTA_PARTITION = 0, 1
+
+
+def penta_partition_chunks(nrow, ncol, direction, nparts=0):
+    """tf_penta_partition_chunks: chunks per system the partition variant will use for this shape (1 = LU)."""
+    return lib().tf_penta_partition_chunks(nrow, ncol, direction, nparts)
+
+
+def penta_solve(direction, e, c, d, a, b, rhs, out=None, workspace=None, stream=None, variant=PENTA_LU, nparts=0):
+    """tf_penta_solve_ex on torch CUDA float64 tensors [nrow][ncol]; direction 0: rows are systems, 1: columns.
+    variant PENTA_LU (thread per system) or PENTA_PARTITION (nparts chunks per system, 0 = automatic).
     Enqueues on the current stream and returns `out` without synchronising."""
     torch = _torch()
     ts = (e, c, d, a, b, rhs)
@@ -226,13 +238,14 @@ def penta_solve(direction, e, c, d, a, b, rhs, out=None, workspace=None, stream=
     if out is None:
         out = torch.empty_like(e)
     L = lib()
-    need = L.tf_penta_workspace_bytes(nrow, ncol)
+    need = L.tf_penta_workspace_bytes_ex(nrow, ncol, direction, variant, nparts)
     if workspace is None:
         workspace = torch.empty(need, dtype=torch.uint8, device=e.device)
     if workspace.numel() * workspace.element_size() < need or workspace.data_ptr() % 256:
         raise ValueError("workspace too small or not 256-byte aligned")
     st = (torch.cuda.current_stream(e.device) if stream is None else stream).cuda_stream
-    rc = L.tf_penta_solve(nrow, ncol, direction, *[t.data_ptr() for t in ts], out.data_ptr(), workspace.data_ptr(), st)
+    rc = L.tf_penta_solve_ex(nrow, ncol, direction, variant, nparts, *[t.data_ptr() for t in ts], out.data_ptr(),
+                             workspace.data_ptr(), st)
     if rc != OK:
-        _err(None, rc, "tf_penta_solve")
+        _err(None, rc, "tf_penta_solve_ex")
     return out

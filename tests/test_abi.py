@@ -37,6 +37,16 @@ def test_workspace_sizes_and_host_side_validation():
     assert L.tf_create(ctypes.byref(h), 128, 128, 0.1, 0.1, 100.0, 0.1, 3, 2, 1) == tf.ERR_UNSUPPORTED
     assert b"2.28" in L.tf_last_error(None)
     assert L.tf_penta_solve(8, 8, 2, *([None] * 9)) == tf.ERR_INVALID_ARG
+    # partition variant: chunk count and workspace are pure host functions of the shape
+    assert L.tf_penta_partition_chunks(256, 16384, 0, 0) >= 16          # few long systems: many chunks
+    assert L.tf_penta_partition_chunks(16384, 16384, 0, 0) == 1         # config 4 itself: thread per line fills the GPU
+    assert L.tf_penta_partition_chunks(64, 100, 0, 0) == 1 and L.tf_penta_partition_chunks(33, 400, 0, 4) == 1
+    assert L.tf_penta_partition_chunks(64, 512, 0, 4) == 4 and L.tf_penta_partition_chunks(512, 64, 1, 4) == 4
+    assert L.tf_penta_partition_chunks(64, 512, 0, 100) == 5            # clamped: chunks keep >= 81 rows
+    assert L.tf_penta_workspace_bytes_ex(64, 512, 0, tf.PENTA_LU, 4) == L.tf_penta_workspace_bytes(64, 512)
+    assert L.tf_penta_workspace_bytes_ex(64, 512, 0, tf.PENTA_PARTITION, 4) >= \
+        L.tf_penta_workspace_bytes(64, 512) + 4 * 36 * 64 * 8
+    assert L.tf_penta_solve_ex(8, 8, 0, 7, 0, *([None] * 9)) == tf.ERR_INVALID_ARG
     assert L.tf_kernel_launches() == 0
 
 
