@@ -83,6 +83,14 @@ tf_status tf_set_pressure(tf_ctx* ctx, tf_pressure kind, const double* params, i
  * iterations per step and the step is always accepted (parity mode). */
 tf_status tf_set_newton(tf_ctx* ctx, double tol, int max_iter, int fixed_iters);
 
+/* Host decision of Fig. 1 (PAPER.md:256-258; the paper reads one flag per 16x16 block per iteration, :675-683).
+ * batch = 0: the host reads the residual after every iteration before launching the next.  batch > 0 (default 2):
+ * speculative launch-ahead -- iterations are enqueued in batches (the first as long as the last accepted step's
+ * iteration count, then `batch` at a time) and the residual records of a batch are read at once; iterations enqueued
+ * past the deciding one return immediately on the device, so iterates, iteration count and residual are exactly
+ * those of batch = 0.  0 <= batch <= 64. */
+tf_status tf_set_launch_ahead(tf_ctx* ctx, int batch);
+
 /* Copy nx*ny doubles into the context as u^n.  `h` is a device pointer if is_device_ptr != 0,
  * else a host pointer.  Rejects non-finite or non-positive values (Pi is singular at h = 0)
  * with TF_ERR_INVALID_ARG; the previous state is then kept. */

@@ -46,6 +46,8 @@ struct tf_ctx {
     double *part;                              // [RED_BLOCKS]
     double *scal;                              // [8] : scal[0] mass, (int*)(scal+1) flag
     double *pinned;                            // [4] host pinned readback
+    double *pinned_red;                        // [2*MAX_ITERS] host pinned copy of the residual records
+    int spec_batch, last_iters;                // speculative launch-ahead: batch size (0 = off), iterations of the last accepted step
     int mid_y, mid_x;                          // split rows / columns of the two-sided sweeps
     int num_sms;
     bool tma_y, tma_x;                         // TMA rings usable (row pitch multiple of 16 B, grid >= one box)
@@ -151,7 +153,7 @@ int num_sms()
 
 template <int NST>
 cudaError_t launch_ybwd2_n(const CUtensorMap* m, dim3 g, int nx, int ny, int mid, const double* al, const double* be,
-                           const double* zz, double* w, cudaStream_t st)
+                           const double* zz, double* w, cudaStream_t st, Gate gate)
 {
     constexpr size_t SM = (size_t)NST * 3 * YT_RS * 32 * 8 + 8 * NST + 1024;
     static DevOnce ready;
@@ -160,13 +162,14 @@ cudaError_t launch_ybwd2_n(const CUtensorMap* m, dim3 g, int nx, int ny, int mid
         if (e != cudaSuccess) return e;
         ready.mark();
     }
-    ybwd2_tma_kernel<NST, YT_RS><<<g, 32, SM, st>>>(m[0], m[1], m[2], nx, ny, mid, al, be, zz, w);
+    ybwd2_tma_kernel<NST, YT_RS><<<g, 32, SM, st>>>(m[0], m[1], m[2], nx, ny, mid, al, be, zz, w, 1, gate);
     return cudaGetLastError();
 }
 
 template <int NST, bool UPDATE>
 cudaError_t launch_xbwd2_n(const CUtensorMap* m, const CUtensorMap& uin, const CUtensorMap& uout, dim3 g, int nx, int ny,
-                           int mid, const double* alT, const double* beT, const double* zzT, double* red, cudaStream_t st)
+                           int mid, const double* alT, const double* beT, const double* zzT, double* red, cudaStream_t st,
+                           Gate gate = Gate{nullptr, 0.0})
 {
     constexpr size_t SM = (size_t)NST * 4 * 16 * 32 * 8 + 8 * NST + 1024;
     static DevOnce ready;
@@ -175,37 +178,37 @@ cudaError_t launch_xbwd2_n(const CUtensorMap* m, const CUtensorMap& uin, const C
         if (e != cudaSuccess) return e;
         ready.mark();
     }
-    xbwd2_tma_kernel<NST, UPDATE><<<g, 32, SM, st>>>(m[0], m[1], m[2], uin, uout, nx, ny, mid, alT, beT, zzT, red);
+    xbwd2_tma_kernel<NST, UPDATE><<<g, 32, SM, st>>>(m[0], m[1], m[2], uin, uout, nx, ny, mid, alT, beT, zzT, red, 1, gate);
     return cudaGetLastError();
 }
 
 // two-sided y back substitution (the y forward kernel is two-sided): TMA ring when the maps exist, else plain
 cudaError_t launch_ybwd2(const CUtensorMap* m, bool tma, int nx, int ny, int mid, const double* al, const double* be,
-                         const double* zz, double* w, cudaStream_t st)
+                         const double* zz, double* w, cudaStream_t st, Gate gate = Gate{nullptr, 0.0})
 {
     const dim3 g((nx + 31) / 32, 2);
     if (!tma) {
-        ybwd2_plain_kernel<<<g, 32, 0, st>>>(nx, ny, mid, al, be, zz, w);
+        ybwd2_plain_kernel<<<g, 32, 0, st>>>(nx, ny, mid, al, be, zz, w, gate);
         return cudaGetLastError();
     }
-    return launch_ybwd2_n<YT_NST>(m, g, nx, ny, mid, al, be, zz, w, st);
+    return launch_ybwd2_n<YT_NST>(m, g, nx, ny, mid, al, be, zz, w, st, gate);
 }
 
 // two-sided x back substitution + update + residual
 cudaError_t launch_xbwd2(const CUtensorMap* m, const CUtensorMap& uin, const CUtensorMap& uout, bool tma, int nx, int ny,
                          int mid, const double* alT, const double* beT, const double* zzT, const double* uk,
-                         double* unew, double* red, cudaStream_t st)
+                         double* unew, double* red, cudaStream_t st, Gate gate)
 {
     const dim3 g((ny + 31) / 32, 2);
     if (!tma) {
-        xbwd2_plain_kernel<<<g, 32, 0, st>>>(nx, ny, mid, alT, beT, zzT, uk, unew, red);
+        xbwd2_plain_kernel<<<g, 32, 0, st>>>(nx, ny, mid, alT, beT, zzT, uk, unew, red, gate);
         return cudaGetLastError();
     }
     // ring depth: 3 stages when every CTA must fit at once (4 per SM); 6 when there are at most 2 CTAs per SM
     // (measured at 4096^2: 0.149 -> 0.138 ms; the y ring showed no gain from more stages)
     if ((int)(g.x * g.y) > 2 * num_sms())
-        return launch_xbwd2_n<XT_NST, true>(m, uin, uout, g, nx, ny, mid, alT, beT, zzT, red, st);
-    return launch_xbwd2_n<2 * XT_NST, true>(m, uin, uout, g, nx, ny, mid, alT, beT, zzT, red, st);
+        return launch_xbwd2_n<XT_NST, true>(m, uin, uout, g, nx, ny, mid, alT, beT, zzT, red, st, gate);
+    return launch_xbwd2_n<2 * XT_NST, true>(m, uin, uout, g, nx, ny, mid, alT, beT, zzT, red, st, gate);
 }
 
 cudaError_t launch_ybwd(int nx, int ny, const double* al, const double* be, const double* zz, double* w,
@@ -234,7 +237,7 @@ constexpr int XW_NP = 4, XW_NSTG = 3;              // xfwd: per sub-problem 1 co
 // forward kernels: NSUB sub-problems per CTA (4: two strips/blocks x two halves; 2: one x two halves)
 template <int N, int M, bool FIRST, int NSUB>
 cudaError_t launch_yfwd(tf_ctx* c, const CUtensorMap& mu, int tma, const Params& P, const Dir& DX, const Dir& DY,
-                        const double* src, int grid)
+                        const double* src, int grid, Gate gate)
 {
     constexpr size_t SM = NSUB * (size_t)YW_NSTG * 5 * YW_RP * 32 * 8 + NSUB * YW_NP * (size_t)(2 * YW_RP + 4) * 32 * 8 +
                           (2 * NSUB * YW_NSTG + NSUB * YW_NP) * 8;
@@ -245,12 +248,12 @@ cudaError_t launch_yfwd(tf_ctx* c, const CUtensorMap& mu, int tma, const Params&
         if (e != cudaSuccess) return e;
         ready.mark();
     }
-    kern<<<grid, 32 * NSUB * (YW_NP + 1), SM, c->stream>>>(mu, c->mBn, tma, P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz);
+    kern<<<grid, 32 * NSUB * (YW_NP + 1), SM, c->stream>>>(mu, c->mBn, tma, P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz, gate);
     return cudaGetLastError();
 }
 
 template <int N, int M, int NSUB>
-cudaError_t launch_xfwd(tf_ctx* c, const Params& P, const Dir& DX, const double* src, int grid)
+cudaError_t launch_xfwd(tf_ctx* c, const Params& P, const Dir& DX, const double* src, int grid, Gate gate)
 {
     constexpr size_t SM = NSUB * ((size_t)XW_NSTG * 5 * XW_CK * XW_LD * 8 + 16 * XW_NSTG);
     auto kern = xfwd_ws_kernel<N, M, XW_NP, XW_NSTG, NSUB>;
@@ -260,15 +263,17 @@ cudaError_t launch_xfwd(tf_ctx* c, const Params& P, const Dir& DX, const double*
         if (e != cudaSuccess) return e;
         ready.mark();
     }
-    kern<<<grid, 32 * NSUB * (XW_NP + 1), SM, c->stream>>>(P, DX, c->mid_x, src, c->w, c->al, c->be, c->zz);
+    kern<<<grid, 32 * NSUB * (XW_NP + 1), SM, c->stream>>>(P, DX, c->mid_x, src, c->w, c->al, c->be, c->zz, gate);
     return cudaGetLastError();
 }
 
-// one pseudo-Newton iteration k: reads src (u^n if k == 0 else uk), writes uk, red[2k..2k+1]
+// one pseudo-Newton iteration k: reads src (u^n if k == 0 else uk), writes uk, red[2k..2k+1].  gated: the four
+// kernels return at once if iteration k-1's record says the step is already decided (speculative launch-ahead).
 template <int N, int M>
-cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
+cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated)
 {
     const Params& P = c->P;
+    const Gate gate = (gated && k > 0) ? Gate{c->red + 2 * (k - 1), c->tol} : Gate{nullptr, 0.0};
     const Dir DX = make_dir(s, P.dx), DY = make_dir(s, P.dy);
     const double* src = (k == 0) ? c->u : c->uk;
     // one CTA = NSUB sub-problems: two strips x two halves, or one strip x two halves when that still leaves SMs idle
@@ -280,38 +285,38 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
         const int tma = c->tma_yf ? 1 : 0;
         cudaError_t e;
         if (nstrip > c->num_sms)
-            e = k == 0 ? launch_yfwd<N, M, true, 4>(c, mu, tma, P, DX, DY, src, (nstrip + 1) / 2)
-                       : launch_yfwd<N, M, false, 4>(c, mu, tma, P, DX, DY, src, (nstrip + 1) / 2);
+            e = k == 0 ? launch_yfwd<N, M, true, 4>(c, mu, tma, P, DX, DY, src, (nstrip + 1) / 2, gate)
+                       : launch_yfwd<N, M, false, 4>(c, mu, tma, P, DX, DY, src, (nstrip + 1) / 2, gate);
         else
-            e = k == 0 ? launch_yfwd<N, M, true, 2>(c, mu, tma, P, DX, DY, src, nstrip)
-                       : launch_yfwd<N, M, false, 2>(c, mu, tma, P, DX, DY, src, nstrip);
+            e = k == 0 ? launch_yfwd<N, M, true, 2>(c, mu, tma, P, DX, DY, src, nstrip, gate)
+                       : launch_yfwd<N, M, false, 2>(c, mu, tma, P, DX, DY, src, nstrip, gate);
         if (e != cudaSuccess) return e;
     }
     if (ev) cudaEventRecord(ev[1], c->stream);
-    cudaError_t le = launch_ybwd2(c->mY, c->tma_y, P.nx, P.ny, c->mid_y, c->al, c->be, c->zz, c->w, c->stream);
+    cudaError_t le = launch_ybwd2(c->mY, c->tma_y, P.nx, P.ny, c->mid_y, c->al, c->be, c->zz, c->w, c->stream, gate);
     if (le != cudaSuccess) return le;
     if (ev) cudaEventRecord(ev[2], c->stream);
     {
         const int nblk = (P.ny + XW_R - 1) / XW_R;
-        cudaError_t e = nblk > c->num_sms ? launch_xfwd<N, M, 4>(c, P, DX, src, (nblk + 1) / 2)
-                                          : launch_xfwd<N, M, 2>(c, P, DX, src, nblk);
+        cudaError_t e = nblk > c->num_sms ? launch_xfwd<N, M, 4>(c, P, DX, src, (nblk + 1) / 2, gate)
+                                          : launch_xfwd<N, M, 2>(c, P, DX, src, nblk, gate);
         if (e != cudaSuccess) return e;
     }
     if (ev) cudaEventRecord(ev[3], c->stream);
     le = launch_xbwd2(c->mX, c->mU[src == c->ubuf[0] ? 0 : 1], c->mU[c->uk == c->ubuf[0] ? 0 : 1], c->tma_x, P.nx, P.ny,
-                      c->mid_x, c->al, c->be, c->zz, src, c->uk, c->red + 2 * k, c->stream);
+                      c->mid_x, c->al, c->be, c->zz, src, c->uk, c->red + 2 * k, c->stream, gate);
     if (le != cudaSuccess) return le;
     if (ev) cudaEventRecord(ev[4], c->stream);
     count_launch(4);
     return cudaGetLastError();
 }
 
-cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot)
+cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated)
 {
-    if (c->model == TF_PI_NLC) return launch_iteration<MODEL_NLC, 0>(c, s, k, slot);
-    if (c->model == TF_PI_POLYMER) return launch_iteration<MODEL_POLYMER, 0>(c, s, k, slot);
-    if (c->P.n == 3 && c->P.m == 2) return launch_iteration<3, 2>(c, s, k, slot);
-    return launch_iteration<0, 0>(c, s, k, slot);
+    if (c->model == TF_PI_NLC) return launch_iteration<MODEL_NLC, 0>(c, s, k, slot, gated);
+    if (c->model == TF_PI_POLYMER) return launch_iteration<MODEL_POLYMER, 0>(c, s, k, slot, gated);
+    if (c->P.n == 3 && c->P.m == 2) return launch_iteration<3, 2>(c, s, k, slot, gated);
+    return launch_iteration<0, 0>(c, s, k, slot, gated);
 }
 
 // after a stream sync: fold the event intervals of `niter` profiled iterations into the totals
@@ -381,12 +386,14 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
     c->red = (double*)sc;
     c->part = c->red + 2 * (MAX_ITERS + 1);
     c->scal = c->part + RED_BLOCKS;
-    e = cudaMallocHost((void**)&c->pinned, 4 * sizeof(double));
+    e = cudaMallocHost((void**)&c->pinned, (4 + 2 * (size_t)MAX_ITERS) * sizeof(double));
     if (e != cudaSuccess) {
         if (own) cudaFree(c->ws);
         delete c;
         return fail(nullptr, TF_ERR_ALLOC, std::string("cudaMallocHost: ") + cudaGetErrorString(e));
     }
+    c->pinned_red = c->pinned + 4;
+    c->spec_batch = 2; c->last_iters = 1;
     c->ubuf[0] = c->u; c->ubuf[1] = c->uk;
     {
         int dev = 0, sms = 148;
@@ -551,6 +558,15 @@ tf_status tf_set_newton(tf_ctx* c, double tol, int max_iter, int fixed_iters)
     return TF_OK;
 }
 
+tf_status tf_set_launch_ahead(tf_ctx* c, int batch)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    if (batch < 0 || batch > 64) return fail(c, TF_ERR_INVALID_ARG, "batch in [0,64]");
+    c->spec_batch = batch;
+    c->last_iters = 1;
+    return TF_OK;
+}
+
 tf_status tf_set_pressure(tf_ctx* c, tf_pressure kind, const double* p, int np)
 {
     if (!c) return TF_ERR_INVALID_ARG;
@@ -627,7 +643,7 @@ tf_status tf_step(tf_ctx* c, double dt, int* newton_iters, double* residual)
     if (fixed) {
         // parity mode: no host decision inside the step, one read at the end
         const bool prof = c->profiling && kmax <= 64;
-        for (; k < kmax; ++k) TF_CUDA(c, launch_iteration(c, s, k, prof ? k : -1));
+        for (; k < kmax; ++k) TF_CUDA(c, launch_iteration(c, s, k, prof ? k : -1, false));
         TF_CUDA(c, cudaMemcpyAsync(c->pinned, c->red + 2 * (kmax - 1), 2 * sizeof(double), cudaMemcpyDeviceToHost,
                                    c->stream));
         TF_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -635,18 +651,32 @@ tf_status tf_step(tf_ctx* c, double dt, int* newton_iters, double* residual)
         res = c->pinned[0];
         status = TF_OK;
     } else {
-        while (k < kmax) {
-            TF_CUDA(c, launch_iteration(c, s, k, 0));
-            TF_CUDA(c, cudaMemcpyAsync(c->pinned, c->red + 2 * k, 2 * sizeof(double), cudaMemcpyDeviceToHost,
-                                       c->stream));
+        // S8 with speculative launch-ahead: iterations are enqueued in batches -- the first as long as the previous
+        // step's iteration count (the count changes slowly from step to step), then `spec_batch` at a time -- and the
+        // host reads the residual records of a whole batch at once.  Iterations enqueued past the deciding one are
+        // gated off on the device (gate_closed), so the result is exactly that of deciding after every iteration.
+        const bool prof = c->profiling;
+        int enq = 0, done = 0;
+        int batch = c->spec_batch > 0 ? std::max(1, std::min(c->last_iters, prof ? 64 : kmax)) : 1;
+        bool decided = false;
+        while (!decided && done < kmax) {
+            const int upto = std::min(kmax, enq + batch);
+            for (; enq < upto; ++enq) TF_CUDA(c, launch_iteration(c, s, enq, prof ? enq - done : -1, true));
+            TF_CUDA(c, cudaMemcpyAsync(c->pinned_red + 2 * done, c->red + 2 * done, 2 * sizeof(double) * (size_t)(enq - done),
+                                       cudaMemcpyDeviceToHost, c->stream));
             TF_CUDA(c, cudaStreamSynchronize(c->stream));
-            collect_profile(c, 1);
-            ++k;
-            res = c->pinned[0];
-            const bool bad = c->pinned[1] != 0.0;
-            if (bad || res != res) break;
-            if (res < c->tol) { status = TF_OK; break; }
+            const int first = done;
+            for (; done < enq && !decided; ++done) {
+                k = done + 1;
+                res = c->pinned_red[2 * done];
+                const bool bad = c->pinned_red[2 * done + 1] != 0.0;
+                if (bad || res != res) decided = true;
+                else if (res < c->tol) { status = TF_OK; decided = true; }
+            }
+            if (prof) collect_profile(c, done - first);
+            batch = std::max(1, c->spec_batch);
         }
+        if (status == TF_OK) c->last_iters = k;
     }
     if (status == TF_OK) std::swap(c->u, c->uk);     // pointer swap
     if (newton_iters) *newton_iters = k;

@@ -91,8 +91,10 @@ template <int NST, int RS, bool CH = false>
 __global__ void __launch_bounds__(32)
 ybwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__ CUtensorMap mB,
                  const __grid_constant__ CUtensorMap mZ, int nx, int ny, int mid_arg, const double* __restrict__ al,
-                 const double* __restrict__ be, const double* __restrict__ zz, double* __restrict__ w, int P = 1)
+                 const double* __restrict__ be, const double* __restrict__ zz, double* __restrict__ w, int P = 1,
+                 Gate gate = Gate{nullptr, 0.0})
 {
+    if (gate_closed(gate)) return;
     extern __shared__ unsigned char raw[];
     unsigned char* base = align1024(raw);
     constexpr int BOX = RS * 32;                             // doubles per box
@@ -191,8 +193,9 @@ ybwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
 // Plain fallback of the same two-sided back substitution (any nx, ny; no TMA): lane <-> column, direct loads.
 __global__ void __launch_bounds__(32)
 ybwd2_plain_kernel(int nx, int ny, int mid, const double* __restrict__ al, const double* __restrict__ be,
-                   const double* __restrict__ zz, double* __restrict__ w)
+                   const double* __restrict__ zz, double* __restrict__ w, Gate gate)
 {
+    if (gate_closed(gate)) return;
     const int i = blockIdx.x * 32 + threadIdx.x;
     const int dir = blockIdx.y;
     if (i >= nx) return;
@@ -228,8 +231,10 @@ __global__ void __launch_bounds__(32)
 xbwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__ CUtensorMap mB,
                  const __grid_constant__ CUtensorMap mZ, const __grid_constant__ CUtensorMap mUin,
                  const __grid_constant__ CUtensorMap mUout, int nx, int ny, int mid_arg, const double* __restrict__ alT,
-                 const double* __restrict__ beT, const double* __restrict__ zzT, double* __restrict__ red, int P = 1)
+                 const double* __restrict__ beT, const double* __restrict__ zzT, double* __restrict__ red, int P = 1,
+                 Gate gate = Gate{nullptr, 0.0})
 {
+    if (gate_closed(gate)) return;
     constexpr int CS = 16;                                   // columns per stage (= one 128-byte swizzled row)
     constexpr int BOX = CS * 32;                             // doubles per coefficient box
     constexpr int STAGE = 4 * BOX * 8;                       // bytes per stage: 3 coefficient boxes + the u tile
@@ -337,8 +342,9 @@ xbwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
 // odd or tiny grids, not a fast path).  uk may alias unew.
 __global__ void __launch_bounds__(32)
 xbwd2_plain_kernel(int nx, int ny, int mid, const double* __restrict__ alT, const double* __restrict__ beT,
-                   const double* __restrict__ zzT, const double* uk, double* unew, double* __restrict__ red)
+                   const double* __restrict__ zzT, const double* uk, double* unew, double* __restrict__ red, Gate gate)
 {
+    if (gate_closed(gate)) return;
     const int lane = threadIdx.x;
     const int j = blockIdx.x * 32 + lane;
     const int dir = blockIdx.y;

@@ -218,6 +218,18 @@ __device__ __forceinline__ void st3_if(int p, double* a0, double v0, double* a1,
 // few tiles from now into L2, so that their register loads one tile ahead see L2 latency, not HBM latency.
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
+// Speculative launch-ahead (S8): the host enqueues iteration k+1 before it has read the residual of iteration k.
+// Every kernel of iteration k+1 first looks at iteration k's record {res, bad} (final: the writing kernel has
+// completed in stream order) and returns at once if that iteration already converged (res < tol), produced a bad
+// iterate, or a NaN -- so the iterate of the deciding iteration is left untouched.  p == nullptr: no gate.
+struct Gate { const double* p; double tol; };
+__device__ __forceinline__ bool gate_closed(const Gate& g)
+{
+    if (g.p == nullptr) return false;
+    const double r = __ldcg(g.p), b = __ldcg(g.p + 1);
+    return !(r >= g.tol) || b != 0.0;
+}
+
 // warp index as a value the compiler knows to be warp-uniform (role branches then do not look divergent)
 __device__ __forceinline__ int uniform_warp_idx() { return __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0); }
 

@@ -96,8 +96,9 @@ template <int N, int M, bool FIRST, int NP, int RP, int NCH, int NSUB>
 __global__ void __launch_bounds__(32 * NSUB * (NP + 1), 1)
 yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ CUtensorMap mB, int use_tma,
                Params P, Dir DX, Dir DY, int mid, const double* __restrict__ u, double* __restrict__ bn,
-               double* __restrict__ al, double* __restrict__ be, double* __restrict__ zz)
+               double* __restrict__ al, double* __restrict__ be, double* __restrict__ zz, Gate gate)
 {
+    if (gate_closed(gate)) return;
     // One CTA per SM: NSUB = 4 sub-problems q = warp % 4 (two adjacent strips x two halves), each with its own
     // ring and its own consumer + NP producers.  Warps w, w+4, w+8, ... share an SM sub-partition, so every
     // sub-partition gets exactly one consumer and NP producers (the consumers' dependent chains and the
@@ -309,8 +310,9 @@ constexpr int XW_LD = 29;            // slot row pitch in doubles (odd)
 template <int N, int M, int NP, int NCH, int NSUB>
 __global__ void __launch_bounds__(32 * NSUB * (NP + 1), 1)
 xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const double* __restrict__ w,
-               double* __restrict__ alT, double* __restrict__ beT, double* __restrict__ zzT)
+               double* __restrict__ alT, double* __restrict__ beT, double* __restrict__ zzT, Gate gate)
 {
+    if (gate_closed(gate)) return;
     constexpr int SV = XW_CK * XW_LD;                 // doubles per value plane of a slot
     constexpr size_t RING = (size_t)NCH * 5 * SV * 8 + 16 * NCH;
     constexpr int NRMAX = (XW_R + NP - 1) / NP;       // rows per producer

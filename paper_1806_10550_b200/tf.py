@@ -31,6 +31,7 @@ SYMBOLS = {
     "tf_destroy": (None, [_vp]),
     "tf_set_newton": (ctypes.c_int, [_vp, ctypes.c_double, ctypes.c_int, ctypes.c_int]),
     "tf_set_pressure": (ctypes.c_int, [_vp, ctypes.c_int, _dp, ctypes.c_int]),
+    "tf_set_launch_ahead": (ctypes.c_int, [_vp, ctypes.c_int]),
     "tf_set_state": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
     "tf_get_state": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
     "tf_step": (ctypes.c_int, [_vp, ctypes.c_double, ctypes.POINTER(ctypes.c_int), _dp]),
@@ -117,6 +118,12 @@ class ThinFilm:
         st = lib().tf_set_newton(self._h, tol, max_iter, fixed_iters)
         if st != OK:
             _err(self._h, st, "tf_set_newton")
+
+    def set_launch_ahead(self, batch):
+        """tf_set_launch_ahead: 0 = host decision after every iteration, > 0 = speculative batches (default 2)."""
+        st = lib().tf_set_launch_ahead(self._h, int(batch))
+        if st != OK:
+            _err(self._h, st, "tf_set_launch_ahead")
 
     def set_pressure(self, kind, params=()):
         """tf_set_pressure: PI_POWER (), PI_NLC (cap0, cap1, K, b, N, beta, w), PI_POLYMER (cap0, cap1, C, A_SiOx, A_Si, d)."""

@@ -232,3 +232,29 @@ def test_penta_solve_parity(tf, tfo, nrow, ncol, direction):
     Ax[:, :-2] += b[:, :-2] * xs[:, 2:]
     normA = np.max(np.abs(e) + np.abs(c) + np.abs(d) + np.abs(a) + np.abs(b))
     assert np.max(np.abs(Ax - y)) / (normA * np.max(np.abs(xs)) + np.max(np.abs(y))) <= 1e-14
+
+
+# ------------------------------------------------------------------ S8: speculative launch-ahead == per-iteration decision
+@pytest.mark.parametrize("nx,ny", [(128, 128), (61, 45), (300, 168)])
+def test_launch_ahead_is_exactly_the_per_iteration_decision(tf, nx, ny):
+    """tf_set_launch_ahead(batch > 0) enqueues iterations past the deciding one; those must be no-ops on the device:
+    iteration counts, residuals and fields are bit-identical to batch = 0, for accepted and for rejected steps."""
+    h0 = inputs.noise_ic(nx, ny, seed=9)
+    runs = []
+    for batch in (0, 1, 2, 7):
+        g = tf.ThinFilm(nx, ny, 0.4259, 0.4259, K, HS, 3, 2)
+        g.set_launch_ahead(batch)
+        g.set_newton(tol=1e-10, max_iter=64)
+        g.set_state(h0)
+        log = [g.step(1e-2) for _ in range(6)]
+        g.set_newton(tol=1e-10, max_iter=3)            # too few iterations: every step is rejected, state must stay
+        before = g.get_state()
+        log += [g.step(1e-2) for _ in range(2)]
+        assert np.array_equal(before, g.get_state())
+        g.set_newton(tol=1e-10, max_iter=64)
+        log += [g.step(1e-2) for _ in range(2)]
+        runs.append((log, g.get_state()))
+    assert all(st == tf.OK for st, _, _ in runs[0][0][:6]) and all(st == tf.NOT_CONVERGED for st, _, _ in runs[0][0][6:8])
+    for log, h in runs[1:]:
+        assert log == runs[0][0]
+        assert np.array_equal(h, runs[0][1])
