@@ -33,6 +33,7 @@ typedef struct tf_ctx tf_ctx;   /* opaque */
 typedef enum {
     TF_OK = 0,
     TF_NOT_CONVERGED = 1,       /* soft: step rejected, state still u^n   */
+    TF_REJECTED = 2,            /* soft: converged, but an extra solution criterion failed (PAPER.md:252 Note 2); state still u^n */
     TF_ERR_INVALID_ARG = -1,
     TF_ERR_UNSUPPORTED = -2,
     TF_ERR_CUDA = -3,
@@ -110,6 +111,32 @@ tf_status tf_get_state(tf_ctx* ctx, double* h_out, int is_device_ptr);
  * (>= 1) and *residual (last res) are filled in both cases; either may be NULL.
  */
 tf_status tf_step(tf_ctx* ctx, double dt, int* newton_iters, double* residual);
+
+/*
+ * Extra "solution criteria" (PAPER.md:252 Note 2: "Other restrictions besides the convergence of the iterative scheme
+ * may be placed on accepting the solution ... e.g. sufficiently small truncation error").  The paper fixes none; this
+ * build offers one: a converged step is accepted only if  max_ij |u^{n+1} - u^n| / u^n  <= max_rel_change, else
+ * tf_step returns TF_REJECTED and the state stays u^n.  0 switches the criterion off (default).
+ */
+tf_status tf_set_solution_criteria(tf_ctx* ctx, double max_rel_change);
+
+/*
+ * Adaptive time stepping of Fig. 1: take a step of size dt; if the solution criteria are met
+ * (status TF_OK) advance time and, after `grow_after` consecutive accepted steps, multiply dt by `grow` (bounded by
+ * dt_max); otherwise multiply dt by `shrink` and retry; fail (TF_NOT_CONVERGED) when dt falls below dt_min or after
+ * max_attempts steps (<= 0: 50 * n_accept).  Runs until n_accept steps were accepted.  ctl->dt is the first step on
+ * entry and the step to continue with on return; *t_advanced = sum of the accepted steps; the first hist_cap attempts
+ * are recorded in hist, *nhist = number of attempts (all optional, may be NULL / 0).  A negative status of a step
+ * stops the run and is returned.  The paper gives no constants; BASELINE.json config 2 uses shrink 0.5, grow 1.1,
+ * grow_after 1.  tf_adaptive_run is the controller over any step function (tf_advance_adaptive = over tf_step).
+ */
+typedef struct { double dt, shrink, grow; int grow_after; double dt_min, dt_max; } tf_adaptive;
+typedef struct { double dt; int status; int newton_iters; double residual; } tf_step_record;
+typedef int (*tf_step_fn)(void* user, double dt, int* newton_iters, double* residual);   /* returns a tf_status */
+tf_status tf_adaptive_run(tf_step_fn step, void* user, tf_adaptive* ctl, int n_accept, int max_attempts,
+                          double* t_advanced, tf_step_record* hist, int hist_cap, int* nhist);
+tf_status tf_advance_adaptive(tf_ctx* ctx, tf_adaptive* ctl, int n_accept, int max_attempts,
+                              double* t_advanced, tf_step_record* hist, int hist_cap, int* nhist);
 
 /* mass = dx*dy*sum(h)  ((3.2), times the domain area); fixed-order fp64 tree. */
 tf_status tf_mass(tf_ctx* ctx, double* mass);

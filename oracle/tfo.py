@@ -165,3 +165,63 @@ def penta_solve(direction, e, c, d, a, b, rhs, omp=False):
 
 def num_threads(omp=False):
     return int(lib(omp).tfo_num_threads())
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Fig. 1, written out step by step.  "If the solution criteria are not met, then the time-step is
+# reduced and the pseudo-Newton iterative scheme is performed with the new reduced time step.  Furthermore, if the new
+# reduced time step is below some minimum, the numerical scheme halts and ends in a failed state. ... the time step is
+# increased if a minimum number of successful time steps have been consecutively computed. ... the time step is bounded
+# from above."  The paper gives no constants (R13); they are arguments.
+# ---------------------------------------------------------------------------------------------------------------
+REJECTED = 2
+
+
+def max_rel_change(u_old, u_new):
+    """The one extra solution criterion the build offers (PAPER.md:252 Note 2 leaves them open; R21):
+    max over the grid of |u^{n+1} - u^n| / u^n."""
+    return float(np.max(np.abs(np.asarray(u_new) - np.asarray(u_old)) / np.asarray(u_old)))
+
+
+class CriteriaStepper:
+    """step(dt) of a ThinFilmOracle with the extra criterion: a converged step whose max_rel_change exceeds
+    `limit` is undone (state back to u^n) and reported as REJECTED."""
+    def __init__(self, oracle, limit):
+        self.o, self.limit, self.last_change = oracle, limit, None
+
+    def step(self, dt):
+        before = self.o.get_state()
+        st, it, res = self.o.step(dt)
+        if st == OK and self.limit > 0:
+            self.last_change = max_rel_change(before, self.o.get_state())
+            if not (self.last_change <= self.limit):
+                self.o.set_state(before)
+                st = REJECTED
+        return st, it, res
+
+
+def advance_adaptive(stepper, dt, n_accept, grow, shrink, dt_max, dt_min, grow_after=1, max_attempts=None):
+    """Flow chart of Fig. 1 over any object with step(dt) -> (status, iters, residual).  Returns
+    (t, dt_next, history, failed) with history = [(dt, status, iters, residual), ...]."""
+    t, hist, accepted, streak, attempts = 0.0, [], 0, 0, 0
+    dt = min(dt, dt_max)                                  # "bounded from above"
+    max_attempts = max_attempts or 50 * max(n_accept, 1)
+    while accepted < n_accept:
+        if attempts >= max_attempts:
+            return t, dt, hist, True
+        attempts += 1
+        st, it, res = stepper.step(dt)
+        hist.append((dt, st, it, res))
+        if st == OK:                                      # solution criteria met: accept
+            accepted += 1
+            t += dt
+            streak += 1
+            if streak >= grow_after:                      # "a minimum number of successful time steps ... consecutively"
+                dt = min(dt * grow, dt_max)
+                streak = 0
+        else:                                             # not met: reduce the time step and redo
+            streak = 0
+            dt = dt * shrink
+            if dt < dt_min:                               # "halts and ends in a failed state"
+                return t, dt, hist, True
+    return t, dt, hist, False

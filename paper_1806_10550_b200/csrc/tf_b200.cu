@@ -47,6 +47,8 @@ struct tf_ctx {
     double *scal;                              // [8] : scal[0] mass, (int*)(scal+1) flag
     double *pinned;                            // [4] host pinned readback
     double *pinned_red;                        // [2*MAX_ITERS] host pinned copy of the residual records
+    double last_change;                        // max |u^{n+1} - u^n| / u^n of the last converged step (criterion on)
+    double max_rel_change;                     // extra solution criterion (0 = off): reject a converged step that changed h by more
     int spec_batch, last_iters;                // speculative launch-ahead: batch size (0 = off), iterations of the last accepted step
     int mid_y, mid_x;                          // split rows / columns of the two-sided sweeps
     int num_sms;
@@ -394,6 +396,7 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
     }
     c->pinned_red = c->pinned + 4;
     c->spec_batch = 2; c->last_iters = 1;
+    c->max_rel_change = 0.0;
     c->ubuf[0] = c->u; c->ubuf[1] = c->uk;
     {
         int dev = 0, sms = 148;
@@ -558,6 +561,63 @@ tf_status tf_set_newton(tf_ctx* c, double tol, int max_iter, int fixed_iters)
     return TF_OK;
 }
 
+tf_status tf_set_solution_criteria(tf_ctx* c, double max_rel_change)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    if (!(max_rel_change >= 0.0) || !std::isfinite(max_rel_change))
+        return fail(c, TF_ERR_INVALID_ARG, "max_rel_change must be >= 0 and finite (0 = off)");
+    c->max_rel_change = max_rel_change;
+    return TF_OK;
+}
+
+tf_status tf_adaptive_run(tf_step_fn step, void* user, tf_adaptive* ctl, int n_accept, int max_attempts, double* t_advanced,
+                          tf_step_record* hist, int hist_cap, int* nhist)
+{
+    if (!step || !ctl || n_accept < 0 || hist_cap < 0 || (hist_cap > 0 && !hist))
+        return fail(nullptr, TF_ERR_INVALID_ARG, "tf_adaptive_run: NULL step/ctl or negative count");
+    if (!(ctl->dt > 0) || !(ctl->shrink > 0 && ctl->shrink < 1) || !(ctl->grow >= 1) || ctl->grow_after < 1 ||
+        !(ctl->dt_min > 0) || !(ctl->dt_max >= ctl->dt_min) || !std::isfinite(ctl->dt) || !std::isfinite(ctl->grow) ||
+        !std::isfinite(ctl->dt_max))
+        return fail(nullptr, TF_ERR_INVALID_ARG, "tf_adaptive_run: need dt > 0, 0 < shrink < 1, grow >= 1, grow_after >= 1, 0 < dt_min <= dt_max");
+    if (max_attempts <= 0) max_attempts = 50 * std::max(n_accept, 1);
+    double t = 0.0, dt = std::min(ctl->dt, ctl->dt_max);
+    int accepted = 0, attempts = 0, streak = 0, nh = 0;
+    tf_status out = TF_OK;
+    while (accepted < n_accept) {
+        if (attempts++ >= max_attempts) { out = TF_NOT_CONVERGED; fail(nullptr, out, "tf_adaptive_run: too many attempts"); break; }
+        int it = 0;
+        double res = 0.0;
+        const int st = step(user, dt, &it, &res);
+        if (nh < hist_cap) { hist[nh].dt = dt; hist[nh].status = st; hist[nh].newton_iters = it; hist[nh].residual = res; }
+        ++nh;
+        if (st < 0) { out = (tf_status)st; break; }                    // hard error of the step: stop, report it
+        if (st == TF_OK) {
+            ++accepted;
+            t += dt;
+            if (++streak >= ctl->grow_after) { dt = std::min(dt * ctl->grow, ctl->dt_max); streak = 0; }
+        } else {                                                         // solution criteria not met: reduce the step
+            streak = 0;
+            dt *= ctl->shrink;
+            if (dt < ctl->dt_min) { out = TF_NOT_CONVERGED; fail(nullptr, out, "tf_adaptive_run: dt fell below dt_min"); break; }
+        }
+    }
+    ctl->dt = dt;
+    if (t_advanced) *t_advanced = t;
+    if (nhist) *nhist = nh;
+    return out;
+}
+
+static int step_of_ctx(void* user, double dt, int* it, double* res) { return (int)tf_step((tf_ctx*)user, dt, it, res); }
+
+tf_status tf_advance_adaptive(tf_ctx* c, tf_adaptive* ctl, int n_accept, int max_attempts, double* t_advanced,
+                              tf_step_record* hist, int hist_cap, int* nhist)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    tf_status st = tf_adaptive_run(step_of_ctx, c, ctl, n_accept, max_attempts, t_advanced, hist, hist_cap, nhist);
+    if (st != TF_OK && c->err.empty()) c->err = g_err;
+    return st;
+}
+
 tf_status tf_set_launch_ahead(tf_ctx* c, int batch)
 {
     if (!c) return TF_ERR_INVALID_ARG;
@@ -677,6 +737,18 @@ tf_status tf_step(tf_ctx* c, double dt, int* newton_iters, double* residual)
             batch = std::max(1, c->spec_batch);
         }
         if (status == TF_OK) c->last_iters = k;
+    }
+    if (status == TF_OK && c->max_rel_change > 0.0) {
+        // "solution criteria" beyond convergence (PAPER.md:252 Note 2): here the largest relative change of h
+        const size_t n = (size_t)c->P.nx * c->P.ny;
+        TF_CUDA(c, cudaMemsetAsync(c->scal + 2, 0, sizeof(double), c->stream));
+        max_rel_change_kernel<<<RED_BLOCKS, RED_THREADS, 0, c->stream>>>(n, c->u, c->uk, c->scal + 2);
+        count_launch(1);
+        TF_CUDA(c, cudaGetLastError());
+        TF_CUDA(c, cudaMemcpyAsync(c->pinned, c->scal + 2, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        TF_CUDA(c, cudaStreamSynchronize(c->stream));
+        c->last_change = c->pinned[0];
+        if (!(c->last_change <= c->max_rel_change)) status = TF_REJECTED;
     }
     if (status == TF_OK) std::swap(c->u, c->uk);     // pointer swap
     if (newton_iters) *newton_iters = k;

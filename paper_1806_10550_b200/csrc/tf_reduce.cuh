@@ -37,6 +37,21 @@ sum_check_kernel(size_t n, const double* __restrict__ h, double* __restrict__ pa
     }
 }
 
+// extra solution criterion of Fig. 1 (PAPER.md:252 Note 2): out[0] = max |u_new - u_old| / u_old over the field
+// (order-independent max on the bit patterns of non-negative doubles -> bitwise reproducible; NaN surfaces)
+__global__ void __launch_bounds__(RED_THREADS)
+max_rel_change_kernel(size_t n, const double* __restrict__ u_old, const double* __restrict__ u_new, double* __restrict__ out)
+{
+    double acc = 0.0;
+    for (size_t p = (size_t)blockIdx.x * RED_THREADS + threadIdx.x; p < n; p += (size_t)RED_BLOCKS * RED_THREADS) {
+        const double o = u_old[p];
+        const double r = fabs(u_new[p] - o) / o;
+        acc = (r != r) ? __longlong_as_double(0x7ff8000000000000LL) : ((acc != acc) ? acc : fmax(acc, r));
+    }
+    acc = warp_max_nonneg(acc);
+    if ((threadIdx.x & 31) == 0) atomic_max_nonneg(out, acc);
+}
+
 __global__ void __launch_bounds__(1024)
 sum_final_kernel(const double* __restrict__ part, double scale, double* __restrict__ out)
 {

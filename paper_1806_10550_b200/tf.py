@@ -11,7 +11,7 @@ import numpy as np
 
 from . import build as _build
 
-OK, NOT_CONVERGED = 0, 1
+OK, NOT_CONVERGED, REJECTED = 0, 1, 2
 ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_ALLOC, ERR_STATE = -1, -2, -3, -4, -5
 BC_NOFLUX = 0
 PI_POWER, PI_NLC, PI_POLYMER = 0, 2, 3
@@ -32,6 +32,11 @@ SYMBOLS = {
     "tf_set_newton": (ctypes.c_int, [_vp, ctypes.c_double, ctypes.c_int, ctypes.c_int]),
     "tf_set_pressure": (ctypes.c_int, [_vp, ctypes.c_int, _dp, ctypes.c_int]),
     "tf_set_launch_ahead": (ctypes.c_int, [_vp, ctypes.c_int]),
+    "tf_set_solution_criteria": (ctypes.c_int, [_vp, ctypes.c_double]),
+    "tf_adaptive_run": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, ctypes.c_int, _dp, _vp, ctypes.c_int,
+                                       ctypes.POINTER(ctypes.c_int)]),
+    "tf_advance_adaptive": (ctypes.c_int, [_vp, _vp, ctypes.c_int, ctypes.c_int, _dp, _vp, ctypes.c_int,
+                                           ctypes.POINTER(ctypes.c_int)]),
     "tf_set_state": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
     "tf_get_state": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
     "tf_step": (ctypes.c_int, [_vp, ctypes.c_double, ctypes.POINTER(ctypes.c_int), _dp]),
@@ -125,6 +130,12 @@ class ThinFilm:
         if st != OK:
             _err(self._h, st, "tf_set_launch_ahead")
 
+    def set_solution_criteria(self, max_rel_change=0.0):
+        """tf_set_solution_criteria: accept a converged step only if max|u^{n+1}-u^n|/u^n <= max_rel_change (0 = off)."""
+        st = lib().tf_set_solution_criteria(self._h, float(max_rel_change))
+        if st != OK:
+            _err(self._h, st, "tf_set_solution_criteria")
+
     def set_pressure(self, kind, params=()):
         """tf_set_pressure: PI_POWER (), PI_NLC (cap0, cap1, K, b, N, beta, w), PI_POLYMER (cap0, cap1, C, A_SiOx, A_Si, d)."""
         arr = (ctypes.c_double * max(len(params), 1))(*[float(v) for v in params])
@@ -197,30 +208,45 @@ class ThinFilm:
         return h.data_ptr(), (1 if h.is_cuda else 0), h
 
 
-def advance_adaptive(ctx, dt, n_accept, grow=1.1, shrink=0.5, dt_max=0.1, dt_min=1e-12, max_attempts=None):
-    """The adaptive time-stepping controller of Fig. 1 around tf_step: a step whose Newton
-    iteration does not converge within max_iter is rejected by the library (state unchanged) and retried with
-    dt*shrink; after an accepted step dt grows by `grow`, bounded by dt_max.  The factors are
-    BASELINE.json config 2's (the paper gives none).  Host logic only (S8); every step runs in the kernels.
+class _Adaptive(ctypes.Structure):
+    _fields_ = [("dt", ctypes.c_double), ("shrink", ctypes.c_double), ("grow", ctypes.c_double),
+                ("grow_after", ctypes.c_int), ("dt_min", ctypes.c_double), ("dt_max", ctypes.c_double)]
+
+
+class _StepRecord(ctypes.Structure):
+    _fields_ = [("dt", ctypes.c_double), ("status", ctypes.c_int), ("newton_iters", ctypes.c_int),
+                ("residual", ctypes.c_double)]
+
+
+_STEP_FN = ctypes.CFUNCTYPE(ctypes.c_int, _vp, ctypes.c_double, ctypes.POINTER(ctypes.c_int), _dp)
+
+
+def advance_adaptive(ctx, dt, n_accept, grow=1.1, shrink=0.5, dt_max=0.1, dt_min=1e-12, max_attempts=None, grow_after=1):
+    """Adaptive time stepping of Fig. 1 until `n_accept` steps were accepted: tf_advance_adaptive
+    for a ThinFilm, tf_adaptive_run (the same controller, driven through a callback) for any object with a
+    step(dt) -> (status, newton_iters, residual) method.  The controller itself is in the library; this marshals.
     Returns (t, dt_next, history) with history = [(dt, status, newton_iters, residual), ...]."""
-    t, hist, accepted = 0.0, [], 0
-    attempts = 0
-    max_attempts = max_attempts or 50 * n_accept
-    while accepted < n_accept:
-        attempts += 1
-        if attempts > max_attempts:
-            raise TfError(NOT_CONVERGED, "advance_adaptive", "too many attempts")
-        st, it, res = ctx.step(dt)
-        hist.append((dt, st, it, res))
-        if st == OK:
-            accepted += 1
-            t += dt
-            dt = min(dt * grow, dt_max)
-        else:
-            dt *= shrink
-            if dt < dt_min:
-                raise TfError(NOT_CONVERGED, "advance_adaptive", f"dt fell below {dt_min}")
-    return t, dt, hist
+    L = lib()
+    ctl = _Adaptive(float(dt), float(shrink), float(grow), int(grow_after), float(dt_min), float(dt_max))
+    cap = int(max_attempts or 50 * max(n_accept, 1))
+    hist = (_StepRecord * cap)()
+    nh, t = ctypes.c_int(0), ctypes.c_double(0.0)
+    if isinstance(ctx, ThinFilm):
+        st = L.tf_advance_adaptive(ctx._h, ctypes.byref(ctl), n_accept, cap, ctypes.byref(t), hist, cap, ctypes.byref(nh))
+        handle = ctx._h
+    else:
+        def cb(_user, dt_, it_p, res_p):
+            s_, it_, res_ = ctx.step(dt_)
+            it_p[0], res_p[0] = int(it_), float(res_)
+            return int(s_)
+        fn = _STEP_FN(cb)
+        st = L.tf_adaptive_run(ctypes.cast(fn, _vp), None, ctypes.byref(ctl), n_accept, cap, ctypes.byref(t), hist, cap,
+                               ctypes.byref(nh))
+        handle = None
+    if st != OK:
+        _err(handle, st, "advance_adaptive")
+    out = [(hist[k].dt, hist[k].status, hist[k].newton_iters, hist[k].residual) for k in range(min(nh.value, cap))]
+    return t.value, ctl.dt, out
 
 
 PENTA_LU, PENTA_PARTITION = 0, 1

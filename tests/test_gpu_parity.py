@@ -258,3 +258,34 @@ def test_launch_ahead_is_exactly_the_per_iteration_decision(tf, nx, ny):
     for log, h in runs[1:]:
         assert log == runs[0][0]
         assert np.array_equal(h, runs[0][1])
+
+
+# ------------------------------------------------------------------ Fig. 1 with an extra solution criterion (Note 2)
+def test_solution_criterion_and_native_controller_against_the_flow_chart(tf, tfo):
+    """tf_set_solution_criteria + tf_advance_adaptive against the oracle's transcription of Fig. 1 with the same
+    criterion (max relative change of h per step): same accept / reject sequence (including TF_REJECTED), same time
+    steps, same fields.  The limit is set from the oracle so that the first attempts are rejected by the criterion."""
+    cfg = inputs.config(0)
+    nx, ny = 96, 80
+    h = inputs.noise_ic(nx, ny, seed=21)
+    g, o = pair(tf, tfo, nx, ny, cfg["dx"], cfg["dy"])
+    for s in (g, o):
+        s.set_newton(1e-10, 64, 0)
+        s.set_state(h)
+    assert o.step(1e-2)[0] == 0
+    limit = 0.3 * tfo.max_rel_change(h, o.get_state())
+    o.set_state(h)
+    g.set_solution_criteria(limit)
+    stepper = tfo.CriteriaStepper(o, limit)
+    t_o, dt_o, hist_o, failed = tfo.advance_adaptive(stepper, 1e-2, 12, grow=1.3, shrink=0.5, dt_max=0.05, dt_min=1e-9, grow_after=2)
+    t_g, dt_g, hist_g = tf.advance_adaptive(g, 1e-2, 12, grow=1.3, shrink=0.5, dt_max=0.05, dt_min=1e-9, grow_after=2)
+    assert not failed
+    assert [x[1] for x in hist_g] == [x[1] for x in hist_o]
+    assert tf.REJECTED in [x[1] for x in hist_g] and hist_g[0][1] == tf.REJECTED
+    assert [x[0] for x in hist_g] == [x[0] for x in hist_o] and (t_g, dt_g) == (t_o, dt_o)
+    assert [x[2] for x in hist_g] == [x[2] for x in hist_o]
+    assert rel_inf(g.get_state(), o.get_state()) <= 1e-9
+    # criterion off again: the same first step is accepted
+    g.set_solution_criteria(0.0)
+    g.set_state(h)
+    assert g.step(1e-2)[0] == tf.OK
