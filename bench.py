@@ -96,14 +96,14 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-NCU_SUMMARY = os.path.join("profiles", "r01_v5_ncu_full_summary.csv")
+NCU_SUMMARY = os.path.join("profiles", "r01_v6_ncu_full_summary.csv")
 NCU_KERNEL = {"y_forward": "yfwd_ws_kernel", "y_backward": "ybwd2_tma_kernel", "x_forward": "xfwd_ws_kernel",
               "x_backward_update": "xbwd2_tma_kernel"}
 
 
 def ncu_traffic(kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` at 8192^2, from the committed
-    ncu --set full summary (profiles/r01_v5_ncu.md names the command), or None."""
+    ncu --set full summary (profiles/r01_v6_ncu.md names the command), or None."""
     import csv
     p = os.path.join(ROOT, NCU_SUMMARY)
     try:
@@ -367,7 +367,8 @@ def run_penta(args, cfg):
                       "value": min(r["unknowns_per_s"] for r in res.values()), "steps": args.steps, "warmup": max(args.warmup, 3),
                       "dtype": "f64", "data": "synthetic (config 4 recipe drawn on the GPU)", "higher_is_better": True,
                       "config": {"workload": cfg["name"], "systems": nsys, "length": n, "variant": args.variant,
-                                 "l2": "256 MiB flush write between timed solves" if small else "inputs 6 x 2 GiB >> 126 MB L2"},
+                                 "l2": "512 MiB flush write between timed solves" if small else
+                                 f"inputs 6 x {nsys * n * 8 / 2**20:.0f} MiB >> 126 MB L2"},
                       "directions": res, "peak": peak, "peak_source": peak_src,
                       "gpu_launches": (4 if variant == tf.PENTA_PARTITION else 2) * 2 * args.steps}), flush=True)
 

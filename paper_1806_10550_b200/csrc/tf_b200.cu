@@ -493,7 +493,7 @@ tf_status penta_partition(int nrow, int ncol, int dir, int P, const double* e, c
             ready.mark();
         }
         penta_col_iface_kernel<PI_NST, PC_RS><<<g, 32, SMI, st>>>(M, nrow, ncol, P, iface);
-        penta_reduced_kernel<<<(unsigned)((nsys + 127) / 128), 128, 0, st>>>((int)nsys, P, iface, rc, X);
+        penta_reduced_kernel<<<(unsigned)((nsys + 31) / 32), 32, 0, st>>>((int)nsys, P, iface, rc, X);
         penta_col_fwd2_kernel<PC_NST, PC_RS><<<g, 32, SMF, st>>>(M, nrow, ncol, 0, al, be, zz, P, X);
         ybwd2_tma_kernel<YT_NST, YT_RS, true><<<g, 32, SMB, st>>>(mw[0], mw[1], mw[2], ncol, nrow, 0, al, be, zz, x, P);
     } else {
@@ -509,7 +509,7 @@ tf_status penta_partition(int nrow, int ncol, int dir, int P, const double* e, c
             ready.mark();
         }
         penta_row_iface_kernel<PJ_NST><<<g, 32, SMI, st>>>(M, nrow, ncol, P, iface);
-        penta_reduced_kernel<<<(unsigned)((nsys + 127) / 128), 128, 0, st>>>((int)nsys, P, iface, rc, X);
+        penta_reduced_kernel<<<(unsigned)((nsys + 31) / 32), 32, 0, st>>>((int)nsys, P, iface, rc, X);
         penta_row_fwd2_kernel<PR_NST><<<g, 32, SMF, st>>>(M, nrow, ncol, 0, al, be, zz, P, X);
         xbwd2_tma_kernel<XT_NST, false, true><<<g, 32, SMB, st>>>(mw[0], mw[1], mw[2], mx, mx, ncol, nrow, 0, al, be, zz, nullptr, P);
     }
