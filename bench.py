@@ -44,6 +44,7 @@ def parse():
     ap.add_argument("--nsys", type=int, default=0, help="config 4 only: number of systems (0: the config's 16384)")
     ap.add_argument("--variant", default="lu", choices=["lu", "partition"], help="config 4 only: tf_penta_solve_ex variant")
     ap.add_argument("--nparts", type=int, default=0, help="config 4 only: chunks per system of the partition variant (0: automatic)")
+    ap.add_argument("--cusparse", action="store_true", help="config 4 only: also time cuSPARSE's interleaved-batch routine (context)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -310,6 +311,61 @@ def run_b200(args, cfg):
         dist.destroy_process_group()
 
 
+# ----------------------------------------------------------------------------------------- vendor library, context only
+def cusparse_gpsv_interleaved(e, c, d, a, b, y, steps):
+    """cuSPARSE's interleaved-batch pentadiagonal solver (cusparseDgpsvInterleavedBatch, algo 0) on the column layout
+    ([len][nsys] = element i of system j at i*nsys + j, exactly its "interleaved" format).  Context for config 4
+    (SURVEY.md 8(d)): a library call, not part of the product path.  The routine overwrites its inputs, so every timed
+    call gets fresh copies made outside the timed region.  Returns (mean ms, solution of the last call) or None."""
+    import ctypes
+    import glob
+    import torch
+    libs = glob.glob(os.path.join(os.path.dirname(torch.__file__), "..", "nvidia", "cusparse", "lib", "libcusparse.so*")) + \
+        glob.glob("/usr/local/cuda/lib64/libcusparse.so*")
+    if not libs:
+        return None
+    L = ctypes.CDLL(libs[0])
+    vp, ci = ctypes.c_void_p, ctypes.c_int
+    L.cusparseCreate.argtypes = [ctypes.POINTER(vp)]
+    L.cusparseSetStream.argtypes = [vp, vp]
+    L.cusparseDgpsvInterleavedBatch_bufferSizeExt.argtypes = [vp, ci, ci] + [vp] * 6 + [ci, ctypes.POINTER(ctypes.c_size_t)]
+    L.cusparseDgpsvInterleavedBatch.argtypes = [vp, ci, ci] + [vp] * 6 + [ci, vp]
+    L.cusparseDestroy.argtypes = [vp]
+    h = vp()
+    if L.cusparseCreate(ctypes.byref(h)) != 0:
+        return None
+    L.cusparseSetStream(h, vp(torch.cuda.current_stream().cuda_stream))
+    m, nsys = e.shape
+
+    def fresh():
+        ts = [t.clone() for t in (e, c, d, a, b, y)]
+        ts[0][:2] = 0.0; ts[1][:1] = 0.0; ts[3][-1:] = 0.0; ts[4][-2:] = 0.0     # the routine wants the outside entries zero
+        return ts
+    ts = fresh()
+    size = ctypes.c_size_t(0)
+    if L.cusparseDgpsvInterleavedBatch_bufferSizeExt(h, 0, m, *[t.data_ptr() for t in ts], nsys, ctypes.byref(size)) != 0:
+        L.cusparseDestroy(h)
+        return None
+    buf = torch.empty(max(size.value, 8), dtype=torch.uint8, device="cuda")
+    total, x = 0.0, None
+    for k in range(steps + 1):                      # first call untimed
+        if k:
+            ts = fresh()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        rc = L.cusparseDgpsvInterleavedBatch(h, 0, m, *[t.data_ptr() for t in ts], nsys, buf.data_ptr())
+        ev1.record()
+        torch.cuda.synchronize()
+        if rc != 0:
+            L.cusparseDestroy(h)
+            return None
+        if k:
+            total += ev0.elapsed_time(ev1)
+        x = ts[5]
+    L.cusparseDestroy(h)
+    return total / steps, x
+
+
 # ----------------------------------------------------------------------------------------- config 4 (side measurement)
 def run_penta(args, cfg):
     """Isolated batched pentadiagonal solve (BASELINE.json config 4), both directions, device-resident inputs of
@@ -362,6 +418,17 @@ def run_penta(args, cfg):
         bpu = 104 if chunks == 1 else 200          # partition: 2 x 48 B interface pass + 104 B chunk solves
         res[name] = {"ms": ms, "chunks": chunks, "unknowns_per_s": nsys * n / (ms * 1e-3), "alg_bytes_per_unknown": bpu,
                      "alg_gbs": bpu * nsys * n / (ms * 1e-3) / 1e9, "frac_of_peak": bpu * nsys * n / (ms * 1e-3) / 1e9 / peak}
+        if args.cusparse and direction == 1:
+            lib_run = cusparse_gpsv_interleaved(e, c, d, a, b, y, min(args.steps, 5))
+            if lib_run is None:
+                res[name]["cusparse_gpsvInterleavedBatch"] = "unavailable"
+            else:
+                solve()
+                torch.cuda.synchronize()
+                res[name]["cusparse_gpsvInterleavedBatch"] = {
+                    "ms": lib_run[0], "unknowns_per_s": nsys * n / (lib_run[0] * 1e-3),
+                    "max_rel_diff_to_ours": float((lib_run[1] - out).abs().max() / out.abs().max()),
+                    "note": "vendor library, QR-based (algo 0), in-place; context only"}
         del e, c, a, b, y, d, ws, out
     print(json.dumps({"metric": "pentadiagonal unknowns/s (fp64), isolated solve", "unit": "unknowns/s", "n_gpus": 1,
                       "value": min(r["unknowns_per_s"] for r in res.values()), "steps": args.steps, "warmup": max(args.warmup, 3),

@@ -19,6 +19,7 @@
 #pragma once
 #include "tf_device.cuh"
 #include "tf_tma.cuh"
+#include "tf_async.cuh"
 
 namespace tf {
 
@@ -239,19 +240,30 @@ penta_reduced_kernel(int nsys, int P, const double* __restrict__ iface, double* 
     if (i >= nsys) return;
     const size_t n = (size_t)nsys;
     double hb0 = 0.0, hb1 = 0.0, cb00 = 0.0, cb01 = 0.0, cb10 = 0.0, cb11 = 0.0;
-    // the 20 interface values of chunk p+1 are fetched while chunk p is eliminated (the loop is a short dependent
-    // chain; without the prefetch every chunk paid a full memory latency: 48 us for 37 chunks, measured)
-    double v[2 * IF_VALS], vn[2 * IF_VALS];
+    // The loop is a short dependent chain (~0.1 us per chunk) fed by 20 loads per chunk: a cp.async ring keeps the
+    // values of the next RD chunks in flight (loading them where they are used cost a full memory latency per
+    // chunk: 48 us for 37 chunks; one chunk of register prefetch: 34 us).  Every thread copies and reads its own
+    // slots, so cp.async.wait_group is the only synchronisation.
+    constexpr int RD = 8;
+    __shared__ double ring[RD][2 * IF_VALS][32];
+    const int lane = threadIdx.x;
+    auto fetch = [&](int q) {
+        if (q < P) {
+            const double* src = iface + (size_t)q * 2 * IF_VALS * n + i;
 #pragma unroll
-    for (int k = 0; k < 2 * IF_VALS; ++k) vn[k] = iface[(size_t)k * n + i];
-    for (int p = 0; p < P; ++p) {
-#pragma unroll
-        for (int k = 0; k < 2 * IF_VALS; ++k) v[k] = vn[k];
-        if (p + 1 < P) {
-            const double* nx = iface + (size_t)(p + 1) * 2 * IF_VALS * n + i;
-#pragma unroll
-            for (int k = 0; k < 2 * IF_VALS; ++k) vn[k] = nx[(size_t)k * n];
+            for (int k = 0; k < 2 * IF_VALS; ++k) cp_async8(&ring[q % RD][k][lane], src + (size_t)k * n);
         }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (int q = 0; q < RD; ++q) fetch(q);
+    double v[2 * IF_VALS];
+    for (int p = 0; p < P; ++p) {
+        cp_async_wait<RD - 1>();
+#pragma unroll
+        for (int k = 0; k < 2 * IF_VALS; ++k) v[k] = ring[p % RD][k][lane];
+        __syncwarp();
+        fetch(p + RD);
         // downward march: row hi-1 (0..4), hi-2 (5..9); upward march: row lo (10..14), lo+1 (15..19)
         const double d1a = v[0], d1b = v[1], d1y = v[2], d1f = v[3], d1n = v[4];
         const double d2a = v[5], d2b = v[6], d2y = v[7], d2f = v[8], d2n = v[9];
@@ -290,16 +302,25 @@ penta_reduced_kernel(int nsys, int P, const double* __restrict__ iface, double* 
         R[6 * n] = hb0; R[7 * n] = hb1; R[8 * n] = cb00; R[9 * n] = cb01; R[10 * n] = cb10; R[11 * n] = cb11;
     }
     double t0 = 0.0, t1 = 0.0;                                // t_{p+1}
-    double w[RC_VALS], wn[RC_VALS];
+    cp_async_wait<0>();
+    auto fetch_rc = [&](int q) {                                // q-th chunk from the end
+        if (q < P) {
+            const double* src = rc + (size_t)(P - 1 - q) * RC_VALS * n + i;
 #pragma unroll
-    for (int k = 0; k < RC_VALS; ++k) wn[k] = rc[((size_t)(P - 1) * RC_VALS + k) * n + i];
-    for (int p = P - 1; p >= 0; --p) {
-#pragma unroll
-        for (int k = 0; k < RC_VALS; ++k) w[k] = wn[k];
-        if (p > 0) {
-#pragma unroll
-            for (int k = 0; k < RC_VALS; ++k) wn[k] = rc[((size_t)(p - 1) * RC_VALS + k) * n + i];
+            for (int k = 0; k < RC_VALS; ++k) cp_async8(&ring[q % RD][k][lane], src + (size_t)k * n);
         }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (int q = 0; q < RD; ++q) fetch_rc(q);
+    double w[RC_VALS];
+    for (int p = P - 1; p >= 0; --p) {
+        const int q = P - 1 - p;
+        cp_async_wait<RD - 1>();
+#pragma unroll
+        for (int k = 0; k < RC_VALS; ++k) w[k] = ring[q % RD][k][lane];
+        __syncwarp();
+        fetch_rc(q + RD);
         const double nt0 = w[0] - (w[2] * t0 + w[3] * t1), nt1 = w[1] - (w[4] * t0 + w[5] * t1);
         const double b0 = w[6] - (w[8] * t0 + w[9] * t1), b1 = w[7] - (w[10] * t0 + w[11] * t1);
         double* x = X + (size_t)p * 4 * n + i;
