@@ -180,6 +180,20 @@ tf_status tf_penta_solve_ex(int nrow, int ncol, int dir, int variant, int nparts
                             const double* a, const double* b, const double* rhs, double* x,
                             void* dev_ws, void* cuda_stream);
 
+/*
+ * Betti numbers of the thresholded film ("b0 counts the number of mountain peaks
+ * (components) above H*, and b1 counts the number of valleys (loops) surrounding the peaks"; the paper uses CHomP on
+ * cubical sets).  For every threshold H* = thresholds[t] (host array), with X = the closed unit squares of the cells
+ * with h > H*:  b0[t] = connected components of X (cells connect through edges and corners), b1[t] = holes of X =
+ * components of the complement (cells connect through edges only) that do not reach the border of the image.
+ * h: DEVICE pointer, nx*ny doubles, row-major; b0, b1: HOST arrays of nthr entries; dev_ws: device scratch of
+ * tf_betti_workspace_bytes(nx, ny, nthr) bytes (256-byte aligned).  nx*ny < 2^31, ny <= 65535.  Synchronises the
+ * stream before returning (the counts are read back).  One union-find labelling per threshold, exact integers.
+ */
+size_t    tf_betti_workspace_bytes(int nx, int ny, int nthr);
+tf_status tf_betti(const double* h, int nx, int ny, const double* thresholds, int nthr,
+                   long long* b0, long long* b1, void* dev_ws, void* cuda_stream);
+
 /* Text of the last error on this context ("" if none); ctx == NULL: last error of a failed
  * tf_create* / tf_penta_solve on this thread.  Valid until the next call. */
 const char* tf_last_error(const tf_ctx* ctx);

@@ -6,6 +6,7 @@
 #include "tf_penta.cuh"
 #include "tf_bwd.cuh"
 #include "tf_fwd.cuh"
+#include "tf_topo.cuh"
 
 #include <algorithm>
 #include <atomic>
@@ -14,6 +15,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 namespace {
 
@@ -910,6 +912,48 @@ tf_status tf_penta_solve_ex(int nrow, int ncol, int dir, int variant, int nparts
     count_launch(2);
     cudaError_t ee = cudaGetLastError();
     if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "tf_penta_solve launch");
+    return TF_OK;
+}
+
+size_t tf_betti_workspace_bytes(int nx, int ny, int nthr)
+{
+    if (nx < 1 || ny < 1 || nthr < 1) return 0;
+    const size_t n = (size_t)nx * ny;
+    return align_up(n * sizeof(int)) + align_up(n) + align_up(2 * sizeof(unsigned long long) * (size_t)nthr);
+}
+
+tf_status tf_betti(const double* h, int nx, int ny, const double* thresholds, int nthr, long long* b0, long long* b1,
+                   void* dev_ws, void* cuda_stream)
+{
+    if (nx < 1 || ny < 1 || nthr < 1) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_betti: bad shape or threshold count");
+    if ((long long)nx * ny >= (1LL << 31)) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_betti: nx*ny must be < 2^31 (32-bit labels)");
+    if (!h || !thresholds || !b0 || !b1 || !dev_ws) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_betti: NULL pointer");
+    for (int t = 0; t < nthr; ++t)
+        if (thresholds[t] != thresholds[t]) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_betti: NaN threshold");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n = (size_t)nx * ny;
+    int* L = (int*)dev_ws;
+    unsigned char* open = (unsigned char*)dev_ws + align_up(n * sizeof(int));
+    unsigned long long* cnt = (unsigned long long*)(open + align_up(n));
+    TF_CUDA(nullptr, cudaMemsetAsync(cnt, 0, 2 * sizeof(unsigned long long) * (size_t)nthr, st));
+    const dim3 g((unsigned)((nx + TOPO_THREADS - 1) / TOPO_THREADS), (unsigned)ny);
+    if (g.y > 65535u) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_betti: ny must be <= 65535");
+    const unsigned gb = (unsigned)((2 * (size_t)nx + 2 * (size_t)ny + TOPO_THREADS - 1) / TOPO_THREADS);
+    const unsigned gc = (unsigned)std::min<size_t>((n + TOPO_THREADS - 1) / TOPO_THREADS, (size_t)num_sms() * 16);
+    for (int t = 0; t < nthr; ++t) {
+        const double thr = thresholds[t];
+        TF_CUDA(nullptr, cudaMemsetAsync(open, 0, n, st));
+        topo_init_kernel<<<g, TOPO_THREADS, 0, st>>>(nx, h, thr, L);
+        topo_merge_kernel<<<g, TOPO_THREADS, 0, st>>>(nx, ny, h, thr, L);
+        topo_border_kernel<<<gb, TOPO_THREADS, 0, st>>>(nx, ny, h, thr, L, open);
+        topo_count_kernel<<<gc, TOPO_THREADS, 0, st>>>(n, h, thr, L, open, cnt + 2 * t);
+        count_launch(4);
+        TF_CUDA(nullptr, cudaGetLastError());
+    }
+    std::vector<unsigned long long> host(2 * (size_t)nthr);
+    TF_CUDA(nullptr, cudaMemcpyAsync(host.data(), cnt, host.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    TF_CUDA(nullptr, cudaStreamSynchronize(st));
+    for (int t = 0; t < nthr; ++t) { b0[t] = (long long)host[2 * t]; b1[t] = (long long)host[2 * t + 1]; }
     return TF_OK;
 }
 

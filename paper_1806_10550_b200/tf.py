@@ -44,6 +44,9 @@ SYMBOLS = {
     "tf_penta_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int, ctypes.c_int]),
     "tf_penta_solve": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int] + [_vp] * 9),
     "tf_penta_partition_chunks": (ctypes.c_int, [ctypes.c_int] * 4),
+    "tf_betti_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int] * 3),
+    "tf_betti": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _dp, ctypes.c_int, ctypes.POINTER(ctypes.c_longlong),
+                                ctypes.POINTER(ctypes.c_longlong), _vp, _vp]),
     "tf_penta_workspace_bytes_ex": (ctypes.c_size_t, [ctypes.c_int] * 5),
     "tf_penta_solve_ex": (ctypes.c_int, [ctypes.c_int] * 5 + [_vp] * 9),
     "tf_set_profiling": (ctypes.c_int, [_vp, ctypes.c_int]),
@@ -282,3 +285,28 @@ def penta_solve(direction, e, c, d, a, b, rhs, out=None, workspace=None, stream=
     if rc != OK:
         _err(None, rc, "tf_penta_solve_ex")
     return out
+
+
+def betti(h, thresholds, workspace=None, stream=None):
+    """tf_betti on a contiguous CUDA float64 [ny][nx] tensor: (b0, b1) int64 numpy arrays, one entry per threshold
+    (superlevel sets {h > H*}: components, and holes that do not reach the border)."""
+    torch = _torch()
+    if not (isinstance(h, torch.Tensor) and h.is_cuda and h.dtype == torch.float64 and h.is_contiguous() and h.dim() == 2):
+        raise ValueError("expected a contiguous CUDA float64 [ny][nx] tensor")
+    ny, nx = h.shape
+    thr = np.ascontiguousarray(np.atleast_1d(thresholds), dtype=np.float64)
+    L = lib()
+    need = L.tf_betti_workspace_bytes(nx, ny, len(thr))
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=h.device)
+    if workspace.numel() * workspace.element_size() < need or workspace.data_ptr() % 256:
+        raise ValueError("workspace too small or not 256-byte aligned")
+    b0 = np.zeros(len(thr), dtype=np.int64)
+    b1 = np.zeros(len(thr), dtype=np.int64)
+    lp = ctypes.POINTER(ctypes.c_longlong)
+    st = (torch.cuda.current_stream(h.device) if stream is None else stream).cuda_stream
+    rc = L.tf_betti(h.data_ptr(), nx, ny, thr.ctypes.data_as(_dp), len(thr), b0.ctypes.data_as(lp), b1.ctypes.data_as(lp),
+                    workspace.data_ptr(), st)
+    if rc != OK:
+        _err(None, rc, "tf_betti")
+    return b0, b1
