@@ -236,7 +236,13 @@ constexpr int PC_NST = 3, PC_RS = 8;      // isolated solver, columns: 3 stages 
 constexpr int PR_NST = 2;                 // isolated solver, rows: 2 stages x 6 arrays x 4 KiB = 48 KiB per warp
 constexpr int YW_NP = 3, YW_RP = 8, YW_NSTG = 4;   // yfwd: consumer warp 0 + 3 producer warps, chunks of 8 rows, ring of 4 chunk slots (40 KiB)
 
-constexpr int XW_NP = 4, XW_NSTG = 3;              // xfwd: per sub-problem 1 consumer + 4 producer warps, ring of 3 slots of 14 columns (48 KiB)
+#ifndef TF_XW_NP
+#define TF_XW_NP 4
+#endif
+#ifndef TF_XW_NSTG
+#define TF_XW_NSTG 3
+#endif
+constexpr int XW_NP = TF_XW_NP, XW_NSTG = TF_XW_NSTG;              // xfwd: per sub-problem 1 consumer + 4 producer warps, ring of 3 slots of 14 columns x 4 planes (38 KiB; 4 slots = two tiles were measured slower: 0.67 vs 0.53 ms -- the producers' unaligned row loads live on the L1 the carve-out leaves)
 
 // forward kernels: NSUB sub-problems per CTA (4: two strips/blocks x two halves; 2: one x two halves)
 template <int N, int M, bool FIRST, int NSUB>
@@ -259,7 +265,7 @@ cudaError_t launch_yfwd(tf_ctx* c, const CUtensorMap& mu, int tma, const Params&
 template <int N, int M, int NSUB>
 cudaError_t launch_xfwd(tf_ctx* c, const Params& P, const Dir& DX, const double* src, int grid, Gate gate)
 {
-    constexpr size_t SM = NSUB * ((size_t)XW_NSTG * 5 * XW_CK * XW_LD * 8 + 16 * XW_NSTG);
+    constexpr size_t SM = NSUB * ((size_t)XW_NSTG * 4 * XW_CK * XW_LD * 8 + 16 * XW_NSTG);
     auto kern = xfwd_ws_kernel<N, M, XW_NP, XW_NSTG, NSUB>;
     static DevOnce ready;
     if (!ready.done()) {

@@ -19,6 +19,9 @@
 
 namespace tf {
 
+#ifndef TF_ROTATE_Y
+#define TF_ROTATE_Y 1
+#endif
 constexpr int YW_VALID = 28;     // columns per strip (lanes 2..29; lanes 0,1,30,31 are x-halo)
 
 // rolling state of a thread marching down a column
@@ -114,7 +117,11 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
     extern __shared__ __align__(128) unsigned char raw[];
     const int nx = P.nx, ny = P.ny;
     const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
-    const int q = warp % NSUB, role = warp / NSUB;    // role 0: consumer, 1..NP: producers
+    // role 0: consumer, 1..NP: producers.  Warp w runs on SM sub-partition w % 4: consumer q sits on sub-partition q,
+    // its producers (TF_ROTATE_Y) on the sub-partitions after it, so that a team's assembly burst uses several fp64
+    // pipes while the other teams' consumers (dependent chains, mostly idle issue slots) share them
+    const int role = warp / NSUB;
+    const int q = TF_ROTATE_Y ? (warp % NSUB + NSUB * NP - role) % NSUB : warp % NSUB;
     double* sm = reinterpret_cast<double*>(raw + q * RING);          // [NCH][5][RP][32]
     uint64_t* bars = reinterpret_cast<uint64_t*>(raw + NSUB * RING + NSUB * NP * STG);
     uint64_t* full = bars + q * 2 * NCH;
@@ -294,13 +301,31 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
 // descending; see yfwd_ws_kernel for the two-sided scheme).  Per sub-problem: one consumer warp (lane <->
 // row of the block, marches along the lines) and NP producer warps.  Producers work with lanes ALONG the
 // lines (lane <-> column, coalesced loads, x-neighbours by shuffle; only x-neighbours are needed,
-// PAPER.md:748) on tiles of 28 columns, split rows r = pw, pw+NP, ... between them, and write the bands
-// transposed into two ring slots of XW_CK = 14 columns each ([plane][column][XW_LD]: conflict-free for the
-// producers' half-warps and for the consumer).  Coefficients go out transposed ([i][j]) so the consumer's
-// stores are coalesced too.
+// PAPER.md:748) on tiles of 28 columns, split rows r = pw, pw+NP, ... between them, and write, transposed,
+// into two ring slots of XW_CK = 14 columns each ([plane][column][XW_LD]: conflict-free for the producers'
+// half-warps and for the consumer).  Coefficients go out transposed ([i][j]) so the consumer's stores are coalesced.
+//
+// What the ring carries: per column the scaled partials (A, p1, p2) of the FORWARD face in marching order (the face
+// towards the next column the consumer will eliminate) and the right-hand side w -- 4 planes.  The consumer keeps the
+// previous column's face in registers and forms the bands c = -(A + p1'), q = (1 + p1) - p2', a = p2 - A' itself
+// (primes: backward face).  Storing faces instead of finished bands (5 planes) saves the producers six shuffles and
+// four additions per row and a fifth of the ring (x forward 0.58 -> 0.52 ms at 8192^2).  Ring depth: three slots
+// (1.5 tiles).  Four slots (two whole tiles, which the smaller planes would allow) remove the waiting of producers and
+// consumer for each other but were measured SLOWER (0.67 ms): the producers' row loads are unaligned 256-byte
+// segments that overlap between neighbouring tiles and live on the L1 cache, and 208 KB of shared memory leave too
+// little of it (two slots, 104 KB: 0.53 ms).  The next tile's rows are therefore prefetched into L1 while the current
+// one is assembled (TF_XW_PREFETCH: 0.52 -> 0.50 ms; the first use of a tile's loads had 12 % of all stall samples).
+// For half 1 (descending columns) lane i-1 writes its face i-1/2 into column i's position with p1, p2 swapped and
+// negated, which is the same formula in the reversed system.
 // ---------------------------------------------------------------------------------------------
 #ifndef XW_RECOMPUTE_C1
 #define XW_RECOMPUTE_C1 1
+#endif
+#ifndef TF_XW_PREFETCH
+#define TF_XW_PREFETCH 1
+#endif
+#ifndef TF_ROTATE_X
+#define TF_ROTATE_X 1
 #endif
 constexpr int XW_CT = 28;            // columns per producer tile (32 lanes minus 2 halo lanes each side)
 constexpr int XW_CK = 14;            // columns per ring slot
@@ -314,15 +339,17 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
 {
     if (gate_closed(gate)) return;
     constexpr int SV = XW_CK * XW_LD;                 // doubles per value plane of a slot
-    constexpr size_t RING = (size_t)NCH * 5 * SV * 8 + 16 * NCH;
+    constexpr int NPL = 4;                            // planes per slot: A, p1, p2 of the forward face, right-hand side
+    constexpr size_t RING = (size_t)NCH * NPL * SV * 8 + 16 * NCH;
     constexpr int NRMAX = (XW_R + NP - 1) / NP;       // rows per producer
     extern __shared__ __align__(16) unsigned char raw[];
     const unsigned FULL = 0xffffffffu;
     const int nx = P.nx, ny = P.ny;
     const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
-    const int q = warp % NSUB, role = warp / NSUB;    // role 0: consumer, 1..NP: producers (NSUB: see yfwd_ws_kernel)
-    double* sm = reinterpret_cast<double*>(raw + q * RING);          // [NCH][5][CK][LD]
-    uint64_t* full = reinterpret_cast<uint64_t*>(raw + q * RING + (size_t)NCH * 5 * SV * 8);
+    const int role = warp / NSUB;                     // role 0: consumer, 1..NP: producers (NSUB, rotation: see yfwd_ws_kernel)
+    const int q = TF_ROTATE_X ? (warp % NSUB + NSUB * NP - role) % NSUB : warp % NSUB;
+    double* sm = reinterpret_cast<double*>(raw + q * RING);          // [NCH][NPL][CK][LD]
+    uint64_t* full = reinterpret_cast<uint64_t*>(raw + q * RING + (size_t)NCH * NPL * SV * 8);
     uint64_t* empty = full + NCH;
     if (role == 0 && lane == 0) {
 #pragma unroll
@@ -343,9 +370,10 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
         size_t rowoff[NRMAX];
 #pragma unroll
         for (int k = 0; k < NRMAX; ++k) rowoff[k] = (size_t)min(j0 + pw + k * NP, ny - 1) * nx;
-        // marching position k of lane's column within the tile: lane-2 (half 0), 29-lane (half 1)
-        const int kk = dir ? XW_CT + 1 - lane : lane - 2;
-        const bool lane_ok = (lane >= 2) && (lane < 2 + XW_CT);
+        // The lane of column i computes face i+1/2.  Half 0 stores it at its own column (marching position lane-2);
+        // half 1 stores it, as the forward face of column i+1, at marching position 29-(lane+1) = 28-lane.
+        const int kk = dir ? XW_CT - lane : lane - 2;
+        const bool lane_ok = (kk >= 0) && (kk < XW_CT);      // lanes 2..29 (half 0), 1..28 (half 1)
         const int slot_sel = lane_ok ? kk / XW_CK : 0;       // first or second slot of the tile
         const int kc = lane_ok ? kk % XW_CK : 0;             // column within the slot
         for (int t = 0; t < ntile; ++t) {
@@ -353,17 +381,29 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
             const int i = ilo - 2 + lane;
             const int ic = ghost(i, nx);
             const bool face_ok = (i >= 0) && (i <= nx - 2);
-            const bool col_ok = lane_ok && (i >= imin) && (i < imax);
+            const int idst = i + dir;                         // the column whose ring position this lane fills
+            const bool col_ok = lane_ok && (idst >= imin) && (idst < imax);
             double hq[NRMAX], wq[NRMAX];
 #pragma unroll
             for (int k = 0; k < NRMAX; ++k) {
                 hq[k] = u[rowoff[k] + ic];
-                wq[k] = col_ok ? w[rowoff[k] + i] : 0.0;
+                wq[k] = col_ok ? w[rowoff[k] + idst] : 0.0;
             }
+#if TF_XW_PREFETCH
+            if (t + 1 < ntile) {                              // pull the next tile's rows into L1 while this one is assembled
+                const int in = (dir ? ilo - XW_CT : ilo + XW_CT) - 2 + lane;
+                const int icn = ghost(in, nx), iwn = clampi(in + dir, 0, nx - 1);
+#pragma unroll
+                for (int k = 0; k < NRMAX; ++k) {
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(u + rowoff[k] + icn));
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(w + rowoff[k] + iwn));
+                }
+            }
+#endif
             const int g0 = 2 * t, g1 = 2 * t + 1;             // global slot numbers of this tile
             mbar_wait(empty + g0 % NCH, ((g0 / NCH) & 1) ^ 1);
             mbar_wait(empty + g1 % NCH, ((g1 / NCH) & 1) ^ 1);
-            double* st = sm + (size_t)((slot_sel ? g1 : g0) % NCH) * 5 * SV + kc * XW_LD;
+            double* st = sm + (size_t)((slot_sel ? g1 : g0) % NCH) * NPL * SV + kc * XW_LD;
             // one row of the tile; INTERIOR: every face of the tile is an interior, unfolded face and every
             // column belongs to this half -- no boundary selects (all tiles but the first, last and the split one)
             auto row = [&](auto interior_tag, int k) {
@@ -388,15 +428,11 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
                     if (i == nx - 2) fp.p2 += fp.A;
                     if (!face_ok) { fp.A = 0.0; fp.p1 = 0.0; fp.p2 = 0.0; }
                 }
-                Face fm;
-                fm.A = __shfl_up_sync(FULL, fp.A, 1); fm.p1 = __shfl_up_sync(FULL, fp.p1, 1);
-                fm.p2 = __shfl_up_sync(FULL, fp.p2, 1);
                 if (INTERIOR ? lane_ok : col_ok) {
-                    st[r] = dir ? fm.A : fp.A;
-                    st[SV + r] = -fp.A - fm.p1;
-                    st[2 * SV + r] = 1.0 + fp.p1 - fm.p2;
-                    st[3 * SV + r] = fp.p2 - fm.A;
-                    st[4 * SV + r] = wq[k];
+                    st[r] = fp.A;
+                    st[SV + r] = dir ? -fp.p2 : fp.p1;
+                    st[2 * SV + r] = dir ? -fp.p1 : fp.p2;
+                    st[3 * SV + r] = wq[k];
                 }
             };
             const bool interior = (ilo >= 3) && (ilo + XW_CT + 2 <= nx - 2) && (ilo >= imin) && (ilo + XW_CT <= imax);
@@ -417,44 +453,34 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
         const int j = j0 + lane;
         const int rowok = (lane < XW_R && j < ny) ? 1 : 0;
         Elim2 S = elim2_init();
-        double e = 0.0;
+        double Ba = 0.0, B1 = 0.0, B2 = 0.0;              // backward face: the boundary face before the first column carries nothing
         const int step = dir ? -ny : ny;
         int o = (dir ? nx : -1) * ny + j;                 // the column before the first one
-        const int offc = dir ? 3 * SV : SV, offa = dir ? SV : 3 * SV;
-        const int nslot = (ncols + XW_CK - 1) / XW_CK;
         const int lr = min(lane, XW_R - 1);               // lanes beyond the block read a valid row (results unused)
         for (int g = 0; g < 2 * ntile; ++g) {
             const int s = g % NCH;
             mbar_wait(full + s, (g / NCH) & 1);
-            const double* st = sm + (size_t)s * 5 * SV + lr;
-            const double* stc = st + offc;
-            const double* sta = st + offa;
+            const double* st = sm + (size_t)s * NPL * SV + lr;
             const int ncol = min(XW_CK, ncols - g * XW_CK);
+            // one column: bands from the forward face (ring) and the backward face (registers), then the recurrence
+            auto column = [&](int c, int pred) {
+                const double Fa = st[c * XW_LD], F1 = st[SV + c * XW_LD], F2 = st[2 * SV + c * XW_LD];
+                const double R = st[3 * SV + c * XW_LD];
+                const double cc = -(Fa + B1), qq = (1.0 + F1) - B2, a = F2 - Ba;
+                double va, vb, vz;
+                elim2_row(S, Ba, cc, qq, a, Fa, R, va, vb, vz);
+                Ba = Fa; B1 = F1; B2 = F2;
+                st3_if(pred, alT + o, va, beT + o, vb, zzT + o, vz);
+                o += step;
+            };
             if (ncol == XW_CK && g > 0) {
 #pragma unroll
-                for (int c = 0; c < XW_CK; ++c) {
-                    const double A = st[c * XW_LD], cc = stc[c * XW_LD], qq = st[2 * SV + c * XW_LD], a = sta[c * XW_LD];
-                    const double R = st[4 * SV + c * XW_LD];
-                    double va, vb, vz;
-                    elim2_row(S, e, cc, qq, a, A, R, va, vb, vz);
-                    e = A;
-                    st3_if(rowok, alT + o, va, beT + o, vb, zzT + o, vz);
-                    o += step;
-                }
+                for (int c = 0; c < XW_CK; ++c) column(c, rowok);
             } else {
-                for (int c = 0; c < ncol; ++c) {
-                    const double A = st[c * XW_LD], cc = stc[c * XW_LD], qq = st[2 * SV + c * XW_LD], a = sta[c * XW_LD];
-                    const double R = st[4 * SV + c * XW_LD];
-                    double va, vb, vz;
-                    elim2_row(S, e, cc, qq, a, A, R, va, vb, vz);
-                    e = A;
-                    st3_if(rowok && (g * XW_CK + c) > 0, alT + o, va, beT + o, vb, zzT + o, vz);
-                    o += step;
-                }
+                for (int c = 0; c < ncol; ++c) column(c, rowok && (g * XW_CK + c) > 0);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(empty + s);
-            (void)nslot;
         }
         double va, vb, vz;
         elim2_flush(S, va, vb, vz);
