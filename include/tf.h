@@ -194,6 +194,26 @@ size_t    tf_betti_workspace_bytes(int nx, int ny, int nthr);
 tf_status tf_betti(const double* h, int nx, int ny, const double* thresholds, int nthr,
                    long long* b0, long long* b1, void* dev_ws, void* cuda_stream);
 
+/*
+ * Radial Fourier transform, steps one to four of Appendix B:
+ *   1. |DFT2(h - H0)| on the nx x ny samples (the FFT itself is cuFFT, loaded at run time: TF_ERR_UNSUPPORTED if
+ *      libcufft.so.11 cannot be found);
+ *   2. convolution with a Gaussian of standard deviation `sigma` in DFT-index units, truncated at ceil(3 sigma) <= 64,
+ *      normalised, periodic, separable (sigma = 0: no filter);
+ *   3./4. eq. (B.1): for every radius that occurs, the mean over the points of equal radius and their number N_k.
+ * The domain must be square, nx dx = ny dy = L: equal radius then means equal kx^2 + ky^2 of the signed DFT indices;
+ * radii up to kmax index units are reported (the paper restricts q to [0, 5 q_m]).
+ * h: DEVICE pointer (nx*ny doubles, row-major).  q, zeta, count: HOST arrays of `cap` entries, filled in ascending q
+ * with q_r = 2 pi sqrt(kx^2 + ky^2) / L, the mean magnitude and N_k; *nk = number of distinct radii (may exceed cap:
+ * then only the first cap are stored).  dev_ws: tf_spectrum_workspace_bytes(nx, ny, kmax) bytes of device scratch.
+ * Synchronises the stream.  Steps five and six of the appendix (least-squares fit, moving average, maxima) are 1-D
+ * post-processing of this output and are left to the caller.
+ */
+size_t    tf_spectrum_workspace_bytes(int nx, int ny, int kmax);
+tf_status tf_radial_spectrum(const double* h, int nx, int ny, double L, double H0, double sigma, int kmax,
+                             double* q, double* zeta, long long* count, int cap, int* nk,
+                             void* dev_ws, void* cuda_stream);
+
 /* Text of the last error on this context ("" if none); ctx == NULL: last error of a failed
  * tf_create* / tf_penta_solve on this thread.  Valid until the next call. */
 const char* tf_last_error(const tf_ctx* ctx);

@@ -7,6 +7,8 @@
 #include "tf_bwd.cuh"
 #include "tf_fwd.cuh"
 #include "tf_topo.cuh"
+#include "tf_spectrum.cuh"
+#include <dlfcn.h>
 
 #include <algorithm>
 #include <atomic>
@@ -960,6 +962,113 @@ tf_status tf_betti(const double* h, int nx, int ny, const double* thresholds, in
     TF_CUDA(nullptr, cudaMemcpyAsync(host.data(), cnt, host.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     TF_CUDA(nullptr, cudaStreamSynchronize(st));
     for (int t = 0; t < nthr; ++t) { b0[t] = (long long)host[2 * t]; b1[t] = (long long)host[2 * t + 1]; }
+    return TF_OK;
+}
+
+// ---- radial Fourier transform, App. B steps 1-4 (tf_spectrum.cuh); the FFT is cuFFT, loaded at run time
+namespace {
+struct CuFFT {
+    void* lib = nullptr;
+    int (*plan2d)(int*, int, int, int) = nullptr;
+    int (*set_stream)(int, cudaStream_t) = nullptr;
+    int (*exec_d2z)(int, double*, void*) = nullptr;
+    int (*destroy)(int) = nullptr;
+    int plan = -1, pnx = 0, pny = 0, pdev = -1;
+    bool load()
+    {
+        if (lib) return true;
+        const char* names[] = {"libcufft.so.11", "/usr/local/cuda/lib64/libcufft.so.11", "libcufft.so", "/usr/local/cuda/lib64/libcufft.so"};
+        for (const char* n : names) {
+            lib = dlopen(n, RTLD_NOW | RTLD_LOCAL);
+            if (lib) break;
+        }
+        if (!lib) return false;
+        plan2d = (int (*)(int*, int, int, int))dlsym(lib, "cufftPlan2d");
+        set_stream = (int (*)(int, cudaStream_t))dlsym(lib, "cufftSetStream");
+        exec_d2z = (int (*)(int, double*, void*))dlsym(lib, "cufftExecD2Z");
+        destroy = (int (*)(int))dlsym(lib, "cufftDestroy");
+        if (!plan2d || !set_stream || !exec_d2z || !destroy) { dlclose(lib); lib = nullptr; return false; }
+        return true;
+    }
+    bool get_plan(int nx, int ny)
+    {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (plan >= 0 && pnx == nx && pny == ny && pdev == dev) return true;
+        if (plan >= 0) { destroy(plan); plan = -1; }
+        if (plan2d(&plan, ny, nx, 0x6a /* CUFFT_D2Z */) != 0) { plan = -1; return false; }
+        pnx = nx; pny = ny; pdev = dev;
+        return true;
+    }
+};
+CuFFT g_fft;
+size_t sp_field_bytes(int nx, int ny) { return align_up((size_t)nx * ny * sizeof(double)); }
+size_t sp_half_bytes(int nx, int ny) { return align_up((size_t)ny * (nx / 2 + 1) * 2 * sizeof(double)); }
+}  // namespace
+
+size_t tf_spectrum_workspace_bytes(int nx, int ny, int kmax)
+{
+    if (nx < 2 || ny < 2 || kmax < 0) return 0;
+    const size_t nk = (size_t)kmax * kmax + 1;
+    return 2 * sp_field_bytes(nx, ny) + sp_half_bytes(nx, ny) + align_up(nk * sizeof(double)) + align_up(nk * sizeof(unsigned long long));
+}
+
+tf_status tf_radial_spectrum(const double* h, int nx, int ny, double L, double H0, double sigma, int kmax, double* q,
+                             double* zeta, long long* count, int cap, int* nk_out, void* dev_ws, void* cuda_stream)
+{
+    if (nx < 2 || ny < 2 || kmax < 0 || cap < 0) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_radial_spectrum: bad shape, kmax or cap");
+    if ((long long)nx * ny >= (1LL << 31)) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_radial_spectrum: nx*ny must be < 2^31");
+    if (!(L > 0) || !std::isfinite(L) || !std::isfinite(H0) || !(sigma >= 0) || !std::isfinite(sigma))
+        return fail(nullptr, TF_ERR_INVALID_ARG, "tf_radial_spectrum: need L > 0, sigma >= 0, finite H0");
+    if (!h || !q || !zeta || !count || !nk_out || !dev_ws) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_radial_spectrum: NULL pointer");
+    if (kmax > 20000) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_radial_spectrum: kmax <= 20000");
+    SpWeights W;
+    W.r = sigma > 0 ? (int)std::ceil(3.0 * sigma) : 0;
+    if (W.r > SP_MAXW) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_radial_spectrum: ceil(3 sigma) must be <= 64");
+    {
+        double sum = 0.0;
+        for (int a = 0; a <= 2 * W.r; ++a) { const double m = a - W.r; W.w[a] = W.r ? std::exp(-m * m / (2.0 * sigma * sigma)) : 1.0; sum += W.w[a]; }
+        for (int a = 0; a <= 2 * W.r; ++a) W.w[a] /= sum;
+    }
+    if (!g_fft.load()) return fail(nullptr, TF_ERR_UNSUPPORTED, "tf_radial_spectrum: libcufft.so.11 not found");
+    if (!g_fft.get_plan(nx, ny)) return fail(nullptr, TF_ERR_CUDA, "tf_radial_spectrum: cufftPlan2d failed");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n = (size_t)nx * ny, nk = (size_t)kmax * kmax + 1;
+    char* ws = (char*)dev_ws;
+    double* A = (double*)ws;
+    double* B = (double*)(ws + sp_field_bytes(nx, ny));
+    double2* Z = (double2*)(ws + 2 * sp_field_bytes(nx, ny));
+    double* sums = (double*)((char*)Z + sp_half_bytes(nx, ny));
+    unsigned long long* cnts = (unsigned long long*)((char*)sums + align_up(nk * sizeof(double)));
+    TF_CUDA(nullptr, cudaMemsetAsync(sums, 0, align_up(nk * sizeof(double)) + nk * sizeof(unsigned long long), st));
+    const unsigned gl = (unsigned)std::min<size_t>((n + SP_THREADS - 1) / SP_THREADS, (size_t)num_sms() * 16);
+    const dim3 g2((unsigned)((nx + SP_THREADS - 1) / SP_THREADS), (unsigned)ny);
+    if (g2.y > 65535u) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_radial_spectrum: ny must be <= 65535");
+    sp_subtract_kernel<<<gl, SP_THREADS, 0, st>>>(n, h, H0, A);
+    if (g_fft.set_stream(g_fft.plan, st) != 0 || g_fft.exec_d2z(g_fft.plan, A, Z) != 0)
+        return fail(nullptr, TF_ERR_CUDA, "tf_radial_spectrum: cufftExecD2Z failed");
+    sp_magnitude_kernel<<<g2, SP_THREADS, 0, st>>>(nx, ny, Z, A);
+    const double* smooth = A;
+    if (W.r > 0) {
+        sp_gauss_kernel<true><<<g2, SP_THREADS, 0, st>>>(nx, ny, A, B, W);
+        sp_gauss_kernel<false><<<g2, SP_THREADS, 0, st>>>(nx, ny, B, A, W);
+    }
+    sp_radial_kernel<<<g2, SP_THREADS, 0, st>>>(nx, ny, smooth, (long long)kmax * kmax, sums, cnts);
+    count_launch(W.r > 0 ? 5 : 3);
+    TF_CUDA(nullptr, cudaGetLastError());
+    std::vector<double> hs(nk);
+    std::vector<unsigned long long> hc(nk);
+    TF_CUDA(nullptr, cudaMemcpyAsync(hs.data(), sums, nk * sizeof(double), cudaMemcpyDeviceToHost, st));
+    TF_CUDA(nullptr, cudaMemcpyAsync(hc.data(), cnts, nk * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    TF_CUDA(nullptr, cudaStreamSynchronize(st));
+    int m = 0;
+    const double PI2 = 6.283185307179586476925286766559;
+    for (size_t k = 0; k < nk; ++k) {
+        if (!hc[k]) continue;
+        if (m < cap) { q[m] = PI2 * std::sqrt((double)k) / L; zeta[m] = hs[k] / (double)hc[k]; count[m] = (long long)hc[k]; }
+        ++m;
+    }
+    *nk_out = m;
     return TF_OK;
 }
 

@@ -45,6 +45,10 @@ SYMBOLS = {
     "tf_penta_solve": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int] + [_vp] * 9),
     "tf_penta_partition_chunks": (ctypes.c_int, [ctypes.c_int] * 4),
     "tf_betti_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int] * 3),
+    "tf_spectrum_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int] * 3),
+    "tf_radial_spectrum": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                          ctypes.c_int, _dp, _dp, ctypes.POINTER(ctypes.c_longlong), ctypes.c_int,
+                                          ctypes.POINTER(ctypes.c_int), _vp, _vp]),
     "tf_betti": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _dp, ctypes.c_int, ctypes.POINTER(ctypes.c_longlong),
                                 ctypes.POINTER(ctypes.c_longlong), _vp, _vp]),
     "tf_penta_workspace_bytes_ex": (ctypes.c_size_t, [ctypes.c_int] * 5),
@@ -310,3 +314,31 @@ def betti(h, thresholds, workspace=None, stream=None):
     if rc != OK:
         _err(None, rc, "tf_betti")
     return b0, b1
+
+
+def radial_spectrum(h, L, H0, sigma, kmax, workspace=None, stream=None):
+    """tf_radial_spectrum (App. B steps 1-4) on a contiguous CUDA float64 [ny][nx] tensor of a square domain of side L:
+    returns numpy arrays (q_r, mean magnitude, N_k) over the distinct radii up to kmax index units."""
+    torch = _torch()
+    if not (isinstance(h, torch.Tensor) and h.is_cuda and h.dtype == torch.float64 and h.is_contiguous() and h.dim() == 2):
+        raise ValueError("expected a contiguous CUDA float64 [ny][nx] tensor")
+    ny, nx = h.shape
+    Lb = lib()
+    need = Lb.tf_spectrum_workspace_bytes(nx, ny, kmax)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=h.device)
+    if workspace.numel() * workspace.element_size() < need or workspace.data_ptr() % 256:
+        raise ValueError("workspace too small or not 256-byte aligned")
+    cap = kmax * kmax + 1
+    q = np.zeros(cap)
+    z = np.zeros(cap)
+    cnt = np.zeros(cap, dtype=np.int64)
+    nk = ctypes.c_int(0)
+    st = (torch.cuda.current_stream(h.device) if stream is None else stream).cuda_stream
+    rc = Lb.tf_radial_spectrum(h.data_ptr(), nx, ny, float(L), float(H0), float(sigma), int(kmax), q.ctypes.data_as(_dp),
+                               z.ctypes.data_as(_dp), cnt.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong)), cap,
+                               ctypes.byref(nk), workspace.data_ptr(), st)
+    if rc != OK:
+        _err(None, rc, "tf_radial_spectrum")
+    m = min(nk.value, cap)
+    return q[:m], z[:m], cnt[:m]
