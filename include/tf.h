@@ -214,6 +214,19 @@ tf_status tf_radial_spectrum(const double* h, int nx, int ny, double L, double H
                              double* q, double* zeta, long long* count, int cap, int* nk,
                              void* dev_ws, void* cuda_stream);
 
+/*
+ * Steps five and six of Appendix B and the extraction of the maxima, on the HOST (a few thousand
+ * numbers): (B.2) least-squares fit of a continuous piecewise-linear function with value 0 at q = 0 whose intervals
+ * hold `per_interval` points each (paper: 10; the last interval takes what is left; points with q = 0 are left out);
+ * evaluation on `ngrid` equispaced points of [0, q_last] (paper: 400); (B.3) moving average with P = 3, 2, 1 (the
+ * window is cut off at the ends of the grid); derivative by second-order differences, roots by sign change and linear
+ * interpolation, kept if the second difference is negative.  q (strictly ascending), zeta: nk host values, e.g. the
+ * output of tf_radial_spectrum.  qgrid, zsmooth: ngrid host values each, or NULL.  peak_q, peak_z: the first peak_cap
+ * maxima in ascending q; *npeaks = number found.  No GPU work.
+ */
+tf_status tf_radial_peaks(const double* q, const double* zeta, int nk, int per_interval, int ngrid,
+                          double* qgrid, double* zsmooth, double* peak_q, double* peak_z, int peak_cap, int* npeaks);
+
 /* Text of the last error on this context ("" if none); ctx == NULL: last error of a failed
  * tf_create* / tf_penta_solve on this thread.  Valid until the next call. */
 const char* tf_last_error(const tf_ctx* ctx);

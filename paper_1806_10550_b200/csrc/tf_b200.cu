@@ -1072,6 +1072,85 @@ tf_status tf_radial_spectrum(const double* h, int nx, int ny, double L, double H
     return TF_OK;
 }
 
+// ---- App. B steps 5-6 and the maxima: host-side 1-D post-processing of the radial spectrum
+tf_status tf_radial_peaks(const double* q, const double* zeta, int nk, int per_interval, int ngrid, double* qgrid,
+                          double* zsmooth, double* peak_q, double* peak_z, int peak_cap, int* npeaks)
+{
+    if (!q || !zeta || nk < 2 || per_interval < 2 || ngrid < 8 || peak_cap < 0 || (peak_cap > 0 && (!peak_q || !peak_z)) || !npeaks)
+        return fail(nullptr, TF_ERR_INVALID_ARG, "tf_radial_peaks: bad arguments");
+    // points with q > 0, ascending
+    std::vector<double> x, y;
+    for (int i = 0; i < nk; ++i) {
+        if (!std::isfinite(q[i]) || !std::isfinite(zeta[i])) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_radial_peaks: non-finite input");
+        if (i > 0 && !(q[i] > q[i - 1])) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_radial_peaks: q must be strictly ascending");
+        if (q[i] > 0.0) { x.push_back(q[i]); y.push_back(zeta[i]); }
+    }
+    const int n = (int)x.size();
+    if (n < per_interval) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_radial_peaks: fewer points than one interval");
+    // (B.2) knots: every interval holds per_interval points, the last one what is left; a_0 = 0 at q = 0
+    std::vector<double> ks(1, 0.0);
+    for (int i = per_interval - 1; i < n; i += per_interval) ks.push_back(x[i]);
+    if (ks.back() < x[n - 1]) ks.push_back(x[n - 1]);
+    const int K = (int)ks.size() - 1;
+    // normal equations of the hat functions of knots 1..K: symmetric positive definite, tridiagonal
+    std::vector<double> d(K, 0.0), u(K, 0.0), r(K, 0.0), a(K + 1, 0.0);
+    int k = 0;
+    for (int i = 0; i < n; ++i) {
+        while (k < K - 1 && x[i] > ks[k + 1]) ++k;               // interval [ks[k], ks[k+1]] containing x[i]
+        const double sft = (x[i] - ks[k]) / (ks[k + 1] - ks[k]);
+        if (k >= 1) { d[k - 1] += (1.0 - sft) * (1.0 - sft); u[k - 1] += (1.0 - sft) * sft; r[k - 1] += (1.0 - sft) * y[i]; }
+        d[k] += sft * sft;
+        r[k] += sft * y[i];
+    }
+    for (int j = 1; j < K; ++j) {                                // Thomas on the symmetric system (sub-diagonal = u)
+        const double m = u[j - 1] / d[j - 1];
+        d[j] -= m * u[j - 1];
+        r[j] -= m * r[j - 1];
+    }
+    if (!(d[K - 1] > 0.0)) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_radial_peaks: singular fit");
+    a[K] = r[K - 1] / d[K - 1];
+    for (int j = K - 2; j >= 0; --j) a[j + 1] = (r[j] - u[j] * a[j + 2]) / d[j];
+    // 400-point grid on [0, q_K], evaluate, (B.3) moving average with P = 3, 2, 1 (window cut at the ends)
+    std::vector<double> g(ngrid), f(ngrid), t(ngrid), df(ngrid);
+    const double h = ks[K] / (ngrid - 1);
+    k = 0;
+    for (int i = 0; i < ngrid; ++i) {
+        g[i] = i == ngrid - 1 ? ks[K] : i * h;
+        while (k < K - 1 && g[i] > ks[k + 1]) ++k;
+        const double sft = (g[i] - ks[k]) / (ks[k + 1] - ks[k]);
+        f[i] = a[k] + sft * (a[k + 1] - a[k]);
+    }
+    for (int P = 3; P >= 1; --P) {
+        for (int i = 0; i < ngrid; ++i) {
+            const int lo = std::max(0, i - P), hi = std::min(ngrid - 1, i + P);
+            double sum = 0.0;
+            for (int j = lo; j <= hi; ++j) sum += f[j];
+            t[i] = sum / (hi - lo + 1);
+        }
+        f.swap(t);
+    }
+    // maxima: second-order differences, roots of the derivative by sign change + linear interpolation
+    for (int i = 1; i < ngrid - 1; ++i) df[i] = (f[i + 1] - f[i - 1]) / (2.0 * h);
+    df[0] = (-3.0 * f[0] + 4.0 * f[1] - f[2]) / (2.0 * h);
+    df[ngrid - 1] = (3.0 * f[ngrid - 1] - 4.0 * f[ngrid - 2] + f[ngrid - 3]) / (2.0 * h);
+    int np = 0;
+    for (int i = 0; i < ngrid - 1; ++i) {
+        if (df[i] > 0.0 && df[i + 1] <= 0.0) {
+            const double tt = df[i] / (df[i] - df[i + 1]);
+            int c = tt < 0.5 ? i : i + 1;
+            c = std::min(std::max(c, 1), ngrid - 2);
+            if (f[c + 1] - 2.0 * f[c] + f[c - 1] < 0.0) {
+                if (np < peak_cap) { peak_q[np] = g[i] + tt * h; peak_z[np] = f[i] + tt * (f[i + 1] - f[i]); }
+                ++np;
+            }
+        }
+    }
+    *npeaks = np;
+    if (qgrid) std::copy(g.begin(), g.end(), qgrid);
+    if (zsmooth) std::copy(f.begin(), f.end(), zsmooth);
+    return TF_OK;
+}
+
 const char* tf_last_error(const tf_ctx* c) { return c ? c->err.c_str() : g_err.c_str(); }
 
 unsigned long long tf_kernel_launches(void) { return g_launches.load(); }

@@ -46,6 +46,8 @@ SYMBOLS = {
     "tf_penta_partition_chunks": (ctypes.c_int, [ctypes.c_int] * 4),
     "tf_betti_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int] * 3),
     "tf_spectrum_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int] * 3),
+    "tf_radial_peaks": (ctypes.c_int, [_dp, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, _dp, _dp, _dp, ctypes.c_int,
+                                       ctypes.POINTER(ctypes.c_int)]),
     "tf_radial_spectrum": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double,
                                           ctypes.c_int, _dp, _dp, ctypes.POINTER(ctypes.c_longlong), ctypes.c_int,
                                           ctypes.POINTER(ctypes.c_int), _vp, _vp]),
@@ -342,3 +344,18 @@ def radial_spectrum(h, L, H0, sigma, kmax, workspace=None, stream=None):
         _err(None, rc, "tf_radial_spectrum")
     m = min(nk.value, cap)
     return q[:m], z[:m], cnt[:m]
+
+
+def radial_peaks(q, zeta, per_interval=10, ngrid=400, max_peaks=64):
+    """tf_radial_peaks (App. B steps 5-6 and the maxima; host only): returns (grid, smoothed spectrum, [(q, value), ...])."""
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    z = np.ascontiguousarray(zeta, dtype=np.float64)
+    g, f = np.zeros(ngrid), np.zeros(ngrid)
+    pq, pz = np.zeros(max_peaks), np.zeros(max_peaks)
+    n = ctypes.c_int(0)
+    rc = lib().tf_radial_peaks(q.ctypes.data_as(_dp), z.ctypes.data_as(_dp), len(q), per_interval, ngrid, g.ctypes.data_as(_dp),
+                               f.ctypes.data_as(_dp), pq.ctypes.data_as(_dp), pz.ctypes.data_as(_dp), max_peaks, ctypes.byref(n))
+    if rc != OK:
+        _err(None, rc, "tf_radial_peaks")
+    m = min(n.value, max_peaks)
+    return g, f, list(zip(pq[:m].tolist(), pz[:m].tolist()))

@@ -55,3 +55,46 @@ def test_radially_symmetric_input_is_its_own_angular_mean():
     f = np.exp(-r2 / 50.0) * (1 + 0.3 * np.cos(0.2 * np.sqrt(r2)))
     keys, means, _ = spectrum.radial_mean(f, 15)
     assert np.allclose(means, np.exp(-keys / 50.0) * (1 + 0.3 * np.cos(0.2 * np.sqrt(keys))), rtol=0, atol=1e-14)
+
+
+# ------------------------------------------------------------------ steps five and six, maxima
+def test_fit_reproduces_a_piecewise_linear_function_on_its_own_knots():
+    rng = np.random.default_rng(1)
+    q = np.sort(rng.uniform(0.01, 5.0, 95))
+    ks = spectrum.knots(q, 10)
+    assert ks[0] == 0.0 and ks[1] == q[9] and ks[2] == q[19] and ks[-1] == q[-1] and len(ks) == 11   # 9 full intervals + 5 left over
+    a_true = np.concatenate([[0.0], rng.uniform(-1, 1, len(ks) - 1)])
+    z = np.interp(q, ks, a_true)
+    ks2, a = spectrum.piecewise_linear_fit(q, z, 10)
+    assert np.array_equal(ks2, ks) and np.allclose(a, a_true, atol=1e-10)       # data on the model: residual zero, parameters recovered
+    # and it IS a least-squares solution for noisy data: the residual is orthogonal to every hat function
+    zn = z + 0.1 * rng.standard_normal(len(q))
+    _, an = spectrum.piecewise_linear_fit(q, zn, 10)
+    r = np.interp(q, ks, an) - zn
+    for k in range(1, len(ks)):
+        e = np.zeros(len(ks)); e[k] = 1.0
+        assert abs(np.dot(r, np.interp(q, ks, e))) < 1e-10
+
+
+def test_moving_average_properties():
+    x = np.linspace(0, 1, 50)
+    lin = 2.0 + 3.0 * x
+    for P in (1, 2, 3):
+        m = spectrum.moving_average(lin, P)
+        assert np.allclose(m[P:-P], lin[P:-P], atol=1e-14)                       # symmetric window: linear functions pass
+        assert abs(m[0] - lin[:P + 1].mean()) < 1e-14                             # truncated window at the end
+    imp = np.zeros(21); imp[10] = 1.0
+    m = spectrum.moving_average(imp, 3)
+    assert np.allclose(m[7:14], 1.0 / 7) and m[6] == 0 and m[14] == 0
+
+
+def test_maximum_of_a_noisy_bump_is_found():
+    rng = np.random.default_rng(2)
+    q = np.sort(rng.uniform(0.0, 6.0, 3000))
+    q0 = 2.2
+    z = q * np.exp(-0.5 * ((q - q0) / 0.8) ** 2) + 0.01 * rng.standard_normal(len(q))
+    true_max = 0.5 * (q0 + np.sqrt(q0 * q0 + 4 * 0.64))                          # d/dq [q exp(-(q-q0)^2/(2 s^2))] = 0
+    x, f, peaks = spectrum.smooth_and_peaks(q, z, 10, 400)
+    assert len(x) == 400 and x[0] == 0.0 and abs(x[-1] - q[-1]) < 1e-15
+    best = max(peaks, key=lambda p: p[1])
+    assert abs(best[0] - true_max) < 0.05
