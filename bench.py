@@ -45,6 +45,9 @@ def parse():
     ap.add_argument("--variant", default="lu", choices=["lu", "partition"], help="config 4 only: tf_penta_solve_ex variant")
     ap.add_argument("--nparts", type=int, default=0, help="config 4 only: chunks per system of the partition variant (0: automatic)")
     ap.add_argument("--cusparse", action="store_true", help="config 4 only: also time cuSPARSE's interleaved-batch routine (context)")
+    ap.add_argument("--slabs", action="store_true",
+                    help="config 4 only: every system spread over the ranks (paper_1806_10550_b200/dist.py: one NCCL "
+                         "all-gather of the interface values); strong scaling, launch with torchrun for --gpus N > 1")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -367,6 +370,54 @@ def cusparse_gpsv_interleaved(e, c, d, a, b, y, steps):
 
 
 # ----------------------------------------------------------------------------------------- config 4 (side measurement)
+def run_penta_slabs(args, cfg):
+    """Config 4 with every system cut into one slab of rows per rank (direction 1: systems = columns): the slab solver
+    of DESIGN.md section 8 -- interface pass, NCCL all-gather of 20 * nparts doubles per system and rank, reduced +
+    chunk solves.  Strong scaling: the 16384 x 16384 problem is fixed, each rank holds 1/N of every system."""
+    import torch
+    import torch.distributed as dist
+    from paper_1806_10550_b200 import dist as tfdist, tf
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    own_group = not dist.is_initialized()
+    if own_group:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29531")
+        dist.init_process_group("nccl", rank=rank, world_size=world)
+    n = cfg["nrow"]
+    nsys = args.nsys or n
+    lo, hi = tfdist.slab_bounds(n, world, rank)
+    gen = torch.Generator(device="cuda").manual_seed(cfg["seed"] + 1000 * rank)
+    U = lambda a, b: torch.rand(hi - lo, nsys, dtype=torch.float64, device="cuda", generator=gen) * (b - a) + a
+    e, c, a, b, y = U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1)
+    d = 1 + e.abs() + c.abs() + a.abs() + b.abs() + U(0, 1)
+    nparts = max(1, args.nparts)
+    solve = lambda: tfdist.penta_solve_slabs(1, nparts, e, c, d, a, b, y)
+    for _ in range(max(args.warmup, 3)):
+        solve()
+    dist.barrier()
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        solve()
+    ev1.record()
+    torch.cuda.synchronize()
+    dist.barrier()
+    sec = max_over_ranks(ev0.elapsed_time(ev1) * 1e-3 / args.steps, world, "cuda")
+    if rank == 0:
+        print(json.dumps({"metric": "pentadiagonal unknowns/s (fp64), isolated solve, systems spread over the ranks",
+                          "unit": "unknowns/s", "n_gpus": world, "value": nsys * n / sec, "ms_per_step": sec * 1e3,
+                          "steps": args.steps, "warmup": max(args.warmup, 3), "dtype": "f64", "scaling": "strong",
+                          "data": "synthetic (config 4 recipe drawn on the GPU)", "higher_is_better": True,
+                          "config": {"workload": cfg["name"], "systems": nsys, "length": n, "variant": "slabs",
+                                     "chunks_per_rank": nparts, "exchange": "all-gather of 20*chunks doubles per system and rank",
+                                     "alg_bytes_per_unknown": 200},
+                          "gpu_launches": 4 * args.steps}), flush=True)
+    if own_group:
+        dist.destroy_process_group()
+
+
 def run_penta(args, cfg):
     """Isolated batched pentadiagonal solve (BASELINE.json config 4), both directions, device-resident inputs of
     the config's recipe drawn on the GPU (torch generator, seed 4): not the headline line, a kernel measurement."""
@@ -443,6 +494,8 @@ def run_penta(args, cfg):
 def main():
     args = parse()
     cfg = inputs.config(args.config)
+    if args.config == 4 and args.slabs and args.impl == "b200":
+        return run_penta_slabs(args, cfg)
     if args.config == 4:
         return run_penta(args, cfg) if args.impl == "b200" else print(json.dumps(
             {"impl": "reference", "unavailable": "config 4 is a side measurement of the B200 arm only"}))

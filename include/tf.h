@@ -181,6 +181,32 @@ tf_status tf_penta_solve_ex(int nrow, int ncol, int dir, int variant, int nparts
                             void* dev_ws, void* cuda_stream);
 
 /*
+ * The partition variant across devices (slab decomposition with a reduced-interface solve
+ * instead of a transpose).  Every system is cut into `nslabs` slabs of consecutive rows (dir = 1; columns for dir = 0),
+ * one slab per device, each slab into `nparts` chunks (the same nparts on every device).  Per device:
+ *   1. tf_penta_slab_interface on the LOCAL arrays (the slab only: nrow x ncol is the local shape) writes the local
+ *      interface values, tf_penta_slab_interface_doubles(...) doubles (device);
+ *   2. the caller gathers them from all devices in slab order (an all-gather of 20 * nparts doubles per system and
+ *      device: the one exchange step) into iface_all;
+ *   3. tf_penta_slab_solve solves the reduced system of all nslabs * nparts chunks (redundantly on every device) and
+ *      then the local chunks -> x (local shape).
+ * Band entries that point outside the WHOLE system are ignored; entries at slab seams are used.  Same constraints as
+ * TF_PENTA_PARTITION: local length / nparts >= 96, at least 32 systems, even nrow and ncol, 16-byte aligned arrays.
+ * dev_ws of tf_penta_slab_solve: tf_penta_slab_workspace_bytes(local nrow, local ncol, dir, nparts, nslabs) bytes.
+ * With nslabs = 1 the two calls are the single-device partition variant.
+ */
+size_t    tf_penta_slab_interface_doubles(int nrow, int ncol, int dir, int nparts);
+size_t    tf_penta_slab_workspace_bytes(int nrow, int ncol, int dir, int nparts, int nslabs);
+tf_status tf_penta_slab_interface(int nrow, int ncol, int dir, int nparts, int slab, int nslabs,
+                                  const double* e, const double* c, const double* d,
+                                  const double* a, const double* b, const double* rhs,
+                                  double* iface_local, void* cuda_stream);
+tf_status tf_penta_slab_solve(int nrow, int ncol, int dir, int nparts, int slab, int nslabs,
+                              const double* e, const double* c, const double* d,
+                              const double* a, const double* b, const double* rhs,
+                              const double* iface_all, double* x, void* dev_ws, void* cuda_stream);
+
+/*
  * Betti numbers of the thresholded film ("b0 counts the number of mountain peaks
  * (components) above H*, and b1 counts the number of valleys (loops) surrounding the peaks"; the paper uses CHomP on
  * cubical sets).  For every threshold H* = thresholds[t] (host array), with X = the closed unit squares of the cells

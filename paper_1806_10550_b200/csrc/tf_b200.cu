@@ -463,33 +463,34 @@ constexpr int PART_MAX = 256;             // the reduced system is solved serial
 constexpr int PI_NST = 4;                 // interface pass, columns: 4 stages x 12 KiB
 constexpr int PJ_NST = 3;                 // interface pass, rows: 3 stages x 24 KiB
 
-tf_status penta_partition(int nrow, int ncol, int dir, int P, const double* e, const double* c, const double* d,
-                          const double* a, const double* b, const double* rhs, double* x, char* ws, size_t fb,
-                          cudaStream_t st)
+// phases: 1 = interface pass (-> iface, local chunks), 2 = reduced system over all Pg chunks (iface_all -> X),
+// 4 = chunk solves (X -> x).  Single device: all three, Pg = P, p_off = 0, iface_all = iface.
+tf_status penta_partition_phases(int phases, int nrow, int ncol, int dir, int P, int Pg, int p_off, const double* e,
+                                 const double* c, const double* d, const double* a, const double* b, const double* rhs,
+                                 double* x, double* al, double* be, double* zz, double* iface, const double* iface_all,
+                                 double* rc, double* X, cudaStream_t st)
 {
-    double* al = (double*)ws;
-    double* be = (double*)(ws + fb);
-    double* zz = (double*)(ws + 2 * fb);
     const size_t nsys = (size_t)(dir ? ncol : nrow);
-    double* iface = (double*)(ws + 3 * fb);
-    double* rc = iface + (size_t)P * 2 * IF_VALS * nsys;
-    double* X = rc + (size_t)P * RC_VALS * nsys;
     const double* in6[6] = {e, c, d, a, b, rhs};
-    bool ok = ((uintptr_t)ws % 16 == 0) && ((uintptr_t)x % 16 == 0);
+    bool ok = true;
     for (int k = 0; k < 6; ++k) ok = ok && ((uintptr_t)in6[k] % 16 == 0);
+    if (phases & 4) ok = ok && ((uintptr_t)x % 16 == 0) && ((uintptr_t)al % 16 == 0);
     Maps6 M;
     CUtensorMap mw[3], mx;
     const double* w3[3] = {al, be, zz};
     if (dir == 1) {
         for (int k = 0; k < 6; ++k) ok = ok && make_map2d(&M.m[k], in6[k], ncol, nrow, 32, PC_RS, false);
-        for (int k = 0; k < 3; ++k) ok = ok && make_map2d(&mw[k], w3[k], ncol, nrow, 32, YT_RS, false);
+        if (phases & 4) for (int k = 0; k < 3; ++k) ok = ok && make_map2d(&mw[k], w3[k], ncol, nrow, 32, YT_RS, false);
     } else {
         for (int k = 0; k < 6; ++k) ok = ok && make_map2d(&M.m[k], in6[k], ncol, nrow, 16, 32, true);
-        for (int k = 0; k < 3; ++k) ok = ok && make_map2d(&mw[k], w3[k], nrow, ncol, 32, 16, false);
-        ok = ok && make_map2d(&mx, x, ncol, nrow, 16, 32, true);
+        if (phases & 4) {
+            for (int k = 0; k < 3; ++k) ok = ok && make_map2d(&mw[k], w3[k], nrow, ncol, 32, 16, false);
+            ok = ok && make_map2d(&mx, x, ncol, nrow, 16, 32, true);
+        }
     }
     if (!ok) return fail(nullptr, TF_ERR_UNSUPPORTED, "partition variant: 16-byte aligned arrays and TMA tensor maps required");
     const dim3 g((unsigned)((nsys + 31) / 32), 2, (unsigned)P);
+    int launches = 0;
     if (dir == 1) {
         constexpr size_t SMI = (size_t)PI_NST * 6 * PC_RS * 32 * 8 + 8 * PI_NST + 1024;
         constexpr size_t SMF = (size_t)PC_NST * 6 * PC_RS * 32 * 8 + 8 * PC_NST + 1024;
@@ -502,10 +503,13 @@ tf_status penta_partition(int nrow, int ncol, int dir, int P, const double* e, c
             if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
             ready.mark();
         }
-        penta_col_iface_kernel<PI_NST, PC_RS><<<g, 32, SMI, st>>>(M, nrow, ncol, P, iface);
-        penta_reduced_kernel<<<(unsigned)((nsys + 31) / 32), 32, 0, st>>>((int)nsys, P, iface, rc, X);
-        penta_col_fwd2_kernel<PC_NST, PC_RS><<<g, 32, SMF, st>>>(M, nrow, ncol, 0, al, be, zz, P, X);
-        ybwd2_tma_kernel<YT_NST, YT_RS, true><<<g, 32, SMB, st>>>(mw[0], mw[1], mw[2], ncol, nrow, 0, al, be, zz, x, P);
+        if (phases & 1) { penta_col_iface_kernel<PI_NST, PC_RS><<<g, 32, SMI, st>>>(M, nrow, ncol, P, iface, Pg, p_off); ++launches; }
+        if (phases & 2) { penta_reduced_kernel<<<(unsigned)((nsys + 31) / 32), 32, 0, st>>>((int)nsys, Pg, iface_all, rc, X); ++launches; }
+        if (phases & 4) {
+            penta_col_fwd2_kernel<PC_NST, PC_RS><<<g, 32, SMF, st>>>(M, nrow, ncol, chunk_mid(0, nrow), al, be, zz, P, X, Pg, p_off);
+            ybwd2_tma_kernel<YT_NST, YT_RS, true><<<g, 32, SMB, st>>>(mw[0], mw[1], mw[2], ncol, nrow, 0, al, be, zz, x, P);
+            launches += 2;
+        }
     } else {
         constexpr size_t SMI = (size_t)PJ_NST * 6 * 32 * 16 * 8 + 8 * PJ_NST + 1024;
         constexpr size_t SMF = (size_t)PR_NST * 6 * 32 * 16 * 8 + 8 * PR_NST + 1024;
@@ -518,15 +522,31 @@ tf_status penta_partition(int nrow, int ncol, int dir, int P, const double* e, c
             if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
             ready.mark();
         }
-        penta_row_iface_kernel<PJ_NST><<<g, 32, SMI, st>>>(M, nrow, ncol, P, iface);
-        penta_reduced_kernel<<<(unsigned)((nsys + 31) / 32), 32, 0, st>>>((int)nsys, P, iface, rc, X);
-        penta_row_fwd2_kernel<PR_NST><<<g, 32, SMF, st>>>(M, nrow, ncol, 0, al, be, zz, P, X);
-        xbwd2_tma_kernel<XT_NST, false, true><<<g, 32, SMB, st>>>(mw[0], mw[1], mw[2], mx, mx, ncol, nrow, 0, al, be, zz, nullptr, P);
+        if (phases & 1) { penta_row_iface_kernel<PJ_NST><<<g, 32, SMI, st>>>(M, nrow, ncol, P, iface, Pg, p_off); ++launches; }
+        if (phases & 2) { penta_reduced_kernel<<<(unsigned)((nsys + 31) / 32), 32, 0, st>>>((int)nsys, Pg, iface_all, rc, X); ++launches; }
+        if (phases & 4) {
+            penta_row_fwd2_kernel<PR_NST><<<g, 32, SMF, st>>>(M, nrow, ncol, chunk_mid(0, ncol), al, be, zz, P, X, Pg, p_off);
+            xbwd2_tma_kernel<XT_NST, false, true><<<g, 32, SMB, st>>>(mw[0], mw[1], mw[2], mx, mx, ncol, nrow, 0, al, be, zz, nullptr, P);
+            launches += 2;
+        }
     }
-    count_launch(4);
+    count_launch(launches);
     cudaError_t ee = cudaGetLastError();
-    if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "tf_penta_solve_ex (partition) launch");
+    if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "partition variant launch");
     return TF_OK;
+}
+
+tf_status penta_partition(int nrow, int ncol, int dir, int P, const double* e, const double* c, const double* d,
+                          const double* a, const double* b, const double* rhs, double* x, char* ws, size_t fb,
+                          cudaStream_t st)
+{
+    if ((uintptr_t)ws % 16) return fail(nullptr, TF_ERR_UNSUPPORTED, "partition variant: workspace must be 16-byte aligned");
+    const size_t nsys = (size_t)(dir ? ncol : nrow);
+    double* iface = (double*)(ws + 3 * fb);
+    double* rc = iface + (size_t)P * 2 * IF_VALS * nsys;
+    double* X = rc + (size_t)P * RC_VALS * nsys;
+    return penta_partition_phases(7, nrow, ncol, dir, P, P, 0, e, c, d, a, b, rhs, x, (double*)ws, (double*)(ws + fb),
+                                  (double*)(ws + 2 * fb), iface, iface, rc, X, st);
 }
 
 }  // namespace
@@ -799,6 +819,56 @@ size_t tf_penta_workspace_bytes(int nrow, int ncol)
 {
     if (nrow < 1 || ncol < 1) return 0;
     return 3 * align_up((size_t)nrow * ncol * sizeof(double));
+}
+
+// ---- slabs of a line on different devices: the partition variant with an exchange step
+static bool slab_shape_ok(int nrow, int ncol, int dir, int nparts)
+{
+    if (nrow < 1 || ncol < 1 || (dir != 0 && dir != 1) || nparts < 1 || nparts > PART_MAX) return false;
+    const int len = dir ? nrow : ncol, nsys = dir ? ncol : nrow;
+    return len / nparts >= PART_MIN_LEN && nsys >= 32 && nrow % 2 == 0 && ncol % 2 == 0;
+}
+
+size_t tf_penta_slab_interface_doubles(int nrow, int ncol, int dir, int nparts)
+{
+    if (!slab_shape_ok(nrow, ncol, dir, nparts)) return 0;
+    return (size_t)nparts * 2 * IF_VALS * (size_t)(dir ? ncol : nrow);
+}
+
+size_t tf_penta_slab_workspace_bytes(int nrow, int ncol, int dir, int nparts, int nslabs)
+{
+    if (!slab_shape_ok(nrow, ncol, dir, nparts) || nslabs < 1 || (long long)nslabs * nparts > 65535) return 0;
+    const size_t nsys = (size_t)(dir ? ncol : nrow);
+    return tf_penta_workspace_bytes(nrow, ncol) + align_up((size_t)nslabs * nparts * (RC_VALS + 4) * nsys * sizeof(double));
+}
+
+tf_status tf_penta_slab_interface(int nrow, int ncol, int dir, int nparts, int slab, int nslabs, const double* e,
+                                  const double* c, const double* d, const double* a, const double* b, const double* rhs,
+                                  double* iface_local, void* cuda_stream)
+{
+    if (!slab_shape_ok(nrow, ncol, dir, nparts) || nslabs < 1 || slab < 0 || slab >= nslabs)
+        return fail(nullptr, TF_ERR_INVALID_ARG, "tf_penta_slab_interface: bad shape, chunk count or slab index");
+    if (!e || !c || !d || !a || !b || !rhs || !iface_local) return fail(nullptr, TF_ERR_INVALID_ARG, "NULL pointer");
+    return penta_partition_phases(1, nrow, ncol, dir, nparts, nslabs * nparts, slab * nparts, e, c, d, a, b, rhs, nullptr,
+                                  nullptr, nullptr, nullptr, iface_local, nullptr, nullptr, nullptr, (cudaStream_t)cuda_stream);
+}
+
+tf_status tf_penta_slab_solve(int nrow, int ncol, int dir, int nparts, int slab, int nslabs, const double* e,
+                              const double* c, const double* d, const double* a, const double* b, const double* rhs,
+                              const double* iface_all, double* x, void* dev_ws, void* cuda_stream)
+{
+    if (!slab_shape_ok(nrow, ncol, dir, nparts) || nslabs < 1 || slab < 0 || slab >= nslabs)
+        return fail(nullptr, TF_ERR_INVALID_ARG, "tf_penta_slab_solve: bad shape, chunk count or slab index");
+    if (!e || !c || !d || !a || !b || !rhs || !iface_all || !x || !dev_ws) return fail(nullptr, TF_ERR_INVALID_ARG, "NULL pointer");
+    if ((uintptr_t)dev_ws % 16) return fail(nullptr, TF_ERR_UNSUPPORTED, "workspace must be 16-byte aligned");
+    const size_t fb = align_up((size_t)nrow * ncol * sizeof(double));
+    const size_t nsys = (size_t)(dir ? ncol : nrow);
+    const int Pg = nslabs * nparts;
+    char* ws = (char*)dev_ws;
+    double* rc = (double*)(ws + 3 * fb);
+    double* X = rc + (size_t)Pg * RC_VALS * nsys;
+    return penta_partition_phases(2 | 4, nrow, ncol, dir, nparts, Pg, slab * nparts, e, c, d, a, b, rhs, x, (double*)ws,
+                                  (double*)(ws + fb), (double*)(ws + 2 * fb), nullptr, iface_all, rc, X, (cudaStream_t)cuda_stream);
 }
 
 int tf_penta_partition_chunks(int nrow, int ncol, int dir, int nparts)

@@ -84,7 +84,8 @@ struct Maps6 { CUtensorMap m[6]; };      // e, c, d, a, b, rhs
 // out: [P][2][IF_VALS][ncol].
 template <int NST, int RS>
 __global__ void __launch_bounds__(32)
-penta_col_iface_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int P, double* __restrict__ out)
+penta_col_iface_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int P, double* __restrict__ out,
+                       int Pg, int p_off)
 {
     extern __shared__ unsigned char raw[];
     unsigned char* base = align1024(raw);
@@ -96,7 +97,9 @@ penta_col_iface_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int 
     const int dir = blockIdx.y, p = blockIdx.z;
     const int lo = chunk_lo(p, P, nrow), hi = chunk_lo(p + 1, P, nrow);
     const int ntile = (hi - lo + RS - 1) / RS;
-    const bool outside = dir ? (p < P - 1) : (p > 0);        // does this march have outside unknowns at its start?
+    // Pg, p_off: the arrays may be one slab of a line that continues on other devices (tf_penta_slab_*): local chunk p
+    // is chunk p_off + p of Pg.  Single device: Pg = P, p_off = 0.
+    const bool outside = dir ? (p_off + p < Pg - 1) : (p_off + p > 0);   // does this march have outside unknowns at its start?
     if (lane == 0) {
 #pragma unroll
         for (int s = 0; s < NST; ++s) mbar_init(full + s, 1);
@@ -155,7 +158,8 @@ penta_col_iface_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int 
 // 128-byte swizzle as in penta_row_fwd2_kernel.  grid (ceil(nrow/32), 2, P).  out: [P][2][IF_VALS][nrow].
 template <int NST>
 __global__ void __launch_bounds__(32)
-penta_row_iface_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int P, double* __restrict__ out)
+penta_row_iface_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int P, double* __restrict__ out,
+                       int Pg, int p_off)
 {
     constexpr int CS = 16;
     constexpr int TILE = 32 * CS * 8;
@@ -167,7 +171,7 @@ penta_row_iface_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int 
     const int dir = blockIdx.y, p = blockIdx.z;
     const int lo = chunk_lo(p, P, ncol), hi = chunk_lo(p + 1, P, ncol);
     const int ntile = (hi - lo + CS - 1) / CS;
-    const bool outside = dir ? (p < P - 1) : (p > 0);
+    const bool outside = dir ? (p_off + p < Pg - 1) : (p_off + p > 0);
     if (lane == 0) {
 #pragma unroll
         for (int s = 0; s < NST; ++s) mbar_init(full + s, 1);

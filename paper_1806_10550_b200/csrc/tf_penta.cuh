@@ -144,7 +144,8 @@ penta_row_bwd_kernel(int nrow, int ncol, const double* __restrict__ alT, const d
 template <int NST, int RS>
 __global__ void __launch_bounds__(32)
 penta_col_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int mid_arg, double* __restrict__ al,
-                      double* __restrict__ be, double* __restrict__ zz, int P, const double* __restrict__ X)
+                      double* __restrict__ be, double* __restrict__ zz, int P, const double* __restrict__ X,
+                      int Pg = 0, int p_off = 0)
 {
     extern __shared__ unsigned char raw[];
     unsigned char* base = align1024(raw);
@@ -160,8 +161,10 @@ penta_col_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int m
     const int jmin = dir ? mid : lo, jmax = dir ? hi : mid;
     const int nrows = jmax - jmin;
     double xfar = 0.0, xnear = 0.0;                          // known unknowns just outside this march's first row
-    if (P > 1 && (dir ? p < P - 1 : p > 0)) {
-        const double* xo = X + (size_t)(dir ? (p + 1) * 4 : (p - 1) * 4 + 2) * ncol + min(i, ncol - 1);
+    if (Pg == 0) Pg = P;                                     // single device; else local chunk p is chunk p_off + p of Pg
+    const int pg = p_off + p;
+    if (Pg > 1 && (dir ? pg < Pg - 1 : pg > 0)) {
+        const double* xo = X + (size_t)(dir ? (pg + 1) * 4 : (pg - 1) * 4 + 2) * ncol + min(i, ncol - 1);
         xfar = dir ? xo[ncol] : xo[0];
         xnear = dir ? xo[0] : xo[ncol];
     }
@@ -238,7 +241,8 @@ penta_col_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int m
 template <int NST>
 __global__ void __launch_bounds__(32)
 penta_row_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int mid_arg, double* __restrict__ alT,
-                      double* __restrict__ beT, double* __restrict__ zzT, int P, const double* __restrict__ X)
+                      double* __restrict__ beT, double* __restrict__ zzT, int P, const double* __restrict__ X,
+                      int Pg = 0, int p_off = 0)
 {
     constexpr int CS = 16;
     constexpr int TILE = 32 * CS * 8;                        // bytes per array tile (4 KiB, 1024-aligned)
@@ -253,8 +257,10 @@ penta_row_fwd2_kernel(const __grid_constant__ Maps6 M, int nrow, int ncol, int m
     const int mid = P > 1 ? chunk_mid(lo, hi) : mid_arg;
     const int imin = dir ? mid : lo, imax = dir ? hi : mid;
     double xfar = 0.0, xnear = 0.0;
-    if (P > 1 && (dir ? p < P - 1 : p > 0)) {
-        const double* xo = X + (size_t)(dir ? (p + 1) * 4 : (p - 1) * 4 + 2) * nrow + min(r0 + lane, nrow - 1);
+    if (Pg == 0) Pg = P;
+    const int pg = p_off + p;
+    if (Pg > 1 && (dir ? pg < Pg - 1 : pg > 0)) {
+        const double* xo = X + (size_t)(dir ? (pg + 1) * 4 : (pg - 1) * 4 + 2) * nrow + min(r0 + lane, nrow - 1);
         xfar = dir ? xo[nrow] : xo[0];
         xnear = dir ? xo[0] : xo[nrow];
     }

@@ -44,6 +44,10 @@ SYMBOLS = {
     "tf_penta_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int, ctypes.c_int]),
     "tf_penta_solve": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int] + [_vp] * 9),
     "tf_penta_partition_chunks": (ctypes.c_int, [ctypes.c_int] * 4),
+    "tf_penta_slab_interface_doubles": (ctypes.c_size_t, [ctypes.c_int] * 4),
+    "tf_penta_slab_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int] * 5),
+    "tf_penta_slab_interface": (ctypes.c_int, [ctypes.c_int] * 6 + [_vp] * 8),
+    "tf_penta_slab_solve": (ctypes.c_int, [ctypes.c_int] * 6 + [_vp] * 10),
     "tf_betti_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int] * 3),
     "tf_spectrum_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int] * 3),
     "tf_radial_peaks": (ctypes.c_int, [_dp, _dp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, _dp, _dp, _dp, ctypes.c_int,
@@ -359,3 +363,58 @@ def radial_peaks(q, zeta, per_interval=10, ngrid=400, max_peaks=64):
         _err(None, rc, "tf_radial_peaks")
     m = min(n.value, max_peaks)
     return g, f, list(zip(pq[:m].tolist(), pz[:m].tolist()))
+
+
+def _check_six(ts):
+    torch = _torch()
+    nrow, ncol = ts[0].shape
+    for t in ts:
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                and tuple(t.shape) == (nrow, ncol)):
+            raise ValueError("expected contiguous CUDA float64 tensors of one shape")
+    return nrow, ncol
+
+
+def penta_slab_interface(direction, nparts, slab, nslabs, e, c, d, a, b, rhs, stream=None):
+    """tf_penta_slab_interface on the local slab [nrow][ncol]: returns the local interface values, a CUDA float64 tensor
+    of shape [nparts, 2, 10, nsys] (nsys = ncol for direction 1, nrow for direction 0)."""
+    torch = _torch()
+    ts = (e, c, d, a, b, rhs)
+    nrow, ncol = _check_six(ts)
+    L = lib()
+    if L.tf_penta_slab_interface_doubles(nrow, ncol, direction, nparts) == 0:
+        raise ValueError("shape not admitted by the slab solver (see include/tf.h)")
+    nsys = ncol if direction == 1 else nrow
+    out = torch.empty((nparts, 2, 10, nsys), dtype=torch.float64, device=e.device)
+    st = (torch.cuda.current_stream(e.device) if stream is None else stream).cuda_stream
+    rc = L.tf_penta_slab_interface(nrow, ncol, direction, nparts, slab, nslabs, *[t.data_ptr() for t in ts], out.data_ptr(), st)
+    if rc != OK:
+        _err(None, rc, "tf_penta_slab_interface")
+    return out
+
+
+def penta_slab_solve(direction, nparts, slab, nslabs, e, c, d, a, b, rhs, iface_all, out=None, workspace=None, stream=None):
+    """tf_penta_slab_solve: iface_all = the interface values of all slabs in slab order, [nslabs * nparts, 2, 10, nsys]."""
+    torch = _torch()
+    ts = (e, c, d, a, b, rhs)
+    nrow, ncol = _check_six(ts)
+    nsys = ncol if direction == 1 else nrow
+    if not (iface_all.is_cuda and iface_all.dtype == torch.float64 and iface_all.is_contiguous()
+            and iface_all.numel() == nslabs * nparts * 20 * nsys):
+        raise ValueError("iface_all must be a contiguous CUDA float64 tensor of nslabs * nparts * 20 * nsys values")
+    L = lib()
+    need = L.tf_penta_slab_workspace_bytes(nrow, ncol, direction, nparts, nslabs)
+    if need == 0:
+        raise ValueError("shape not admitted by the slab solver (see include/tf.h)")
+    if out is None:
+        out = torch.empty_like(e)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=e.device)
+    if workspace.numel() * workspace.element_size() < need or workspace.data_ptr() % 256:
+        raise ValueError("workspace too small or not 256-byte aligned")
+    st = (torch.cuda.current_stream(e.device) if stream is None else stream).cuda_stream
+    rc = L.tf_penta_slab_solve(nrow, ncol, direction, nparts, slab, nslabs, *[t.data_ptr() for t in ts], iface_all.data_ptr(),
+                               out.data_ptr(), workspace.data_ptr(), st)
+    if rc != OK:
+        _err(None, rc, "tf_penta_slab_solve")
+    return out
