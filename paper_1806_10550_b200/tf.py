@@ -130,7 +130,11 @@ class ThinFilm:
             self._h = _vp()
             self._ws = None
 
-    __del__ = close
+    def __del__(self):
+        try:                       # at interpreter shutdown module globals may already be gone
+            self.close()
+        except Exception:
+            pass
 
     def set_newton(self, tol=1e-10, max_iter=10, fixed_iters=0):
         st = lib().tf_set_newton(self._h, tol, max_iter, fixed_iters)
