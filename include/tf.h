@@ -138,6 +138,24 @@ tf_status tf_adaptive_run(tf_step_fn step, void* user, tf_adaptive* ctl, int n_a
 tf_status tf_advance_adaptive(tf_ctx* ctx, tf_adaptive* ctl, int n_accept, int max_attempts,
                               double* t_advanced, tf_step_record* hist, int hist_cap, int* nhist);
 
+/*
+ * The rows of the path one at a time, for callers that put an exchange step between the sweeps (a film distributed over
+ * several devices).  tf_step is: for k = 0, 1, ...: tf_sweep(ctx, dt, k, 3); decide on
+ * tf_residual(ctx, k); on acceptance tf_accept(ctx).
+ *   tf_field     device address of a field the context owns: 0 = u^n (the state), 1 = the iterate buffer (u_(k) for
+ *                k >= 1 on input of a sweep, u_(k+1) on output of the x-sweep), 2 = b^n, 3 = w.  The addresses of 0 and
+ *                1 swap on tf_accept / an accepted tf_step: ask again afterwards.
+ *   tf_sweep     which = 1: y-sweep of iteration k (S1-S4; reads field 0 if k == 0 else field 1, and b^n; k == 0 also
+ *                writes b^n; writes w); which = 2: x-sweep (S5-S7; reads the same source field and w; writes field 1 and
+ *                the residual record of iteration k); which = 3: both.  Enqueues only.
+ *   tf_residual  (2.22) of iteration k and the bad-iterate flag; synchronises the stream.
+ *   tf_accept    u^{n+1} = u_(k+1): swaps fields 0 and 1.
+ */
+tf_status tf_field(tf_ctx* ctx, int which, double** dev_ptr);
+tf_status tf_sweep(tf_ctx* ctx, double dt, int k, int which);
+tf_status tf_residual(tf_ctx* ctx, int k, double* res, int* bad);
+tf_status tf_accept(tf_ctx* ctx);
+
 /* mass = dx*dy*sum(h)  ((3.2), times the domain area); fixed-order fp64 tree. */
 tf_status tf_mass(tf_ctx* ctx, double* mass);
 

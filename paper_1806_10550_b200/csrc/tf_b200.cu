@@ -281,8 +281,9 @@ cudaError_t launch_xfwd(tf_ctx* c, const Params& P, const Dir& DX, const double*
 
 // one pseudo-Newton iteration k: reads src (u^n if k == 0 else uk), writes uk, red[2k..2k+1].  gated: the four
 // kernels return at once if iteration k-1's record says the step is already decided (speculative launch-ahead).
+// which: 1 = the y-sweep (S1-S4: y forward + y backward -> w), 2 = the x-sweep (S5-S7 -> uk, red[2k]), 3 = both
 template <int N, int M>
-cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated)
+cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, int which = 3)
 {
     const Params& P = c->P;
     const Gate gate = (gated && k > 0) ? Gate{c->red + 2 * (k - 1), c->tol} : Gate{nullptr, 0.0};
@@ -292,7 +293,7 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated)
     const int nstrip = (P.nx + YW_VALID - 1) / YW_VALID;
     cudaEvent_t* ev = (c->profiling && slot >= 0) ? c->ev + 5 * slot : nullptr;
     if (ev) cudaEventRecord(ev[0], c->stream);
-    {
+    if (which & 1) {
         const CUtensorMap& mu = c->mUy[src == c->ubuf[0] ? 0 : 1];
         const int tma = c->tma_yf ? 1 : 0;
         cudaError_t e;
@@ -305,30 +306,32 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated)
         if (e != cudaSuccess) return e;
     }
     if (ev) cudaEventRecord(ev[1], c->stream);
-    cudaError_t le = launch_ybwd2(c->mY, c->tma_y, P.nx, P.ny, c->mid_y, c->al, c->be, c->zz, c->w, c->stream, gate);
+    cudaError_t le = cudaSuccess;
+    if (which & 1) le = launch_ybwd2(c->mY, c->tma_y, P.nx, P.ny, c->mid_y, c->al, c->be, c->zz, c->w, c->stream, gate);
     if (le != cudaSuccess) return le;
     if (ev) cudaEventRecord(ev[2], c->stream);
-    {
+    if (which & 2) {
         const int nblk = (P.ny + XW_R - 1) / XW_R;
         cudaError_t e = nblk > c->num_sms ? launch_xfwd<N, M, 4>(c, P, DX, src, (nblk + 1) / 2, gate)
                                           : launch_xfwd<N, M, 2>(c, P, DX, src, nblk, gate);
         if (e != cudaSuccess) return e;
     }
     if (ev) cudaEventRecord(ev[3], c->stream);
-    le = launch_xbwd2(c->mX, c->mU[src == c->ubuf[0] ? 0 : 1], c->mU[c->uk == c->ubuf[0] ? 0 : 1], c->tma_x, P.nx, P.ny,
-                      c->mid_x, c->al, c->be, c->zz, src, c->uk, c->red + 2 * k, c->stream, gate);
+    if (which & 2)
+        le = launch_xbwd2(c->mX, c->mU[src == c->ubuf[0] ? 0 : 1], c->mU[c->uk == c->ubuf[0] ? 0 : 1], c->tma_x, P.nx, P.ny,
+                          c->mid_x, c->al, c->be, c->zz, src, c->uk, c->red + 2 * k, c->stream, gate);
     if (le != cudaSuccess) return le;
     if (ev) cudaEventRecord(ev[4], c->stream);
-    count_launch(4);
+    count_launch((which & 1 ? 2 : 0) + (which & 2 ? 2 : 0));
     return cudaGetLastError();
 }
 
-cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated)
+cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, int which = 3)
 {
-    if (c->model == TF_PI_NLC) return launch_iteration<MODEL_NLC, 0>(c, s, k, slot, gated);
-    if (c->model == TF_PI_POLYMER) return launch_iteration<MODEL_POLYMER, 0>(c, s, k, slot, gated);
-    if (c->P.n == 3 && c->P.m == 2) return launch_iteration<3, 2>(c, s, k, slot, gated);
-    return launch_iteration<0, 0>(c, s, k, slot, gated);
+    if (c->model == TF_PI_NLC) return launch_iteration<MODEL_NLC, 0>(c, s, k, slot, gated, which);
+    if (c->model == TF_PI_POLYMER) return launch_iteration<MODEL_POLYMER, 0>(c, s, k, slot, gated, which);
+    if (c->P.n == 3 && c->P.m == 2) return launch_iteration<3, 2>(c, s, k, slot, gated, which);
+    return launch_iteration<0, 0>(c, s, k, slot, gated, which);
 }
 
 // after a stream sync: fold the event intervals of `niter` profiled iterations into the totals
@@ -784,6 +787,45 @@ tf_status tf_step(tf_ctx* c, double dt, int* newton_iters, double* residual)
     if (newton_iters) *newton_iters = k;
     if (residual) *residual = res;
     return status;
+}
+
+// ---- the rows of the path one by one (for callers that put an exchange step between the sweeps: section 8 of DESIGN.md)
+tf_status tf_field(tf_ctx* c, int which, double** dev_ptr)
+{
+    if (!c || !dev_ptr) return TF_ERR_INVALID_ARG;
+    double* f[4] = {c->u, c->uk, c->bn, c->w};
+    if (which < 0 || which > 3) return fail(c, TF_ERR_INVALID_ARG, "tf_field: which in 0..3");
+    *dev_ptr = f[which];
+    return TF_OK;
+}
+
+tf_status tf_sweep(tf_ctx* c, double dt, int k, int which)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    if (!(dt > 0) || !std::isfinite(dt)) return fail(c, TF_ERR_INVALID_ARG, "dt must be positive and finite");
+    if (k < 0 || k >= MAX_ITERS || which < 1 || which > 3) return fail(c, TF_ERR_INVALID_ARG, "tf_sweep: k in [0,4096), which in 1..3");
+    if (!c->have_state) return fail(c, TF_ERR_STATE, "no state set");
+    if (which & 2) TF_CUDA(c, cudaMemsetAsync(c->red + 2 * k, 0, 2 * sizeof(double), c->stream));
+    TF_CUDA(c, launch_iteration(c, 0.5 * dt, k, -1, false, which));
+    return TF_OK;
+}
+
+tf_status tf_residual(tf_ctx* c, int k, double* res, int* bad)
+{
+    if (!c || k < 0 || k >= MAX_ITERS) return TF_ERR_INVALID_ARG;
+    TF_CUDA(c, cudaMemcpyAsync(c->pinned, c->red + 2 * k, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    TF_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (res) *res = c->pinned[0];
+    if (bad) *bad = (c->pinned[1] != 0.0 || c->pinned[0] != c->pinned[0]) ? 1 : 0;
+    return TF_OK;
+}
+
+tf_status tf_accept(tf_ctx* c)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    if (!c->have_state) return fail(c, TF_ERR_STATE, "no state set");
+    std::swap(c->u, c->uk);
+    return TF_OK;
 }
 
 tf_status tf_mass(tf_ctx* c, double* mass)

@@ -1,0 +1,169 @@
+"""The time step with the film spread over the ranks of a torch.distributed group.
+
+Classic ADI decomposition: the x-sweep runs on ROW blocks (its lines are rows: nothing to exchange), the y-sweep on
+COLUMN blocks (its lines are columns), and the field is redistributed between the two layouts, one all-to-all each way
+per Newton iteration:
+
+    rank r:   ctx_y = film of [ny] x [columns i0_r-2 .. i1_r+2)     (two halo columns per side: the 13-point operator
+                                                                      of the y-sweep's right-hand side reaches i +- 2)
+              ctx_x = film of [rows j0_r .. j1_r) x [nx]
+    k = 0, 1, ...:
+        ctx_y: y-sweep of iteration k            (S1-S4 of DESIGN.md; tf_sweep(.., which = 1))  -> w   [column block]
+        all-to-all: w -> row blocks
+        ctx_x: x-sweep of iteration k            (S5-S7; tf_sweep(.., which = 2))               -> u_(k+1), residual
+        all-to-all: u_(k+1) -> column blocks with halos (reflection at the domain's own edges)
+        all-reduce (max) of the residual record; accept / iterate / reject on every rank alike
+
+Both contexts are ordinary single-device contexts: ctx_y simply is a film that is four columns wider than the block it
+owns, and whatever the kernels compute in those halo columns is never used.  At a domain edge the halo holds the
+reflected values, so the flux through the boundary face is zero to rounding instead of exactly zero; everything else
+is the arithmetic of the single-device path (parity with it to 1e-11, not bit for bit).
+
+The collectives go through a small `comm` object (all_to_all of flat buffers with split sizes, all_reduce max / sum):
+TorchComm wraps a torch.distributed group (NCCL over NVLink on GPUs); tests pass an in-process stand-in.
+Packing and unpacking of the blocks are strided tensor copies (memory movement only; all arithmetic of the path
+stays in the library's kernels).
+"""
+import numpy as np
+
+from .dist import slab_bounds
+
+
+class TorchComm:
+    def __init__(self, group=None):
+        import torch.distributed as dist
+        self.dist, self.group = dist, group
+        self.world, self.rank = dist.get_world_size(group), dist.get_rank(group)
+
+    def all_to_all(self, send, send_counts, recv_counts):
+        import torch
+        recv = torch.empty(int(sum(recv_counts)), dtype=send.dtype, device=send.device)
+        self.dist.all_to_all_single(recv, send, list(map(int, recv_counts)), list(map(int, send_counts)), group=self.group)
+        return recv
+
+    def all_reduce(self, t, op):
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX if op == "max" else self.dist.ReduceOp.SUM, group=self.group)
+        return t
+
+
+class Layout:
+    """who owns what: row blocks [j0, j1) and column blocks [i0, i1) of every rank, and the halo'd column range"""
+    HALO = 2
+
+    def __init__(self, nx, ny, world):
+        self.nx, self.ny, self.world = nx, ny, world
+        self.rows = [slab_bounds(ny, world, r) for r in range(world)]
+        self.cols = [slab_bounds(nx, world, r) for r in range(world)]
+
+    def halo_cols(self, r):
+        """global columns rank r receives for its column block: its own plus up to HALO neighbours per side"""
+        i0, i1 = self.cols[r]
+        return max(i0 - self.HALO, 0), min(i1 + self.HALO, self.nx)
+
+    def local_width(self, r):
+        return self.cols[r][1] - self.cols[r][0] + 2 * self.HALO
+
+
+def rows_to_cols(lay, r, comm, f_rows, f_cols):
+    """f_rows: [ny_loc][nx] of rank r  ->  f_cols: [ny][nxl + 4] of rank r, halos included (reflection at domain edges)"""
+    import torch
+    pieces, scount, rcount = [], [], []
+    for q in range(lay.world):
+        a, b = lay.halo_cols(q)
+        pieces.append(f_rows[:, a:b].reshape(-1))
+        scount.append(pieces[-1].numel())
+    a, b = lay.halo_cols(r)
+    for p in range(lay.world):
+        rcount.append((lay.rows[p][1] - lay.rows[p][0]) * (b - a))
+    recv = comm.all_to_all(torch.cat(pieces), scount, rcount)
+    off = a - (lay.cols[r][0] - lay.HALO)                       # local column of global column a (2 at the left domain edge)
+    pos = 0
+    for p in range(lay.world):
+        j0, j1 = lay.rows[p]
+        f_cols[j0:j1, off:off + (b - a)] = recv[pos:pos + rcount[p]].view(j1 - j0, b - a)
+        pos += rcount[p]
+    n = lay.cols[r][1] - lay.cols[r][0]
+    if r == 0:                                                   # h_{-1} = h_0, h_{-2} = h_1
+        f_cols[:, 1] = f_cols[:, 2]
+        f_cols[:, 0] = f_cols[:, 3]
+    if r == lay.world - 1:                                       # h_{nx} = h_{nx-1}, h_{nx+1} = h_{nx-2}
+        f_cols[:, n + 2] = f_cols[:, n + 1]
+        f_cols[:, n + 3] = f_cols[:, n]
+
+
+def cols_to_rows(lay, r, comm, f_cols, f_rows):
+    """interior of f_cols [ny][nxl + 4] of rank r  ->  f_rows [ny_loc][nx] of rank r"""
+    import torch
+    n = lay.cols[r][1] - lay.cols[r][0]
+    pieces, scount, rcount = [], [], []
+    for q in range(lay.world):
+        j0, j1 = lay.rows[q]
+        pieces.append(f_cols[j0:j1, lay.HALO:lay.HALO + n].reshape(-1))
+        scount.append(pieces[-1].numel())
+    j0, j1 = lay.rows[r]
+    for p in range(lay.world):
+        rcount.append((j1 - j0) * (lay.cols[p][1] - lay.cols[p][0]))
+    recv = comm.all_to_all(torch.cat(pieces), scount, rcount)
+    pos = 0
+    for p in range(lay.world):
+        i0, i1 = lay.cols[p]
+        f_rows[:, i0:i1] = recv[pos:pos + rcount[p]].view(j1 - j0, i1 - i0)
+        pos += rcount[p]
+
+
+class DistributedFilm:
+    """tf_step for a film spread over the ranks of `comm`; every rank constructs it with the same arguments."""
+
+    def __init__(self, nx, ny, dx, dy, kappa=100.0, hstar=0.1, n=3, m=2, comm=None, tol=1e-10, max_iter=10):
+        from . import tf
+        self.tf = tf
+        self.comm = comm if comm is not None else TorchComm()
+        self.rank, self.world = self.comm.rank, self.comm.world
+        self.lay = Layout(nx, ny, self.world)
+        self.nx, self.ny, self.dx, self.dy = nx, ny, dx, dy
+        self.tol, self.max_iter = tol, max_iter
+        j0, j1 = self.lay.rows[self.rank]
+        self.ctx_x = tf.ThinFilm(nx, j1 - j0, dx, dy, kappa, hstar, n, m)
+        self.ctx_y = tf.ThinFilm(self.lay.local_width(self.rank), ny, dx, dy, kappa, hstar, n, m)
+
+    def set_state_rows(self, h_rows):
+        """h_rows: this rank's row block [ny_loc][nx] (numpy or CUDA tensor); distributes the column layout too"""
+        import torch
+        self.ctx_x.set_state(h_rows)
+        tmp = torch.ones(self.ny, self.lay.local_width(self.rank), dtype=torch.float64, device="cuda")
+        rows_to_cols(self.lay, self.rank, self.comm, self.ctx_x.field(self.ctx_x.FIELD_STATE), tmp)
+        self.ctx_y.set_state(tmp)
+
+    def get_state_rows(self):
+        return self.ctx_x.get_state()
+
+    def step(self, dt):
+        """returns (status, newton_iters, residual) like ThinFilm.step; on rejection the state is unchanged"""
+        import torch
+        tf, cx, cy = self.tf, self.ctx_x, self.ctx_y
+        rec = torch.zeros(2, dtype=torch.float64, device="cuda")
+        k, res, status = 0, 0.0, tf.NOT_CONVERGED
+        while k < self.max_iter:
+            cy.sweep(dt, k, cy.SWEEP_Y)
+            cols_to_rows(self.lay, self.rank, self.comm, cy.field(cy.FIELD_W), cx.field(cx.FIELD_W))
+            cx.sweep(dt, k, cx.SWEEP_X)
+            rows_to_cols(self.lay, self.rank, self.comm, cx.field(cx.FIELD_ITERATE), cy.field(cy.FIELD_ITERATE))
+            r, bad = cx.residual(k)
+            rec[0], rec[1] = (float("inf") if r != r else r), float(bad)
+            self.comm.all_reduce(rec, "max")
+            res, bad = float(rec[0]), bool(rec[1] != 0)
+            k += 1
+            if bad or not np.isfinite(res):
+                break
+            if res < self.tol:
+                status = tf.OK
+                break
+        if status == tf.OK:
+            cx.accept()
+            cy.accept()
+        return status, k, res
+
+    def mass(self):
+        import torch
+        t = torch.tensor([self.ctx_x.mass()], dtype=torch.float64, device="cuda")
+        return float(self.comm.all_reduce(t, "sum")[0])

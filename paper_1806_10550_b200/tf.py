@@ -41,6 +41,10 @@ SYMBOLS = {
     "tf_get_state": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
     "tf_step": (ctypes.c_int, [_vp, ctypes.c_double, ctypes.POINTER(ctypes.c_int), _dp]),
     "tf_mass": (ctypes.c_int, [_vp, _dp]),
+    "tf_field": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.POINTER(_vp)]),
+    "tf_sweep": (ctypes.c_int, [_vp, ctypes.c_double, ctypes.c_int, ctypes.c_int]),
+    "tf_residual": (ctypes.c_int, [_vp, ctypes.c_int, _dp, ctypes.POINTER(ctypes.c_int)]),
+    "tf_accept": (ctypes.c_int, [_vp]),
     "tf_penta_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int, ctypes.c_int]),
     "tf_penta_solve": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int] + [_vp] * 9),
     "tf_penta_partition_chunks": (ctypes.c_int, [ctypes.c_int] * 4),
@@ -184,6 +188,41 @@ class ThinFilm:
         if st < 0:
             _err(self._h, st, "tf_step")
         return st, it.value, res.value
+
+    # ---- the rows of the path one at a time (tf_field / tf_sweep / tf_residual / tf_accept)
+    FIELD_STATE, FIELD_ITERATE, FIELD_BN, FIELD_W = 0, 1, 2, 3
+    SWEEP_Y, SWEEP_X = 1, 2
+
+    def field(self, which):
+        """a torch view [ny][nx] of a field the context owns (no copy; the addresses of 0 and 1 swap on accept)"""
+        torch = _torch()
+        p = _vp()
+        st = lib().tf_field(self._h, int(which), ctypes.byref(p))
+        if st != OK:
+            _err(self._h, st, "tf_field")
+        n = self.nx * self.ny
+        if self._ws is not None:
+            off = (p.value - self._ws.data_ptr()) // 8
+            if 0 <= off and off + n <= self._ws.numel() * self._ws.element_size() // 8:
+                return self._ws.view(torch.float64)[off:off + n].view(self.ny, self.nx)
+        raise TfError(ERR_STATE, "tf_field", "field views need a context created on a torch workspace")
+
+    def sweep(self, dt, k, which):
+        st = lib().tf_sweep(self._h, dt, k, which)
+        if st != OK:
+            _err(self._h, st, "tf_sweep")
+
+    def residual(self, k):
+        res, bad = ctypes.c_double(0.0), ctypes.c_int(0)
+        st = lib().tf_residual(self._h, k, ctypes.byref(res), ctypes.byref(bad))
+        if st != OK:
+            _err(self._h, st, "tf_residual")
+        return res.value, bool(bad.value)
+
+    def accept(self):
+        st = lib().tf_accept(self._h)
+        if st != OK:
+            _err(self._h, st, "tf_accept")
 
     def mass(self):
         m = ctypes.c_double(0.0)

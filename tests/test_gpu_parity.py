@@ -289,3 +289,44 @@ def test_solution_criterion_and_native_controller_against_the_flow_chart(tf, tfo
     g.set_solution_criteria(0.0)
     g.set_state(h)
     assert g.step(1e-2)[0] == tf.OK
+
+
+# ------------------------------------------------------------------ the rows of the path one at a time
+@pytest.mark.parametrize("nx,ny", [(128, 96), (61, 45)])
+def test_sweeps_driven_one_by_one_equal_tf_step(tf, nx, ny):
+    """tf_sweep (y, then x) / tf_residual / tf_accept reproduce tf_step bit for bit, and the field views alias the
+    context's buffers (w of the y-sweep can be overwritten between the sweeps: the x-sweep then solves with it)."""
+    import torch
+    h0 = inputs.noise_ic(nx, ny, seed=17)
+    a = tf.ThinFilm(nx, ny, 0.4259, 0.4259, K, HS, 3, 2)
+    b = tf.ThinFilm(nx, ny, 0.4259, 0.4259, K, HS, 3, 2)
+    a.set_newton(1e-10, 64, 0)
+    for g in (a, b):
+        g.set_state(h0)
+    for step in range(3):
+        st, its, res = a.step(1e-2)
+        assert st == tf.OK
+        k, r = 0, None
+        while True:
+            b.sweep(1e-2, k, b.SWEEP_Y)
+            b.sweep(1e-2, k, b.SWEEP_X)
+            r, bad = b.residual(k)
+            k += 1
+            assert not bad
+            if r < 1e-10:
+                break
+        b.accept()
+        assert (k, r) == (its, res)
+        assert np.array_equal(a.get_state(), b.get_state())
+    # the views: state view equals get_state; scaling w between the sweeps scales the correction v = u_1 - u_0 (linear solve)
+    u = b.field(b.FIELD_STATE).clone()
+    assert np.array_equal(u.cpu().numpy(), b.get_state())
+    b.sweep(1e-2, 0, b.SWEEP_Y)
+    b.sweep(1e-2, 0, b.SWEEP_X)
+    v1 = (b.field(b.FIELD_ITERATE) - u).clone()
+    b.sweep(1e-2, 0, b.SWEEP_Y)
+    b.field(b.FIELD_W).mul_(0.5)
+    b.sweep(1e-2, 0, b.SWEEP_X)
+    v2 = b.field(b.FIELD_ITERATE) - u
+    torch.cuda.synchronize()
+    assert float((v2 - 0.5 * v1).abs().max()) <= 1e-13 * float(v1.abs().max())
