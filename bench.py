@@ -48,6 +48,9 @@ def parse():
     ap.add_argument("--slabs", action="store_true",
                     help="config 4 only: every system spread over the ranks (paper_1806_10550_b200/dist.py: one NCCL "
                          "all-gather of the interface values); strong scaling, launch with torchrun for --gpus N > 1")
+    ap.add_argument("--distributed", action="store_true",
+                    help="ONE film spread over the ranks (paper_1806_10550_b200/dist_step.py: two all-to-alls and one "
+                         "all-reduce per Newton iteration) instead of one replica per rank; strong scaling")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -370,6 +373,50 @@ def cusparse_gpsv_interleaved(e, c, d, a, b, y, steps):
 
 
 # ----------------------------------------------------------------------------------------- config 4 (side measurement)
+def run_distributed(args, cfg):
+    """The headline workload as ONE film over all ranks: strong scaling, max over ranks."""
+    import torch
+    import torch.distributed as dist
+    from paper_1806_10550_b200 import dist_step as ds
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    own_group = not dist.is_initialized()
+    if own_group:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29532")
+        dist.init_process_group("nccl", rank=rank, world_size=world)
+    nx, ny, dt = cfg["nx"], cfg["ny"], cfg["dt"]
+    f = ds.DistributedFilm(nx, ny, cfg["dx"], cfg["dy"], cfg["kappa"], cfg["hstar"], cfg["n"], cfg["m"], tol=cfg["tol"],
+                           max_iter=cfg["max_iter"])
+    j0, j1 = f.lay.rows[rank]
+    f.set_state_rows(inputs.initial_condition(cfg)[j0:j1].copy())
+    for _ in range(args.warmup):
+        f.step(dt)
+    dist.barrier()
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    iters = 0
+    for _ in range(args.steps):
+        st, k, _ = f.step(dt)
+        iters += k
+    ev1.record()
+    torch.cuda.synchronize()
+    dist.barrier()
+    sec = max_over_ranks(ev0.elapsed_time(ev1) * 1e-3, world, "cuda")
+    if rank == 0:
+        print(json.dumps({"metric": "grid-point ADI steps/sec (fp64)", "value": nx * ny * args.steps / sec,
+                          "unit": "grid-point-steps/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                          "ms_per_step": sec * 1e3 / args.steps, "higher_is_better": True, "scaling": "strong",
+                          "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                          "config": {"workload": cfg["name"], "grid": [nx, ny], "dt": dt, "tol": cfg["tol"],
+                                     "parallelism": f"one film over {world} ranks: row blocks (x-sweep) / column blocks "
+                                                    "(y-sweep), 2 all-to-alls + 1 all-reduce per Newton iteration"},
+                          "newton_iters_total": iters, "gpu_launches": 4 * iters}), flush=True)
+    if own_group:
+        dist.destroy_process_group()
+
+
 def run_penta_slabs(args, cfg):
     """Config 4 with every system cut into one slab of rows per rank (direction 1: systems = columns): the slab solver
     of DESIGN.md section 8 -- interface pass, NCCL all-gather of 20 * nparts doubles per system and rank, reduced +
@@ -501,6 +548,8 @@ def main():
             {"impl": "reference", "unavailable": "config 4 is a side measurement of the B200 arm only"}))
     if args.impl == "reference":
         run_reference(args, cfg)
+    elif args.distributed:
+        run_distributed(args, cfg)
     else:
         run_b200(args, cfg)
 
