@@ -35,7 +35,7 @@ def single(tf, h0, dx, dy, dts):
     return log, g.get_state(), g.mass()
 
 
-@pytest.mark.parametrize("world,nx,ny", [(2, 128, 96), (3, 208, 160), (4, 256, 130)])
+@pytest.mark.parametrize("world,nx,ny", [(2, 128, 96), (3, 208, 160), (4, 256, 130), (2, 2048, 1536)])
 def test_ranks_as_threads_equal_the_single_device_step(tf, world, nx, ny):
     import local_comm
     from paper_1806_10550_b200 import dist_step as ds
