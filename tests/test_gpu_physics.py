@@ -1,0 +1,88 @@
+"""The CUDA path against what the paper and the mathematics fix, WITHOUT the oracle in between (the same checks that
+pin the oracle, tests/test_oracle_pins.py, here applied to the product): the growth rate of a single Fourier mode against
+the dispersion relation (1.4), second order in time, conservation of mass
+(PAPER.md:348-360), the fixed point and the transpose symmetry of the scheme."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1806_10550_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+K, HS, N_, M_ = 100.0, 0.1, 3, 2
+
+
+@pytest.fixture(scope="module")
+def tf():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1806_10550_b200 import tf as tfmod
+    tfmod.lib()
+    return tfmod
+
+
+@pytest.mark.parametrize("direction", [0, 1])
+@pytest.mark.parametrize("k", [1, 2, 3])
+def test_growth_rate_of_a_single_mode(tf, direction, k):
+    """k = 1, 2: unstable modes (q = q_m/2 and q_m): within 1 % of sigma(q) = -h0^3 (q^4 - Pi'(h0) q^2) and within 2e-4 of
+    the exact Crank-Nicolson amplification of the discrete symbol; k = 3: q = 1.5 q_m > q_c, the mode decays."""
+    h0, eps, npts, nsteps = 1.0, 1e-4, 32, 400
+    P1 = K * (M_ * HS**M_ / h0**(M_ + 1) - N_ * HS**N_ / h0**(N_ + 1))
+    L = inputs.LAMBDA_M
+    d = L / npts
+    q = k * math.pi / L
+    sigma = -h0**3 * (q**4 - P1 * q**2)
+    T = math.log(1.3) / abs(sigma)
+    dt = T / nsteps
+    nx, ny = (npts, 6) if direction == 0 else (6, npts)
+    g = tf.ThinFilm(nx, ny, d, d, K, HS, N_, M_)
+    g.set_newton(1e-14, 200, 0)
+    mode = np.cos(k * math.pi * (np.arange(npts) + 0.5) * d / L)
+    shape = mode[None, :] if direction == 0 else mode[:, None]
+    g.set_state(h0 * (1 + eps * shape) * np.ones((ny, nx)))
+    for _ in range(nsteps):
+        assert g.step(dt)[0] == 0
+    dev = g.get_state() / h0 - 1.0
+    amp = (dev * shape).sum() / ((shape * np.ones((ny, nx))) ** 2).sum()
+    sigma_num = math.log(amp / eps) / T
+    q2t = (4.0 / d**2) * math.sin(q * d / 2) ** 2
+    sig_d = -h0**3 * (q2t**2 - P1 * q2t)
+    sigma_cn = math.log((1 + sig_d * dt / 2) / (1 - sig_d * dt / 2)) / dt
+    assert (sigma > 0) == (k < 3) and (sigma_num > 0) == (k < 3)
+    if k < 3:
+        assert abs(sigma_num - sigma) / abs(sigma) <= 1e-2
+    assert abs(sigma_num - sigma_cn) / abs(sigma_cn) <= 2e-4
+
+
+def test_second_order_in_time_mass_fixed_point_symmetry(tf):
+    nx = ny = 32
+    dx = dy = 2 * inputs.LAMBDA_M / nx
+    h = inputs.cosine_ic(nx, ny, dx, dy, kx=4, ky=2, h0=1.0, eps=0.1)
+    T, sols, m0 = 0.04, [], None
+    for lev in range(5):
+        g = tf.ThinFilm(nx, ny, dx, dy, K, HS, N_, M_)
+        g.set_newton(1e-14, 2000, 0)
+        g.set_state(h)
+        m0 = g.mass()
+        for _ in range(2 ** lev):
+            assert g.step(T / 2 ** lev)[0] == 0
+        assert abs(g.mass() - m0) <= 1e-13 * m0                          # (3.2): mass is conserved
+        sols.append(g.get_state())
+    err = [np.sqrt(np.mean((s - sols[-1]) ** 2)) for s in sols[:-1]]
+    orders = [math.log2(err[i] / err[i + 1]) for i in range(len(err) - 1)]
+    assert all(1.9 <= p <= 2.6 for p in orders), orders
+    # a flat film is a fixed point: one iteration, zero residual, unchanged bit for bit
+    g = tf.ThinFilm(48, 40, 0.4, 0.4, K, HS, N_, M_)
+    flat = np.full((40, 48), 0.7)
+    g.set_state(flat)
+    assert g.step(1e-2) == (0, 1, 0.0) and np.array_equal(g.get_state(), flat)
+    # the converged step of the transposed film (dx <-> dy) is the transpose of the converged step
+    ha = inputs.cosine_ic(40, 56, 0.3, 0.35, kx=3, ky=2, h0=1.0, eps=0.1)
+    a = tf.ThinFilm(40, 56, 0.3, 0.35, K, HS, N_, M_)
+    b = tf.ThinFilm(56, 40, 0.35, 0.3, K, HS, N_, M_)
+    for g_, h_ in ((a, ha), (b, np.ascontiguousarray(ha.T))):
+        g_.set_newton(1e-14, 500, 0)
+        g_.set_state(h_)
+        assert g_.step(5e-3)[0] == 0
+    assert np.max(np.abs(a.get_state() - b.get_state().T)) <= 1e-12 * np.max(np.abs(ha))
