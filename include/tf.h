@@ -143,11 +143,15 @@ tf_status tf_advance_adaptive(tf_ctx* ctx, tf_adaptive* ctl, int n_accept, int m
  * several devices).  tf_step is: for k = 0, 1, ...: tf_sweep(ctx, dt, k, 3); decide on
  * tf_residual(ctx, k); on acceptance tf_accept(ctx).
  *   tf_field     device address of a field the context owns: 0 = u^n (the state), 1 = the iterate buffer (u_(k) for
- *                k >= 1 on input of a sweep, u_(k+1) on output of the x-sweep), 2 = b^n, 3 = w.  The addresses of 0 and
- *                1 swap on tf_accept / an accepted tf_step: ask again afterwards.
+ *                k >= 1 on input of a sweep, u_(k+1) on output of the x-sweep), 2 = b^n, 3 = w; 4 = the residual records,
+ *                2 doubles {res, bad} per iteration, 4096 iterations.  The addresses of 0 and 1 swap on tf_accept / an
+ *                accepted tf_step: ask again afterwards.
  *   tf_sweep     which = 1: y-sweep of iteration k (S1-S4; reads field 0 if k == 0 else field 1, and b^n; k == 0 also
  *                writes b^n; writes w); which = 2: x-sweep (S5-S7; reads the same source field and w; writes field 1 and
- *                the residual record of iteration k); which = 3: both.  Enqueues only.
+ *                the residual record of iteration k); which = 3: both.  Adding 4 gates the sweep on the record of
+ *                iteration k-1 (k >= 1): its kernels return at once if that record says res < tol, bad iterate or NaN --
+ *                a caller that launches iterations ahead of its decisions (tf_set_launch_ahead does the same inside
+ *                tf_step) and, across devices, writes the all-reduced record back into field 4 first.  Enqueues only.
  *   tf_residual  (2.22) of iteration k and the bad-iterate flag; synchronises the stream.
  *   tf_accept    u^{n+1} = u_(k+1): swaps fields 0 and 1.
  */

@@ -793,8 +793,8 @@ tf_status tf_step(tf_ctx* c, double dt, int* newton_iters, double* residual)
 tf_status tf_field(tf_ctx* c, int which, double** dev_ptr)
 {
     if (!c || !dev_ptr) return TF_ERR_INVALID_ARG;
-    double* f[4] = {c->u, c->uk, c->bn, c->w};
-    if (which < 0 || which > 3) return fail(c, TF_ERR_INVALID_ARG, "tf_field: which in 0..3");
+    double* f[5] = {c->u, c->uk, c->bn, c->w, c->red};
+    if (which < 0 || which > 4) return fail(c, TF_ERR_INVALID_ARG, "tf_field: which in 0..4");
     *dev_ptr = f[which];
     return TF_OK;
 }
@@ -803,10 +803,11 @@ tf_status tf_sweep(tf_ctx* c, double dt, int k, int which)
 {
     if (!c) return TF_ERR_INVALID_ARG;
     if (!(dt > 0) || !std::isfinite(dt)) return fail(c, TF_ERR_INVALID_ARG, "dt must be positive and finite");
-    if (k < 0 || k >= MAX_ITERS || which < 1 || which > 3) return fail(c, TF_ERR_INVALID_ARG, "tf_sweep: k in [0,4096), which in 1..3");
+    if (k < 0 || k >= MAX_ITERS || (which & 3) == 0 || which > 7)
+        return fail(c, TF_ERR_INVALID_ARG, "tf_sweep: k in [0,4096), which = 1, 2 or 3, + 4 for the gate");
     if (!c->have_state) return fail(c, TF_ERR_STATE, "no state set");
     if (which & 2) TF_CUDA(c, cudaMemsetAsync(c->red + 2 * k, 0, 2 * sizeof(double), c->stream));
-    TF_CUDA(c, launch_iteration(c, 0.5 * dt, k, -1, false, which));
+    TF_CUDA(c, launch_iteration(c, 0.5 * dt, k, -1, (which & 4) != 0, which & 3));
     return TF_OK;
 }
 

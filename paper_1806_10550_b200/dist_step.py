@@ -125,6 +125,9 @@ class DistributedFilm:
         j0, j1 = self.lay.rows[self.rank]
         self.ctx_x = tf.ThinFilm(nx, j1 - j0, dx, dy, kappa, hstar, n, m)
         self.ctx_y = tf.ThinFilm(self.lay.local_width(self.rank), ny, dx, dy, kappa, hstar, n, m)
+        for c in (self.ctx_x, self.ctx_y):
+            c.set_newton(tol, min(max_iter, 4096), 0)                 # the gate compares with the context's tol
+        self.last_iters = 1
 
     def set_state_rows(self, h_rows):
         """h_rows: this rank's row block [ny_loc][nx] (numpy or CUDA tensor); distributes the column layout too"""
@@ -137,31 +140,48 @@ class DistributedFilm:
     def get_state_rows(self):
         return self.ctx_x.get_state()
 
-    def step(self, dt):
-        """returns (status, newton_iters, residual) like ThinFilm.step; on rejection the state is unchanged"""
+    def step(self, dt, batch=None):
+        """returns (status, newton_iters, residual) like ThinFilm.step; on rejection the state is unchanged.
+        Iterations are enqueued `batch` at a time (the first batch as long as the previous accepted step's count) and
+        the host reads the records of a batch at once: the sweeps of iteration k are gated on the ALL-REDUCED record
+        of iteration k-1, which is written into both contexts, so iterations past the deciding one do nothing on any
+        rank (their redistributions move unchanged data) -- the scheme of tf_set_launch_ahead across ranks."""
         import torch
         tf, cx, cy = self.tf, self.ctx_x, self.ctx_y
-        rec = torch.zeros(2, dtype=torch.float64, device="cuda")
-        k, res, status = 0, 0.0, tf.NOT_CONVERGED
-        while k < self.max_iter:
-            cy.sweep(dt, k, cy.SWEEP_Y)
-            cols_to_rows(self.lay, self.rank, self.comm, cy.field(cy.FIELD_W), cx.field(cx.FIELD_W))
-            cx.sweep(dt, k, cx.SWEEP_X)
-            rows_to_cols(self.lay, self.rank, self.comm, cx.field(cx.FIELD_ITERATE), cy.field(cy.FIELD_ITERATE))
-            r, bad = cx.residual(k)
-            rec[0], rec[1] = (float("inf") if r != r else r), float(bad)
-            self.comm.all_reduce(rec, "max")
-            res, bad = float(rec[0]), bool(rec[1] != 0)
-            k += 1
-            if bad or not np.isfinite(res):
-                break
-            if res < self.tol:
-                status = tf.OK
-                break
+        rx, ry = cx.field(cx.FIELD_RECORDS), cy.field(cy.FIELD_RECORDS)
+        gate = cx.SWEEP_GATED
+        batch = max(1, int(batch if batch is not None else self.last_iters))
+        k = done = 0
+        res, status, decided = 0.0, tf.NOT_CONVERGED, False
+        while not decided and done < self.max_iter:
+            upto = min(self.max_iter, k + batch)
+            while k < upto:
+                cy.sweep(dt, k, cy.SWEEP_Y | gate)
+                cols_to_rows(self.lay, self.rank, self.comm, cy.field(cy.FIELD_W), cx.field(cx.FIELD_W))
+                cx.sweep(dt, k, cx.SWEEP_X | gate)
+                rows_to_cols(self.lay, self.rank, self.comm, cx.field(cx.FIELD_ITERATE), cy.field(cy.FIELD_ITERATE))
+                rec = rx[k]
+                rec[0].nan_to_num_(nan=float("inf"))                 # a NaN anywhere must win the max ...
+                rec[1].copy_(torch.maximum(rec[1], torch.isinf(rec[0]).to(rec.dtype)))   # ... and close the gate
+                self.comm.all_reduce(rec, "max")
+                ry[k].copy_(rec)
+                k += 1
+            recs = rx[done:k].cpu().numpy()                          # one synchronising read per batch
+            for r, bad in recs:
+                done += 1
+                res = float(r)
+                if bad != 0 or not np.isfinite(res):
+                    decided = True
+                    break
+                if res < self.tol:
+                    status, decided = tf.OK, True
+                    break
+            batch = 2
         if status == tf.OK:
             cx.accept()
             cy.accept()
-        return status, k, res
+            self.last_iters = done
+        return status, done, res
 
     def mass(self):
         import torch

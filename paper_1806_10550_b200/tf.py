@@ -190,8 +190,8 @@ class ThinFilm:
         return st, it.value, res.value
 
     # ---- the rows of the path one at a time (tf_field / tf_sweep / tf_residual / tf_accept)
-    FIELD_STATE, FIELD_ITERATE, FIELD_BN, FIELD_W = 0, 1, 2, 3
-    SWEEP_Y, SWEEP_X = 1, 2
+    FIELD_STATE, FIELD_ITERATE, FIELD_BN, FIELD_W, FIELD_RECORDS = 0, 1, 2, 3, 4
+    SWEEP_Y, SWEEP_X, SWEEP_GATED = 1, 2, 4
 
     def field(self, which):
         """a torch view [ny][nx] of a field the context owns (no copy; the addresses of 0 and 1 swap on accept)"""
@@ -200,11 +200,12 @@ class ThinFilm:
         st = lib().tf_field(self._h, int(which), ctypes.byref(p))
         if st != OK:
             _err(self._h, st, "tf_field")
-        n = self.nx * self.ny
+        n = self.nx * self.ny if which != self.FIELD_RECORDS else 2 * 4096
         if self._ws is not None:
             off = (p.value - self._ws.data_ptr()) // 8
             if 0 <= off and off + n <= self._ws.numel() * self._ws.element_size() // 8:
-                return self._ws.view(torch.float64)[off:off + n].view(self.ny, self.nx)
+                v = self._ws.view(torch.float64)[off:off + n]
+                return v.view(self.ny, self.nx) if which != self.FIELD_RECORDS else v.view(4096, 2)
         raise TfError(ERR_STATE, "tf_field", "field views need a context created on a torch workspace")
 
     def sweep(self, dt, k, which):
