@@ -137,6 +137,11 @@ class DistributedFilm:
         rows_to_cols(self.lay, self.rank, self.comm, self.ctx_x.field(self.ctx_x.FIELD_STATE), tmp)
         self.ctx_y.set_state(tmp)
 
+    def set_pressure(self, kind, params=()):
+        """tf_set_pressure on both contexts (NLC / polymer models)"""
+        self.ctx_x.set_pressure(kind, params)
+        self.ctx_y.set_pressure(kind, params)
+
     def get_state_rows(self):
         return self.ctx_x.get_state()
 
