@@ -47,6 +47,21 @@ def test_workspace_sizes_and_host_side_validation():
     assert L.tf_penta_workspace_bytes_ex(64, 512, 0, tf.PENTA_PARTITION, 4) >= \
         L.tf_penta_workspace_bytes(64, 512) + 4 * 36 * 64 * 8
     assert L.tf_penta_solve_ex(8, 8, 0, 7, 0, *([None] * 9)) == tf.ERR_INVALID_ARG
+    # analysis and slab entry points validate their arguments before any device work
+    import numpy as np
+    one = (ctypes.c_double * 1)(float("nan"))
+    ll = (ctypes.c_longlong * 1)()
+    assert L.tf_betti_workspace_bytes(0, 8, 1) == 0 and L.tf_betti_workspace_bytes(64, 64, 3) >= 64 * 64 * 5
+    assert L.tf_betti(None, 8, 8, one, 1, ll, ll, None, None) == tf.ERR_INVALID_ARG
+    assert L.tf_spectrum_workspace_bytes(64, 64, 10) >= 3 * 64 * 64 * 8 and L.tf_spectrum_workspace_bytes(1, 64, 10) == 0
+    assert L.tf_radial_spectrum(None, 64, 64, 1.0, 1.0, 1.0, 10, None, None, None, 0, None, None, None) == tf.ERR_INVALID_ARG
+    assert L.tf_penta_slab_interface_doubles(64, 512, 0, 4) == 4 * 20 * 64
+    assert L.tf_penta_slab_interface_doubles(64, 100, 0, 4) == 0                     # chunks would be shorter than 96
+    assert L.tf_penta_slab_workspace_bytes(512, 64, 1, 2, 3) >= 3 * 512 * 64 * 8 + 6 * 16 * 64 * 8
+    assert L.tf_penta_slab_interface(64, 512, 0, 4, 5, 3, *([None] * 8)) == tf.ERR_INVALID_ARG   # slab index >= nslabs
+    q = np.linspace(0.1, 5.0, 50)
+    g, f, peaks = tf.radial_peaks(q, np.exp(-(q - 2.0) ** 2))                          # host-only entry point works without a GPU
+    assert len(g) == 400 and abs(max(peaks, key=lambda p: p[1])[0] - 2.0) < 0.1
     assert L.tf_kernel_launches() == 0
 
 
