@@ -30,30 +30,34 @@ _libs = {}
 _dp = ctypes.POINTER(ctypes.c_double)
 
 
+def _declare(L):
+    """ctypes signatures of the tfo_* entry points (also used by tests that load a mutated build of tfo.c)."""
+    L.tfo_create.argtypes = [ctypes.POINTER(ctypes.c_void_p), ctypes.c_int, ctypes.c_int, ctypes.c_double,
+                             ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
+                             ctypes.c_int]
+    L.tfo_set_model_linear.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_double]
+    L.tfo_set_pressure.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, ctypes.c_int]
+    L.tfo_pressure.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, _dp]
+    L.tfo_cell_functions.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, _dp, _dp, _dp, _dp]
+    L.tfo_set_newton.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_int, ctypes.c_int]
+    L.tfo_set_state.argtypes = [ctypes.c_void_p, _dp]
+    L.tfo_get_state.argtypes = [ctypes.c_void_p, _dp]
+    L.tfo_step.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.POINTER(ctypes.c_int), _dp]
+    L.tfo_mass.argtypes = [ctypes.c_void_p, _dp]
+    L.tfo_destroy.argtypes = [ctypes.c_void_p]
+    L.tfo_destroy.restype = None
+    L.tfo_operator_D.argtypes = [ctypes.c_void_p, _dp, _dp]
+    L.tfo_jacobian_bands.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, _dp, _dp, _dp, _dp, _dp]
+    L.tfo_directional_solve.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double, _dp, _dp, _dp]
+    L.tfo_penta_solve.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int] + [_dp] * 7
+    return L
+
+
 def lib(omp=False):
     key = bool(omp)
     if key not in _libs:
         build()
-        L = ctypes.CDLL(os.path.join(_HERE, "libtfo_omp.so" if omp else "libtfo.so"))
-        L.tfo_create.argtypes = [ctypes.POINTER(ctypes.c_void_p), ctypes.c_int, ctypes.c_int, ctypes.c_double,
-                                 ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
-                                 ctypes.c_int]
-        L.tfo_set_model_linear.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_double]
-        L.tfo_set_pressure.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, ctypes.c_int]
-        L.tfo_pressure.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, _dp]
-        L.tfo_cell_functions.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, _dp, _dp, _dp, _dp]
-        L.tfo_set_newton.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_int, ctypes.c_int]
-        L.tfo_set_state.argtypes = [ctypes.c_void_p, _dp]
-        L.tfo_get_state.argtypes = [ctypes.c_void_p, _dp]
-        L.tfo_step.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.POINTER(ctypes.c_int), _dp]
-        L.tfo_mass.argtypes = [ctypes.c_void_p, _dp]
-        L.tfo_destroy.argtypes = [ctypes.c_void_p]
-        L.tfo_destroy.restype = None
-        L.tfo_operator_D.argtypes = [ctypes.c_void_p, _dp, _dp]
-        L.tfo_jacobian_bands.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, _dp, _dp, _dp, _dp, _dp]
-        L.tfo_directional_solve.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double, _dp, _dp, _dp]
-        L.tfo_penta_solve.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int] + [_dp] * 7
-        _libs[key] = L
+        _libs[key] = _declare(ctypes.CDLL(os.path.join(_HERE, "libtfo_omp.so" if omp else "libtfo.so")))
     return _libs[key]
 
 
@@ -75,8 +79,8 @@ def _chk(rc, what):
 class ThinFilmOracle:
     """Same call names as the CUDA binding (create/set_newton/set_state/step/get_state/mass)."""
 
-    def __init__(self, nx, ny, dx, dy, kappa=100.0, hstar=0.1, n=3, m=2, bc=0, omp=False):
-        self.L = lib(omp)
+    def __init__(self, nx, ny, dx, dy, kappa=100.0, hstar=0.1, n=3, m=2, bc=0, omp=False, library=None):
+        self.L = library if library is not None else lib(omp)   # library: a mutated build (tests/test_oracle_mutants.py)
         self.nx, self.ny = nx, ny
         self._h = ctypes.c_void_p()
         _chk(self.L.tfo_create(ctypes.byref(self._h), nx, ny, dx, dy, kappa, hstar, n, m, bc), "tfo_create")

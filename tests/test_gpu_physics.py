@@ -86,3 +86,64 @@ def test_second_order_in_time_mass_fixed_point_symmetry(tf):
         g_.set_state(h_)
         assert g_.step(5e-3)[0] == 0
     assert np.max(np.abs(a.get_state() - b.get_state().T)) <= 1e-12 * np.max(np.abs(ha))
+
+
+def _iterate(tf, h, dx, dy, dt, k):
+    """u_(k) of the step from u^n = h on the CUDA path (fixed count k) and the residual it returned."""
+    if k == 0:
+        return h.copy(), None
+    g = tf.ThinFilm(h.shape[1], h.shape[0], dx, dy, K, HS, N_, M_)
+    g.set_newton(1e-10, 64, k)
+    g.set_state(h)
+    st, it, res = g.step(dt)
+    assert st == 0 and it == k
+    return g.get_state(), res
+
+
+@pytest.mark.parametrize("shape", [(37, 29), (96, 160)])
+def test_residual_is_max_rel_update_over_previous_iterate(tf, shape):
+    """(2.22), reading R7, on the CUDA path alone: the residual tf_step returns for iteration k+1
+    equals max |u_(k+1) - u_(k)| / |u_(k)| formed in numpy from the iterates of two fixed-count runs (pre-update
+    iterate in the denominator; the post-update reading differs by ~1e-4 relative on this film)."""
+    nx, ny = shape
+    dx, dy, dt = 0.41, 0.47, 1e-2
+    rng = np.random.default_rng(11)
+    x, y = (np.arange(nx) + 0.5) / nx, (np.arange(ny) + 0.5) / ny
+    h = np.ascontiguousarray(1.0 + 0.35 * np.cos(3 * np.pi * x)[None, :] * np.cos(2 * np.pi * y)[:, None]
+                             + 0.2 * rng.uniform(-1, 1, (ny, nx)))
+    for k in (0, 1, 3):
+        uk, _ = _iterate(tf, h, dx, dy, dt, k)
+        uk1, res = _iterate(tf, h, dx, dy, dt, k + 1)
+        expect = float(np.max(np.abs(uk1 - uk) / np.abs(uk)))
+        other = float(np.max(np.abs(uk1 - uk) / np.abs(uk1)))
+        assert abs(other - expect) > 1e-9 * expect
+        assert abs(res - expect) <= 1e-14, (k, res, expect)
+    # the Newton count of a tol-converged step is the first k whose numpy residual is below tol
+    tol = 1e-8
+    g = tf.ThinFilm(nx, ny, dx, dy, K, HS, N_, M_)
+    g.set_newton(tol, 64, 0)
+    g.set_state(h)
+    st, iters, _ = g.step(dt)
+    assert st == 0 and 3 <= iters < 64
+    prev, first = h, None
+    for k in range(1, iters + 2):
+        uk, _ = _iterate(tf, h, dx, dy, dt, k)
+        r = float(np.max(np.abs(uk - prev) / np.abs(prev)))
+        if first is None and r < tol * (1 - 1e-6):
+            first = k
+        assert not (first is None and r < tol * (1 + 1e-6))
+        prev = uk
+    assert first == iters
+    assert np.array_equal(g.get_state(), _iterate(tf, h, dx, dy, dt, iters)[0])
+
+
+def test_mass_uses_dx_times_dy(tf):
+    """(3.2), times the domain area, dx != dy, against math.fsum (no oracle)."""
+    for nx, ny, dx, dy in ((17, 23, 0.3, 0.7), (64, 9, 2.0, 0.125), (300, 167, 0.11, 0.9)):
+        rng = np.random.default_rng(nx)
+        h = np.ascontiguousarray(1.0 + 0.5 * rng.uniform(-1, 1, (ny, nx)))
+        g = tf.ThinFilm(nx, ny, dx, dy, K, HS, N_, M_)
+        g.set_state(h)
+        expect = dx * dy * math.fsum(h.ravel().tolist())
+        assert abs(g.mass() - expect) <= 1e-13 * abs(expect)
+        assert abs(g.mass() - dx * dx * math.fsum(h.ravel().tolist())) > 0.1 * abs(expect)
