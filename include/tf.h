@@ -80,8 +80,9 @@ tf_status tf_set_pressure(tf_ctx* ctx, tf_pressure kind, const double* params, i
 
 /* Newton controls, (2.22) and Notes 1-2.  Defaults: tol = 1e-10,
  * max_iter = 10, fixed_iters = 0 (off).  tol >= 1e-14;
- * 1 <= max_iter <= 4096; 0 <= fixed_iters <= 4096.  fixed_iters = K > 0: exactly K
- * iterations per step and the step is always accepted (parity mode). */
+ * 1 <= max_iter <= 4096; 0 <= fixed_iters <= 4096.  fixed_iters = K > 0 (parity mode): exactly K
+ * iterations per step, no convergence test; the step is accepted unless one of the K iterates was
+ * non-finite or non-positive (then TF_NOT_CONVERGED, state unchanged, *residual = NaN if a residual was NaN). */
 tf_status tf_set_newton(tf_ctx* ctx, double tol, int max_iter, int fixed_iters);
 
 /* Host decision of Fig. 1 (PAPER.md:256-258; the paper reads one flag per 16x16 block per iteration, :675-683).
@@ -172,6 +173,9 @@ tf_status tf_mass(tf_ctx* ctx, double* mass);
  *   dir = 1: system s = column s (strided;   nsys = ncol, len = nrow)   -- the y-sweep shape
  * dev_ws: device scratch of tf_penta_workspace_bytes(nrow, ncol) bytes.  x may not alias inputs.
  * len >= 3.  Runs on cuda_stream; returns after enqueueing (no host sync).
+ * Pivots: no pivoting, and the reciprocal of every pivot is formed from a hardware seed
+ * (rcp.approx.ftz.f64) plus one cubic correction, <= 1 ulp for pivots with |mu| in [1e-290, 1e290]; pivots outside
+ * that range (or zero) give inf / NaN in the affected system, as a division would for a zero pivot.
  */
 size_t    tf_penta_workspace_bytes(int nrow, int ncol);
 tf_status tf_penta_solve(int nrow, int ncol, int dir,
@@ -255,7 +259,7 @@ tf_status tf_betti(const double* h, int nx, int ny, const double* thresholds, in
  * with q_r = 2 pi sqrt(kx^2 + ky^2) / L, the mean magnitude and N_k; *nk = number of distinct radii (may exceed cap:
  * then only the first cap are stored).  dev_ws: tf_spectrum_workspace_bytes(nx, ny, kmax) bytes of device scratch.
  * Synchronises the stream.  Steps five and six of the appendix (least-squares fit, moving average, maxima) are 1-D
- * post-processing of this output and are left to the caller.
+ * post-processing of this output: tf_radial_peaks below.
  */
 size_t    tf_spectrum_workspace_bytes(int nx, int ny, int kmax);
 tf_status tf_radial_spectrum(const double* h, int nx, int ny, double L, double H0, double sigma, int kmax,

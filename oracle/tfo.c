@@ -386,8 +386,9 @@ int tfo_get_state(tfo_ctx *c, double *h)
  *   repeat: R = b^n - u_(k) - s D(u_(k));  (I + s J_y) w = R;  (I + s J_x) v = w;
  *           res = max |v/u_(k)|;  u_(k+1) = u_(k) + v;
  *   accept when res < tol; reject (state stays u^n) after max_iter iterations or when
- *   an iterate is not finite / not positive.  With fixed_iters = K > 0: exactly K
- *   iterations, always accepted.  Sweep order y then x (reading R3).
+ *   an iterate is not finite / not positive (reading R18).  With fixed_iters = K > 0:
+ *   exactly K iterations, accepted unless one of the K iterates was not finite / not
+ *   positive (R18 again: such a field is not a state).  Sweep order y then x (R3).
  */
 int tfo_step(tfo_ctx *c, double dt, int *newton_iters, double *residual)
 {
@@ -400,7 +401,7 @@ int tfo_step(tfo_ctx *c, double dt, int *newton_iters, double *residual)
     for (size_t p = 0; p < N; ++p) c->bn[p] = c->u[p] - s * c->R[p];
     memcpy(c->uk, c->u, N * sizeof(double));
     const int kmax = c->fixed_iters > 0 ? c->fixed_iters : c->max_iter;
-    int k = 0, status = TFO_NOT_CONVERGED; double res = 0.0;
+    int k = 0, status = TFO_NOT_CONVERGED, anybad = 0; double res = 0.0;
     while (k < kmax) {
         fill_functions(c, c->uk);
         operator_D(c, c->uk, c->R);
@@ -415,7 +416,8 @@ int tfo_step(tfo_ctx *c, double dt, int *newton_iters, double *residual)
             if (!isfinite(c->uk[p]) || (c->model != 1 && !(c->uk[p] > 0))) bad = 1;
         }
         ++k;
-        if (c->fixed_iters > 0) { if (k == kmax) status = TFO_OK; continue; }
+        if (bad || res != res) anybad = 1;
+        if (c->fixed_iters > 0) { if (k == kmax && !anybad) status = TFO_OK; continue; }
         if (bad) break;
         if (res < c->tol) { status = TFO_OK; break; }
     }

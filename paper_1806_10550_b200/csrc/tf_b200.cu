@@ -15,6 +15,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -97,18 +98,21 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+EncodeTiledFn lookup_encode_tiled()
+{
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+        return (EncodeTiledFn)p;
+    return nullptr;
+}
+
+// contexts are created from several host threads (one per rank in the in-process multi-rank tests): the
+// function-local static is initialised exactly once, thread-safely
 EncodeTiledFn encode_tiled_fn()
 {
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = (EncodeTiledFn)p;
-    }
+    static const EncodeTiledFn fn = lookup_encode_tiled();
     return fn;
 }
 
@@ -131,10 +135,10 @@ constexpr int YB_NST = 8, YB_RS = 16;     // 8 stages x 16 rows x 3 arrays x 256
 
 // "has this kernel's shared-memory opt-in been done on the current device" (function attributes are per device)
 struct DevOnce {
-    unsigned long long mask = 0;
+    std::atomic<unsigned long long> mask{0};
     static int dev() { int d = 0; cudaGetDevice(&d); return d & 63; }
-    bool done() const { return (mask >> dev()) & 1ull; }
-    void mark() { mask |= 1ull << dev(); }
+    bool done() const { return (mask.load(std::memory_order_acquire) >> dev()) & 1ull; }
+    void mark() { mask.fetch_or(1ull << dev(), std::memory_order_release); }   // setting the attribute twice is harmless
 };
 
 template <typename K>
@@ -146,13 +150,16 @@ cudaError_t opt_in_smem(K kernel, size_t bytes)
 constexpr int YT_NST = 4, YT_RS = 16;     // TMA ring: 4 stages x 3 boxes of 16 x 32 doubles = 48 KiB per warp: all 512 CTAs resident (4 per SM)
 constexpr int XT_NST = 3;                 // TMA ring: 3 stages x 16 KiB: all 512 CTAs resident (4 per SM)
 
+// SM count of the CURRENT device (context-free entry points; a context keeps its own in c->num_sms)
 int num_sms()
 {
-    static int sms = 0;
+    static std::atomic<int> cache[64];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+    int sms = cache[dev & 63].load(std::memory_order_relaxed);
     if (!sms) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-            sms = 148;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) sms = 148;
+        cache[dev & 63].store(sms, std::memory_order_relaxed);
     }
     return sms;
 }
@@ -203,7 +210,7 @@ cudaError_t launch_ybwd2(const CUtensorMap* m, bool tma, int nx, int ny, int mid
 // two-sided x back substitution + update + residual
 cudaError_t launch_xbwd2(const CUtensorMap* m, const CUtensorMap& uin, const CUtensorMap& uout, bool tma, int nx, int ny,
                          int mid, const double* alT, const double* beT, const double* zzT, const double* uk,
-                         double* unew, double* red, cudaStream_t st, Gate gate)
+                         double* unew, double* red, cudaStream_t st, Gate gate, int sms)
 {
     const dim3 g((ny + 31) / 32, 2);
     if (!tma) {
@@ -212,7 +219,7 @@ cudaError_t launch_xbwd2(const CUtensorMap* m, const CUtensorMap& uin, const CUt
     }
     // ring depth: 3 stages when every CTA must fit at once (4 per SM); 6 when there are at most 2 CTAs per SM
     // (measured at 4096^2: 0.149 -> 0.138 ms; the y ring showed no gain from more stages)
-    if ((int)(g.x * g.y) > 2 * num_sms())
+    if ((int)(g.x * g.y) > 2 * sms)
         return launch_xbwd2_n<XT_NST, true>(m, uin, uout, g, nx, ny, mid, alT, beT, zzT, red, st, gate);
     return launch_xbwd2_n<2 * XT_NST, true>(m, uin, uout, g, nx, ny, mid, alT, beT, zzT, red, st, gate);
 }
@@ -330,7 +337,7 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, i
     if (ev) cudaEventRecord(ev[3], c->stream);
     if (which & 2)
         le = launch_xbwd2(c->mX, c->mU[src == c->ubuf[0] ? 0 : 1], c->mU[c->uk == c->ubuf[0] ? 0 : 1], c->tma_x, P.nx, P.ny,
-                          c->mid_x, c->al, c->be, c->zz, src, c->uk, c->red + 2 * k, c->stream, gate);
+                          c->mid_x, c->al, c->be, c->zz, src, c->uk, c->red + 2 * k, c->stream, gate, c->num_sms);
     if (le != cudaSuccess) return le;
     if (ev) cudaEventRecord(ev[4], c->stream);
     count_launch((which & 1 ? 2 : 0) + (which & 2 ? 2 : 0));
@@ -748,12 +755,18 @@ tf_status tf_step(tf_ctx* c, double dt, int* newton_iters, double* residual)
         // parity mode: no host decision inside the step, one read at the end
         const bool prof = c->profiling && kmax <= 64;
         for (; k < kmax; ++k) TF_CUDA(c, launch_iteration(c, s, k, prof ? k : -1, false));
-        TF_CUDA(c, cudaMemcpyAsync(c->pinned, c->red + 2 * (kmax - 1), 2 * sizeof(double), cudaMemcpyDeviceToHost,
+        TF_CUDA(c, cudaMemcpyAsync(c->pinned_red, c->red, 2 * sizeof(double) * (size_t)kmax, cudaMemcpyDeviceToHost,
                                    c->stream));
         TF_CUDA(c, cudaStreamSynchronize(c->stream));
         if (prof) collect_profile(c, kmax);
-        res = c->pinned[0];
+        res = c->pinned_red[2 * (kmax - 1)];
         status = TF_OK;
+        // reading R18 also holds here: an iterate that was not finite or not positive must not become the state
+        // (tf_set_state would refuse the same field, and the cell functions assume h > 0)
+        for (int it = 0; it < kmax; ++it) {
+            const double r = c->pinned_red[2 * it];
+            if (c->pinned_red[2 * it + 1] != 0.0 || r != r) { status = TF_NOT_CONVERGED; res = r != r ? r : res; }
+        }
     } else {
         // S8 with speculative launch-ahead: iterations are enqueued in batches -- the first as long as the previous
         // step's iteration count (the count changes slowly from step to step), then `spec_batch` at a time -- and the
@@ -1126,6 +1139,7 @@ struct CuFFT {
     }
 };
 CuFFT g_fft;
+std::mutex g_fft_mutex;                      // one plan cache per process: tf_radial_spectrum holds it from plan lookup to exec
 size_t sp_field_bytes(int nx, int ny) { return align_up((size_t)nx * ny * sizeof(double)); }
 size_t sp_half_bytes(int nx, int ny) { return align_up((size_t)ny * (nx / 2 + 1) * 2 * sizeof(double)); }
 }  // namespace
@@ -1154,6 +1168,7 @@ tf_status tf_radial_spectrum(const double* h, int nx, int ny, double L, double H
         for (int a = 0; a <= 2 * W.r; ++a) { const double m = a - W.r; W.w[a] = W.r ? std::exp(-m * m / (2.0 * sigma * sigma)) : 1.0; sum += W.w[a]; }
         for (int a = 0; a <= 2 * W.r; ++a) W.w[a] /= sum;
     }
+    std::lock_guard<std::mutex> fft_lock(g_fft_mutex);
     if (!g_fft.load()) return fail(nullptr, TF_ERR_UNSUPPORTED, "tf_radial_spectrum: libcufft.so.11 not found");
     if (!g_fft.get_plan(nx, ny)) return fail(nullptr, TF_ERR_CUDA, "tf_radial_spectrum: cufftPlan2d failed");
     cudaStream_t st = (cudaStream_t)cuda_stream;

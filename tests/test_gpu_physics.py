@@ -147,3 +147,19 @@ def test_mass_uses_dx_times_dy(tf):
         expect = dx * dy * math.fsum(h.ravel().tolist())
         assert abs(g.mass() - expect) <= 1e-13 * abs(expect)
         assert abs(g.mass() - dx * dx * math.fsum(h.ravel().tolist())) > 0.1 * abs(expect)
+
+
+def test_fixed_count_step_with_a_bad_iterate_is_not_accepted(tf):
+    """Reading R18 in parity mode (include/tf.h, tf_set_newton): a fixed-count step whose iterates leave h > 0 is
+    returned as TF_NOT_CONVERGED with the state untouched; a sane step afterwards is accepted."""
+    nx, ny = 64, 48
+    rng = np.random.default_rng(5)
+    h = np.ascontiguousarray(0.12 + 0.1 * rng.uniform(0, 1, (ny, nx)))
+    g = tf.ThinFilm(nx, ny, 0.05, 0.05, K, HS, N_, M_)
+    g.set_newton(1e-10, 64, 2)
+    g.set_state(h)
+    st, it, res = g.step(10.0)
+    assert st == tf.NOT_CONVERGED and it == 2
+    assert np.array_equal(g.get_state(), h)
+    st, it, res = g.step(1e-9)
+    assert st == tf.OK and it == 2 and np.all(g.get_state() > 0)

@@ -126,3 +126,19 @@ def test_mutants_are_rejected(name, tmp_path):
 
     with pytest.raises(AssertionError):
         check(factory)
+
+
+def test_fixed_count_step_with_a_bad_iterate_is_not_accepted():
+    """Reading R18 in parity mode: with fixed_iters = K the step is accepted unless one of the K iterates
+    was non-finite or non-positive; then the state stays u^n (a non-positive film is not a state: Pi is singular)."""
+    nx, ny = 24, 20
+    rng = np.random.default_rng(5)
+    h = np.ascontiguousarray(0.12 + 0.1 * rng.uniform(0, 1, (ny, nx)))       # thin, rough film; dt far too large
+    o = tfo.ThinFilmOracle(nx, ny, 0.05, 0.05, 100.0, 0.1, 3, 2)
+    o.set_newton(1e-10, 64, 2)
+    o.set_state(h)
+    st, it, res = o.step(10.0)
+    assert st == tfo.NOT_CONVERGED and it == 2
+    assert np.array_equal(o.get_state(), h)
+    st, it, res = o.step(1e-9)                                                # a sane step is still accepted afterwards
+    assert st == tfo.OK and it == 2 and np.all(o.get_state() > 0)
