@@ -346,10 +346,12 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, i
 
 cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, int which = 3)
 {
+#ifndef TF_ONLY_POWER32                      /* experiment builds instantiate the (3,2) power law only */
     if (c->model == TF_PI_NLC) return launch_iteration<MODEL_NLC, 0>(c, s, k, slot, gated, which);
     if (c->model == TF_PI_POLYMER) return launch_iteration<MODEL_POLYMER, 0>(c, s, k, slot, gated, which);
-    if (c->P.n == 3 && c->P.m == 2) return launch_iteration<3, 2>(c, s, k, slot, gated, which);
-    return launch_iteration<0, 0>(c, s, k, slot, gated, which);
+    if (!(c->P.n == 3 && c->P.m == 2)) return launch_iteration<0, 0>(c, s, k, slot, gated, which);
+#endif
+    return launch_iteration<3, 2>(c, s, k, slot, gated, which);
 }
 
 // after a stream sync: fold the event intervals of `niter` profiled iterations into the totals
@@ -388,6 +390,7 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
     Params& P = c->P;
     P.nx = nx; P.ny = ny; P.dx = dx; P.dy = dy;
     P.rdx2 = 1.0 / (dx * dx); P.rdy2 = 1.0 / (dy * dy);
+    P.m2r = -2.0 * (P.rdx2 + P.rdy2);
     P.n = n; P.m = m;
     double hm = 1.0, hn = 1.0;
     for (int k = 0; k < m; ++k) hm *= hstar;

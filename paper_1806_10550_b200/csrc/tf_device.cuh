@@ -18,6 +18,7 @@ struct Params {
     int nx, ny;
     double dx, dy;
     double rdx2, rdy2;      // 1/dx^2, 1/dy^2
+    double m2r;             // -2 (rdx2 + rdy2)
     int n, m;               // Pi exponents, n > m >= 1
     double cm, cn;          // kappa*m*hstar^m, kappa*n*hstar^n
     double mp[10];          // constants of the NLC / polymer pressures (tf_set_pressure), see cell_functions
@@ -175,7 +176,11 @@ __device__ __forceinline__ void elim2_row(Elim2& S, double e, double c, double q
     const double T = fma(-S.b2, e, q);
     const double g = S.p1 * gam;
     const double bg = S.b1 * gam;
+#ifdef TF_EXP_NOZ
+    const double sy = y;
+#else
     const double sy = fma(-S.z2, e, y);
+#endif
     const double u1 = fma(-g, S.y1, T);
     const double G = g * S.y1;
     const double mu = fma(-G, S.t1, u1);             // the only op between t1 and the next seed
@@ -184,9 +189,14 @@ __device__ __forceinline__ void elim2_row(Elim2& S, double e, double c, double q
     const double ee = fma(-mu, y0, 1.0);
     const double tt = fma(ee, ee, ee);
     const double r1 = fma(S.y1, S.t1, S.y1);         // finish row i-1, off the critical path
-    al = S.p1 * r1; be = S.b1 * r1; zz = S.s1 * r1;
-    const double p = fma(-bg, r1, a);
+    al = S.p1 * r1; be = S.b1 * r1;
+#ifdef TF_EXP_NOZ
+    zz = sy; const double s = sy;
+#else
+    zz = S.s1 * r1;
     const double s = fma(-zz, gam, sy);
+#endif
+    const double p = fma(-bg, r1, a);
     S.a2 = al; S.b2 = be; S.z2 = zz;
     S.y1 = y0; S.t1 = tt; S.p1 = p; S.b1 = b; S.s1 = s;
 }

@@ -22,6 +22,15 @@ namespace tf {
 #ifndef TF_ROTATE_Y
 #define TF_ROTATE_Y 1
 #endif
+#ifndef TF_WAIT_HINT_NS
+#define TF_WAIT_HINT_NS 0
+#endif
+#ifndef TF_Y_TRIM
+#define TF_Y_TRIM 0
+#endif
+#ifndef TF_Y_ELIM1
+#define TF_Y_ELIM1 0
+#endif
 constexpr int YW_VALID = 28;     // columns per strip (lanes 2..29; lanes 0,1,30,31 are x-halo)
 
 // rolling state of a thread marching down a column
@@ -44,7 +53,12 @@ __device__ __forceinline__ void y_advance(YState& S, int j, double hp2, const Pa
     const unsigned FULL = 0xffffffffu;
     const int ny = P.ny;
     const double hL = __shfl_up_sync(FULL, S.hp1, 1), hR = __shfl_down_sync(FULL, S.hp1, 1);
+#if TF_Y_TRIM
+    // 5 fp64 instead of 6: lap h = rdx2 (hL + hR) + rdy2 (h(j+2) + h(j)) - 2 (rdx2 + rdy2) h(j+1)
+    const double Lp = fma(P.rdy2, hp2 + S.h0, fma(P.rdx2, hL + hR, P.m2r * S.hp1));
+#else
     const double Lp = fma((hL + hR) - 2.0 * S.hp1, P.rdx2, ((hp2 + S.h0) - 2.0 * S.hp1) * P.rdy2);
+#endif
     const Cell cp = cell_functions<N, M>(S.hp1, P);
     Face fp = {0.0, 0.0, 0.0};
     double phip = 0.0;
@@ -61,6 +75,27 @@ __device__ __forceinline__ void y_advance(YState& S, int j, double hp2, const Pa
         }
     }
     if (MODE == 2) {
+#ifdef TF_PERT_SHFL
+        {   // perturbation probe: 4 extra 32-bit shuffles per row
+            int t = __double2loint(hp2);
+            t ^= __shfl_xor_sync(FULL, t, 1); t ^= __shfl_xor_sync(FULL, t, 2); t ^= __shfl_xor_sync(FULL, t, 4); t ^= __shfl_xor_sync(FULL, t, 8);
+            if (t == 0x7fffffff) S.phim += 1.0;
+        }
+#endif
+#ifdef TF_PERT_FMA
+        {   // perturbation probe: 4 extra independent DFMAs per row
+            const double a0 = fma(hp2, 1.25, S.h0), a1 = fma(hp2, 1.5, S.hm1), a2 = fma(S.h0, 1.75, S.hm1), a3 = fma(S.hp1, 2.25, S.hm1);
+            if (__double2hiint(a0) == 0x7ff12345 || __double2hiint(a1) == 0x7ff12345 || __double2hiint(a2) == 0x7ff12345 || __double2hiint(a3) == 0x7ff12345) S.phim += 1.0;
+        }
+#endif
+#ifdef TF_PERT_INT
+        {   // perturbation probe: 8 extra integer ops per row
+            int t = __double2loint(hp2);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) t = t * 1664525 + j;
+            if (t == 0x7fffffff) S.phim += 1.0;
+        }
+#endif
         const double f0R = __shfl_down_sync(FULL, S.c0.f0, 1), f1R = __shfl_down_sync(FULL, S.c0.f1, 1);
         const double LR = __shfl_down_sync(FULL, S.L0, 1);
         double phixp = DX.cb * fma(S.c0.f0 + f0R, LR - S.L0, (S.c0.f1 + f1R) * (S.hR0 - S.h0));
@@ -204,7 +239,11 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
             }
             __syncwarp();
             issue_tma(c + NP);                                  // staging is free again: fetch my next chunk
+#if TF_WAIT_HINT_NS
+            mbar_wait_hint(empty + s, ((c / NCH) & 1) ^ 1, TF_WAIT_HINT_NS);
+#else
             mbar_wait(empty + s, ((c / NCH) & 1) ^ 1);
+#endif
             // slot row of chunk row r: r (half 0), RP-1-r (half 1)
             double* st = sm + (size_t)s * 5 * SV + (dir ? RP - 1 : 0) * 32 + lane;
             const int sstep = dir ? -32 : 32;
@@ -212,6 +251,15 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
             S.hm1 = 0.0; S.h0 = hq[0]; S.hp1 = hq[1]; S.hR0 = 0.0;
             S.c0 = {0, 0, 0, 0}; S.L0 = 0.0; S.fm = {0, 0, 0}; S.phim = 0.0;
             double o6[6], sD;
+#ifdef TF_EXP_NOPROD
+            if (interior) {
+#pragma unroll
+                for (int r = 0; r < RP; ++r) {
+                    double* sr = st + r * sstep;
+                    sr[0] = hq[r]; sr[SV] = hq[r + 1]; sr[2 * SV] = hq[r + 2] + 4.0; sr[3 * SV] = hq[r + 3]; sr[4 * SV] = bq[r];
+                }
+            } else
+#endif
             if (interior) {
                 y_advance<N, M, 0, true>(S, jlo - 2, hq[2], P, DX, DY, xface, 0.0, o6, sD);
                 y_advance<N, M, 1, true>(S, jlo - 1, hq[3], P, DX, DY, xface, 0.0, o6, sD);
@@ -252,9 +300,53 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
         }
     } else {
         // ------------------------------------------------------------------ consumer: the recurrence.
+#if TF_Y_ELIM1
+        // textbook row elimination (12 fp64 + 1 MUFU per row, 75-cycle chain): with four teams per SM the kernel is
+        // bound by instruction throughput, not by the chain, and elim2_row's shorter chain costs 4 more fp64 per row
+        Elim S = {0, 0, 0, 0, 0, 0};
+        double e = 0.0;
+        const int step = dir ? -nx : nx;
+        int o = (dir ? ny - 1 : 0) * nx + i;
+        const int offc = dir ? 3 * SV : SV, offa = dir ? SV : 3 * SV;
+        for (int c = 0; c < nchunk; ++c) {
+            const int s = c % NCH;
+            mbar_wait(full + s, (c / NCH) & 1);
+            const double* st = sm + (size_t)s * 5 * SV + lane;
+            const double* stc = st + offc;
+            const double* sta = st + offa;
+            const int nrow = min(RP, nrows - c * RP);
+            if (nrow == RP) {
+#pragma unroll
+                for (int r = 0; r < RP; ++r) {
+                    const double A = st[r * 32], cc = stc[r * 32], q = st[2 * SV + r * 32], a = sta[r * 32];
+                    const double R = st[4 * SV + r * 32];
+                    double va, vb, vz;
+                    elim_row(S, e, cc, q, a, A, R, va, vb, vz);
+                    e = A;
+                    st3_if(outl, al + o, va, be + o, vb, zz + o, vz);
+                    o += step;
+                }
+            } else {
+                for (int r = 0; r < nrow; ++r) {
+                    const double A = st[r * 32], cc = stc[r * 32], q = st[2 * SV + r * 32], a = sta[r * 32];
+                    const double R = st[4 * SV + r * 32];
+                    double va, vb, vz;
+                    elim_row(S, e, cc, q, a, A, R, va, vb, vz);
+                    e = A;
+                    st3_if(outl, al + o, va, be + o, vb, zz + o, vz);
+                    o += step;
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + s);
+        }
+#else
         // elim2_row emits the coefficients of the PREVIOUS row, so every store goes one row behind.
         Elim2 S = elim2_init();
         double e = 0.0;
+#ifdef TF_EXP_NOSTORE
+        int xacc = 0;
+#endif
         const int step = dir ? -nx : nx;
         int o = (dir ? ny : -1) * nx + i;                 // the row before the first one (32-bit element offset)
         const int offc = dir ? 3 * SV : SV, offa = dir ? SV : 3 * SV;   // half 1: c' = a, a' = c
@@ -265,6 +357,9 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
             const double* stc = st + offc;
             const double* sta = st + offa;
             const int nrow = min(RP, nrows - c * RP);
+#ifdef TF_EXP_NOCONS
+            if (nrow == RP && c > 0) { o += RP * step; } else
+#endif
             if (nrow == RP && c > 0) {
 #pragma unroll
                 for (int r = 0; r < RP; ++r) {
@@ -273,7 +368,13 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
                     double va, vb, vz;
                     elim2_row(S, e, cc, q, a, A, R, va, vb, vz);
                     e = A;
+#ifdef TF_EXP_NOSTORE
+                    xacc ^= __double2hiint(va) ^ __double2hiint(vb) ^ __double2hiint(vz);
+#elif defined(TF_EXP_STORE_L2)
+                    { const int o2 = (o & 0x3fffff); st3_if(outl, al + o2, va, be + o2, vb, zz + o2, vz); }   // 32 MB window per plane: stays in L2
+#else
                     st3_if(outl, al + o, va, be + o, vb, zz + o, vz);
+#endif
                     o += step;
                 }
             } else {
@@ -292,7 +393,11 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
         }
         double va, vb, vz;
         elim2_flush(S, va, vb, vz);
+#ifdef TF_EXP_NOSTORE
+        if (xacc == 0x12345) vz = 1.0;
+#endif
         st3_if(outl, al + o, va, be + o, vb, zz + o, vz);
+#endif
     }
 }
 
@@ -402,8 +507,13 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
             }
 #endif
             const int g0 = 2 * t, g1 = 2 * t + 1;             // global slot numbers of this tile
+#if TF_WAIT_HINT_NS
+            mbar_wait_hint(empty + g0 % NCH, ((g0 / NCH) & 1) ^ 1, TF_WAIT_HINT_NS);
+            mbar_wait_hint(empty + g1 % NCH, ((g1 / NCH) & 1) ^ 1, TF_WAIT_HINT_NS);
+#else
             mbar_wait(empty + g0 % NCH, ((g0 / NCH) & 1) ^ 1);
             mbar_wait(empty + g1 % NCH, ((g1 / NCH) & 1) ^ 1);
+#endif
             double* st = sm + (size_t)((slot_sel ? g1 : g0) % NCH) * NPL * SV + kc * XW_LD;
             // one row of the tile; INTERIOR: every face of the tile is an interior, unfolded face and every
             // column belongs to this half -- no boundary selects (all tiles but the first, last and the split one)

@@ -61,6 +61,43 @@ def test_ranks_as_threads_equal_the_single_device_step(tf, world, nx, ny):
     assert np.max(np.abs(h - ref_h)) <= 1e-11 * np.max(np.abs(ref_h))
 
 
+@pytest.mark.parametrize("world,nx,ny", [(2, 128, 96), (3, 208, 160)])
+def test_ranks_as_threads_equal_the_oracle(tf, world, nx, ny):
+    """The assembled film of the distributed step against the CPU oracle (not the single-device CUDA path): same
+    Newton counts, every element to 1e-11 after one converged step and after three steps with a fixed count."""
+    import local_comm
+    from oracle import tfo
+    from paper_1806_10550_b200 import dist_step as ds
+    dx, dy = 0.4259, 0.45
+    h0 = inputs.noise_ic(nx, ny, seed=nx + world)
+    lay = ds.Layout(nx, ny, world)
+    o = tfo.ThinFilmOracle(nx, ny, dx, dy, K, HS, 3, 2)
+    o.set_newton(1e-10, 64, 0)
+    o.set_state(h0)
+    ref_log = [o.step(1e-2)]
+    ref_h1 = o.get_state()
+    ref_log += [o.step(1e-2), o.step(5e-3)]
+    ref_h3 = o.get_state()
+
+    def rank_main(comm):
+        f = ds.DistributedFilm(nx, ny, dx, dy, K, HS, 3, 2, comm=comm, tol=1e-10, max_iter=64)
+        j0, j1 = lay.rows[comm.rank]
+        f.set_state_rows(np.ascontiguousarray(h0[j0:j1]))
+        log = [f.step(1e-2)]
+        h1 = f.get_state_rows()
+        log += [f.step(1e-2), f.step(5e-3)]
+        return log, h1, f.get_state_rows(), f.mass()
+
+    out = local_comm.run_ranks(world, rank_main)
+    h1 = np.concatenate([r[1] for r in out], axis=0)
+    h3 = np.concatenate([r[2] for r in out], axis=0)
+    for r in range(world):
+        assert [(s, k) for s, k, _ in out[r][0]] == [(s, k) for s, k, _ in ref_log]
+        assert abs(out[r][3] - o.mass()) <= 1e-13 * o.mass()
+    assert np.max(np.abs(h1 - ref_h1)) <= 1e-11 * np.max(np.abs(ref_h1))
+    assert np.max(np.abs(h3 - ref_h3)) <= 1e-10 * np.max(np.abs(ref_h3))     # three converged steps (tol 1e-10 each)
+
+
 def test_rejected_step_leaves_the_distributed_state_unchanged(tf):
     import local_comm
     from paper_1806_10550_b200 import dist_step as ds
