@@ -1,0 +1,66 @@
+"""Out-of-bounds evidence without compute-sanitizer (closed on this GPU pool, profiles/r02_sanitizer.md): the context
+gets a caller-supplied workspace that sits between two guard zones filled with a bit pattern, runs steps on grids with
+ragged strips / tiles / splits, and the guards must come back untouched.  (A write past one of the context's seven
+fields lands in the next field and shows up as a parity failure in tests/test_gpu_parity.py instead.)"""
+import ctypes
+
+import numpy as np
+import pytest
+
+from paper_1806_10550_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+GUARD = 1 << 20
+
+
+@pytest.mark.parametrize("nx,ny", [(61, 45), (192, 160), (300, 167), (1030, 70), (70, 1030), (4228, 64), (64, 4228)])
+def test_workspace_guards_stay_intact(nx, ny):
+    import torch
+    from paper_1806_10550_b200 import tf
+    L = tf.lib()
+    nbytes = L.tf_workspace_bytes(nx, ny)
+    buf = torch.empty(nbytes + 2 * GUARD + 256, dtype=torch.uint8, device="cuda")
+    off = (-buf.data_ptr()) % 256
+    buf.fill_(0xA5)
+    h = ctypes.c_void_p()
+    stream = torch.cuda.current_stream()
+    cfg = inputs.config(0)
+    st = L.tf_create_with_workspace(ctypes.byref(h), nx, ny, cfg["dx"], cfg["dy"], 100.0, 0.1, 3, 2, 0,
+                                    buf.data_ptr() + off + GUARD, nbytes, stream.cuda_stream)
+    assert st == 0
+    try:
+        film = torch.from_numpy(inputs.noise_ic(nx, ny, seed=nx)).cuda()
+        assert L.tf_set_state(h, film.data_ptr(), 1) == 0
+        it, res, m = ctypes.c_int(0), ctypes.c_double(0.0), ctypes.c_double(0.0)
+        for _ in range(2):
+            assert L.tf_step(h, 1e-2, ctypes.byref(it), ctypes.byref(res)) == 0
+        assert L.tf_mass(h, ctypes.byref(m)) == 0
+        torch.cuda.synchronize()
+    finally:
+        L.tf_destroy(h)
+    lo = buf[off:off + GUARD]
+    hi = buf[off + GUARD + nbytes:off + GUARD + nbytes + GUARD]
+    assert bool((lo == 0xA5).all()) and bool((hi == 0xA5).all())
+
+
+@pytest.mark.parametrize("nx,ny", [(1024, 1024), (4228, 96), (300, 167)])
+def test_steps_are_bitwise_reproducible_run_to_run(nx, ny):
+    """Five runs of the same three steps: fields, residuals and iteration counts identical to the last bit.  The ring
+    hand-overs (mbarrier full/empty, TMA stores from shared tiles) have no run-to-run freedom when they are correct:
+    a slot released early or a missing proxy fence shows up as a difference between runs."""
+    from paper_1806_10550_b200 import tf
+    cfg = inputs.config(0)
+    h = inputs.noise_ic(nx, ny, seed=7)
+    ref = None
+    for _ in range(5):
+        g = tf.ThinFilm(nx, ny, cfg["dx"], cfg["dy"])
+        g.set_newton(1e-10, 64, 0)
+        g.set_state(h)
+        log = [g.step(1e-2) for _ in range(3)]
+        out = (log, g.get_state())
+        g.close()
+        if ref is None:
+            ref = out
+        else:
+            assert out[0] == ref[0]
+            assert np.array_equal(out[1], ref[1])
