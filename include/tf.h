@@ -161,6 +161,31 @@ tf_status tf_sweep(tf_ctx* ctx, double dt, int k, int which);
 tf_status tf_residual(tf_ctx* ctx, int k, double* res, int* bad);
 tf_status tf_accept(tf_ctx* ctx);
 
+/*
+ * Exchange steps of a time step whose film is spread over several devices (the paper names a multi-GPU
+ * implementation as future work).  The caller (paper_1806_10550_b200/dist_step.py) owns the collective;
+ * the library moves the blocks and applies the boundary condition:
+ *   tf_blocks_gather   buf[offset_k + r*ncols_k + c] = field[(row0_k + r)*ld + col0_k + c] for every block k -- the send
+ *                      buffer of an all-to-all in ONE kernel;
+ *   tf_blocks_scatter  the reverse, from the receive buffer into a field of row pitch ld; in the same pass the ghost
+ *                      columns of a halo'd column block at a domain edge are filled by the reflection of (2.28),
+ *                      reflect_left != 0: columns 1, 0 := columns 2, 3 (h_{-1} = h_0, h_{-2} = h_1);
+ *                      reflect_right_at = g >= 0: columns g, g+1 := columns g-1, g-2; g < 0: none;
+ *   tf_record_sanitize the residual record {res, bad} of iteration k before it is max-reduced over the ranks: a NaN
+ *                      (or +inf) residual becomes {+inf, 1}, so that it wins the max and closes the gates.
+ * field, buf: DEVICE pointers; rects: HOST array of nrect <= 64 blocks (copied into the launch); offsets in doubles.
+ * Blocks must lie inside the field (col0 + ncols <= ld).  All four enqueue on a stream and return (no host sync).
+ *   tf_block_copy      one block straight from field to field (what a rank keeps for itself never enters the buffers):
+ *                      dst[(drow0 + r)*dld + dcol0 + c] = src[(srow0 + r)*sld + scol0 + c], ghost columns as in scatter.
+ */
+typedef struct { int row0, nrows, col0, ncols; long long offset; } tf_rect;
+tf_status tf_block_copy(const double* src, int sld, int srow0, int scol0, double* dst, int dld, int drow0, int dcol0,
+                        int nrows, int ncols, int reflect_left, int reflect_right_at, void* cuda_stream);
+tf_status tf_blocks_gather(const double* field, int ld, const tf_rect* rects, int nrect, double* buf, void* cuda_stream);
+tf_status tf_blocks_scatter(const double* buf, const tf_rect* rects, int nrect, double* field, int ld,
+                            int reflect_left, int reflect_right_at, void* cuda_stream);
+tf_status tf_record_sanitize(tf_ctx* ctx, int k);
+
 /* mass = dx*dy*sum(h)  ((3.2), times the domain area); fixed-order fp64 tree. */
 tf_status tf_mass(tf_ctx* ctx, double* mass);
 

@@ -8,6 +8,7 @@
 #include "tf_fwd.cuh"
 #include "tf_topo.cuh"
 #include "tf_spectrum.cuh"
+#include "tf_blocks.cuh"
 #include <dlfcn.h>
 
 #include <algorithm>
@@ -853,6 +854,86 @@ tf_status tf_accept(tf_ctx* c)
     if (!c) return TF_ERR_INVALID_ARG;
     if (!c->have_state) return fail(c, TF_ERR_STATE, "no state set");
     std::swap(c->u, c->uk);
+    return TF_OK;
+}
+
+// ---- exchange steps of the distributed time step: block pack / unpack and the record to be max-reduced
+static tf_status blocks_common(const tf_rect* rects, int nrect, int ld, Rects* R, dim3* grid)
+{
+    if (!rects || nrect < 1 || nrect > BLK_MAX || ld < 1)
+        return fail(nullptr, TF_ERR_INVALID_ARG, "tf_blocks_*: 1 <= nrect <= 64 blocks, ld >= 1");
+    int maxr = 0, maxc = 0;
+    for (int k = 0; k < nrect; ++k) {
+        const tf_rect& q = rects[k];
+        if (q.row0 < 0 || q.col0 < 0 || q.nrows < 0 || q.ncols < 0 || q.offset < 0 || q.col0 + q.ncols > ld)
+            return fail(nullptr, TF_ERR_INVALID_ARG, "tf_blocks_*: block outside the field or negative offset");
+        R->r[k] = Rect{q.row0, q.nrows, q.col0, q.ncols, q.offset};
+        maxr = std::max(maxr, q.nrows);
+        maxc = std::max(maxc, q.ncols);
+    }
+    R->n = nrect;
+    const unsigned gy = (unsigned)((maxr + BLK_ROWS - 1) / BLK_ROWS);
+    if (gy > 65535u) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_blocks_*: more than 524280 rows in a block");
+    *grid = dim3((unsigned)std::max(1, std::min((maxc + BLK_THREADS - 1) / BLK_THREADS, 64)), std::max(gy, 1u), (unsigned)nrect);
+    return TF_OK;
+}
+
+tf_status tf_blocks_gather(const double* field, int ld, const tf_rect* rects, int nrect, double* buf, void* cuda_stream)
+{
+    if (!field || !buf) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_blocks_gather: NULL pointer");
+    Rects R;
+    dim3 g;
+    tf_status st = blocks_common(rects, nrect, ld, &R, &g);
+    if (st != TF_OK) return st;
+    blocks_gather_kernel<<<g, BLK_THREADS, 0, (cudaStream_t)cuda_stream>>>(field, ld, R, buf);
+    count_launch(1);
+    TF_CUDA(nullptr, cudaGetLastError());
+    return TF_OK;
+}
+
+tf_status tf_blocks_scatter(const double* buf, const tf_rect* rects, int nrect, double* field, int ld, int reflect_left,
+                            int reflect_right_at, void* cuda_stream)
+{
+    if (!field || !buf) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_blocks_scatter: NULL pointer");
+    if (reflect_right_at >= 0 && (reflect_right_at < 2 || reflect_right_at + 2 > ld))
+        return fail(nullptr, TF_ERR_INVALID_ARG, "tf_blocks_scatter: right ghost columns outside the field");
+    if (reflect_left && ld < 4) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_blocks_scatter: field narrower than its ghosts");
+    Rects R;
+    dim3 g;
+    tf_status st = blocks_common(rects, nrect, ld, &R, &g);
+    if (st != TF_OK) return st;
+    blocks_scatter_kernel<<<g, BLK_THREADS, 0, (cudaStream_t)cuda_stream>>>(buf, R, field, ld, reflect_left ? 1 : 0,
+                                                                             reflect_right_at);
+    count_launch(1);
+    TF_CUDA(nullptr, cudaGetLastError());
+    return TF_OK;
+}
+
+tf_status tf_block_copy(const double* src, int sld, int srow0, int scol0, double* dst, int dld, int drow0, int dcol0,
+                        int nrows, int ncols, int reflect_left, int reflect_right_at, void* cuda_stream)
+{
+    if (!src || !dst) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_block_copy: NULL pointer");
+    if (nrows < 0 || ncols < 0 || srow0 < 0 || scol0 < 0 || drow0 < 0 || dcol0 < 0 || scol0 + ncols > sld || dcol0 + ncols > dld)
+        return fail(nullptr, TF_ERR_INVALID_ARG, "tf_block_copy: block outside a field");
+    if (reflect_right_at >= 0 && (reflect_right_at < 2 || reflect_right_at + 2 > dld))
+        return fail(nullptr, TF_ERR_INVALID_ARG, "tf_block_copy: right ghost columns outside the field");
+    if (nrows == 0 || ncols == 0) return TF_OK;
+    const unsigned gy = (unsigned)((nrows + BLK_ROWS - 1) / BLK_ROWS);
+    if (gy > 65535u) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_block_copy: more than 524280 rows");
+    const dim3 g((unsigned)std::max(1, std::min((ncols + BLK_THREADS - 1) / BLK_THREADS, 64)), gy);
+    block_copy_kernel<<<g, BLK_THREADS, 0, (cudaStream_t)cuda_stream>>>(src, sld, srow0, scol0, dst, dld, drow0, dcol0, nrows,
+                                                                         ncols, reflect_left ? 1 : 0, reflect_right_at);
+    count_launch(1);
+    TF_CUDA(nullptr, cudaGetLastError());
+    return TF_OK;
+}
+
+tf_status tf_record_sanitize(tf_ctx* c, int k)
+{
+    if (!c || k < 0 || k >= MAX_ITERS) return TF_ERR_INVALID_ARG;
+    record_sanitize_kernel<<<1, 1, 0, c->stream>>>(c->red + 2 * k);
+    count_launch(1);
+    TF_CUDA(c, cudaGetLastError());
     return TF_OK;
 }
 

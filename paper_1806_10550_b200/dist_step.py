@@ -21,8 +21,9 @@ is the arithmetic of the single-device path (parity with it to 1e-11, not bit fo
 
 The collectives go through a small `comm` object (all_to_all of flat buffers with split sizes, all_reduce max / sum):
 TorchComm wraps a torch.distributed group (NCCL over NVLink on GPUs); tests pass an in-process stand-in.
-Packing and unpacking of the blocks are strided tensor copies (memory movement only; all arithmetic of the path
-stays in the library's kernels).
+Packing and unpacking of the blocks, the ghost reflection of (2.28) at the domain's own edges and the preparation of
+the residual record for the reduction are library kernels (tf_blocks_gather / tf_blocks_scatter / tf_record_sanitize,
+include/tf.h): this module holds no arithmetic of the method.
 """
 import numpy as np
 
@@ -64,51 +65,78 @@ class Layout:
         return self.cols[r][1] - self.cols[r][0] + 2 * self.HALO
 
 
-def rows_to_cols(lay, r, comm, f_rows, f_cols):
-    """f_rows: [ny_loc][nx] of rank r  ->  f_cols: [ny][nxl + 4] of rank r, halos included (reflection at domain edges)"""
-    import torch
-    pieces, scount, rcount = [], [], []
-    for q in range(lay.world):
-        a, b = lay.halo_cols(q)
-        pieces.append(f_rows[:, a:b].reshape(-1))
-        scount.append(pieces[-1].numel())
-    a, b = lay.halo_cols(r)
-    for p in range(lay.world):
-        rcount.append((lay.rows[p][1] - lay.rows[p][0]) * (b - a))
-    recv = comm.all_to_all(torch.cat(pieces), scount, rcount)
-    off = a - (lay.cols[r][0] - lay.HALO)                       # local column of global column a (2 at the left domain edge)
-    pos = 0
-    for p in range(lay.world):
-        j0, j1 = lay.rows[p]
-        f_cols[j0:j1, off:off + (b - a)] = recv[pos:pos + rcount[p]].view(j1 - j0, b - a)
-        pos += rcount[p]
-    n = lay.cols[r][1] - lay.cols[r][0]
-    if r == 0:                                                   # h_{-1} = h_0, h_{-2} = h_1  (PAPER.md:297-304)
-        f_cols[:, 1] = f_cols[:, 2]
-        f_cols[:, 0] = f_cols[:, 3]
-    if r == lay.world - 1:                                       # h_{nx} = h_{nx-1}, h_{nx+1} = h_{nx-2}
-        f_cols[:, n + 2] = f_cols[:, n + 1]
-        f_cols[:, n + 3] = f_cols[:, n]
+class Exchange:
+    """The two redistributions of rank r with everything that does not change from call to call worked out once:
+    block lists (tf_rect arrays), split sizes, send / receive buffers.  Packing, unpacking and the ghost reflection of
+    (2.28) run in the library (tf_blocks_gather / tf_blocks_scatter); this class only strings them around the
+    all-to-all."""
 
+    def __init__(self, lay, r, tf, device="cuda"):
+        import torch
+        self.lay, self.r, self.tf = lay, r, tf
+        j0, j1 = lay.rows[r]
+        nyl = j1 - j0
+        i0, i1 = lay.cols[r]
+        n = i1 - i0
+        a, b = lay.halo_cols(r)
+        # rows -> columns: send to q the columns q needs (own + halo) of my rows; receive my halo'd columns of p's rows
+        # (the block a rank keeps for itself goes straight from field to field: tf_block_copy, zero split size)
+        blocks, off, self.rc_scount, self.rc_rcount = [], 0, [], []
+        for q in range(lay.world):
+            aq, bq = lay.halo_cols(q)
+            cnt = 0 if q == r else nyl * (bq - aq)
+            blocks.append((0, nyl if q != r else 0, aq, bq - aq, off))
+            self.rc_scount.append(cnt)
+            off += cnt
+        self.rc_send_rects, self.rc_send = tf.make_rects(blocks), torch.empty(max(off, 1), dtype=torch.float64, device=device)
+        loc = a - (i0 - lay.HALO)                      # local column of global column a (2 at the left domain edge)
+        blocks, off = [], 0
+        for p in range(lay.world):
+            p0, p1 = lay.rows[p]
+            cnt = 0 if p == r else (p1 - p0) * (b - a)
+            blocks.append((p0, p1 - p0 if p != r else 0, loc, b - a, off))
+            self.rc_rcount.append(cnt)
+            off += cnt
+        self.rc_recv_rects = tf.make_rects(blocks)
+        self.rc_self = (0, a, j0, loc, nyl, b - a)      # src row0, col0 -> dst row0, col0, rows, cols
+        self.refl_left = (r == 0)                      # h_{-1} = h_0, h_{-2} = h_1  (PAPER.md:297-304)
+        self.refl_right_at = n + 2 if r == lay.world - 1 else -1
+        # columns -> rows: send to q its rows of my own columns; receive p's columns of my rows
+        blocks, off, self.cr_scount, self.cr_rcount = [], 0, [], []
+        for q in range(lay.world):
+            q0, q1 = lay.rows[q]
+            cnt = 0 if q == r else (q1 - q0) * n
+            blocks.append((q0, q1 - q0 if q != r else 0, lay.HALO, n, off))
+            self.cr_scount.append(cnt)
+            off += cnt
+        self.cr_send_rects, self.cr_send = tf.make_rects(blocks), torch.empty(max(off, 1), dtype=torch.float64, device=device)
+        blocks, off = [], 0
+        for p in range(lay.world):
+            c0, c1 = lay.cols[p]
+            cnt = 0 if p == r else nyl * (c1 - c0)
+            blocks.append((0, nyl if p != r else 0, c0, c1 - c0, off))
+            self.cr_rcount.append(cnt)
+            off += cnt
+        self.cr_recv_rects = tf.make_rects(blocks)
+        self.cr_self = (j0, lay.HALO, 0, i0, nyl, n)
 
-def cols_to_rows(lay, r, comm, f_cols, f_rows):
-    """interior of f_cols [ny][nxl + 4] of rank r  ->  f_rows [ny_loc][nx] of rank r"""
-    import torch
-    n = lay.cols[r][1] - lay.cols[r][0]
-    pieces, scount, rcount = [], [], []
-    for q in range(lay.world):
-        j0, j1 = lay.rows[q]
-        pieces.append(f_cols[j0:j1, lay.HALO:lay.HALO + n].reshape(-1))
-        scount.append(pieces[-1].numel())
-    j0, j1 = lay.rows[r]
-    for p in range(lay.world):
-        rcount.append((j1 - j0) * (lay.cols[p][1] - lay.cols[p][0]))
-    recv = comm.all_to_all(torch.cat(pieces), scount, rcount)
-    pos = 0
-    for p in range(lay.world):
-        i0, i1 = lay.cols[p]
-        f_rows[:, i0:i1] = recv[pos:pos + rcount[p]].view(j1 - j0, i1 - i0)
-        pos += rcount[p]
+    def rows_to_cols(self, comm, f_rows, f_cols):
+        """f_rows: [ny_loc][nx] of this rank -> f_cols: [ny][nxl + 4] of this rank, halos and ghosts included"""
+        sr, sc, dr, dc, nr, nc = self.rc_self
+        self.tf.block_copy(f_rows, sr, sc, f_cols, dr, dc, nr, nc, self.refl_left, self.refl_right_at)
+        if self.lay.world > 1:
+            self.tf.blocks_gather(f_rows, self.rc_send_rects, self.rc_send)
+            recv = comm.all_to_all(self.rc_send, self.rc_scount, self.rc_rcount)
+            self.tf.blocks_scatter(recv, self.rc_recv_rects, f_cols, self.refl_left, self.refl_right_at)
+
+    def cols_to_rows(self, comm, f_cols, f_rows):
+        """interior of f_cols [ny][nxl + 4] of this rank -> f_rows [ny_loc][nx] of this rank"""
+        sr, sc, dr, dc, nr, nc = self.cr_self
+        self.tf.block_copy(f_cols, sr, sc, f_rows, dr, dc, nr, nc)
+        if self.lay.world > 1:
+            self.tf.blocks_gather(f_cols, self.cr_send_rects, self.cr_send)
+            recv = comm.all_to_all(self.cr_send, self.cr_scount, self.cr_rcount)
+            self.tf.blocks_scatter(recv, self.cr_recv_rects, f_rows)
 
 
 class DistributedFilm:
@@ -128,13 +156,14 @@ class DistributedFilm:
         for c in (self.ctx_x, self.ctx_y):
             c.set_newton(tol, min(max_iter, 4096), 0)                 # the gate compares with the context's tol
         self.last_iters = 1
+        self.ex = Exchange(self.lay, self.rank, tf)
 
     def set_state_rows(self, h_rows):
         """h_rows: this rank's row block [ny_loc][nx] (numpy or CUDA tensor); distributes the column layout too"""
         import torch
         self.ctx_x.set_state(h_rows)
         tmp = torch.ones(self.ny, self.lay.local_width(self.rank), dtype=torch.float64, device="cuda")
-        rows_to_cols(self.lay, self.rank, self.comm, self.ctx_x.field(self.ctx_x.FIELD_STATE), tmp)
+        self.ex.rows_to_cols(self.comm, self.ctx_x.field(self.ctx_x.FIELD_STATE), tmp)
         self.ctx_y.set_state(tmp)
 
     def set_pressure(self, kind, params=()):
@@ -162,12 +191,11 @@ class DistributedFilm:
             upto = min(self.max_iter, k + batch)
             while k < upto:
                 cy.sweep(dt, k, cy.SWEEP_Y | gate)
-                cols_to_rows(self.lay, self.rank, self.comm, cy.field(cy.FIELD_W), cx.field(cx.FIELD_W))
+                self.ex.cols_to_rows(self.comm, cy.field(cy.FIELD_W), cx.field(cx.FIELD_W))
                 cx.sweep(dt, k, cx.SWEEP_X | gate)
-                rows_to_cols(self.lay, self.rank, self.comm, cx.field(cx.FIELD_ITERATE), cy.field(cy.FIELD_ITERATE))
+                self.ex.rows_to_cols(self.comm, cx.field(cx.FIELD_ITERATE), cy.field(cy.FIELD_ITERATE))
+                cx.record_sanitize(k)                                # a NaN must win the max and close the gates
                 rec = rx[k]
-                rec[0].nan_to_num_(nan=float("inf"))                 # a NaN anywhere must win the max ...
-                rec[1].copy_(torch.maximum(rec[1], torch.isinf(rec[0]).to(rec.dtype)))   # ... and close the gate
                 self.comm.all_reduce(rec, "max")
                 ry[k].copy_(rec)
                 k += 1

@@ -45,6 +45,11 @@ SYMBOLS = {
     "tf_sweep": (ctypes.c_int, [_vp, ctypes.c_double, ctypes.c_int, ctypes.c_int]),
     "tf_residual": (ctypes.c_int, [_vp, ctypes.c_int, _dp, ctypes.POINTER(ctypes.c_int)]),
     "tf_accept": (ctypes.c_int, [_vp]),
+    "tf_blocks_gather": (ctypes.c_int, [_vp, ctypes.c_int, _vp, ctypes.c_int, _vp, _vp]),
+    "tf_blocks_scatter": (ctypes.c_int, [_vp, _vp, ctypes.c_int, _vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp]),
+    "tf_record_sanitize": (ctypes.c_int, [_vp, ctypes.c_int]),
+    "tf_block_copy": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                     ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp]),
     "tf_penta_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int, ctypes.c_int]),
     "tf_penta_solve": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int] + [_vp] * 9),
     "tf_penta_partition_chunks": (ctypes.c_int, [ctypes.c_int] * 4),
@@ -225,6 +230,12 @@ class ThinFilm:
         if st != OK:
             _err(self._h, st, "tf_accept")
 
+    def record_sanitize(self, k):
+        """tf_record_sanitize: record k ready for a max-reduction over ranks (NaN -> {+inf, bad})."""
+        st = lib().tf_record_sanitize(self._h, int(k))
+        if st != OK:
+            _err(self._h, st, "tf_record_sanitize")
+
     def mass(self):
         m = ctypes.c_double(0.0)
         st = lib().tf_mass(self._h, ctypes.byref(m))
@@ -263,6 +274,52 @@ class ThinFilm:
         if h.dtype != torch.float64 or not h.is_contiguous() or tuple(h.shape) != (self.ny, self.nx):
             raise ValueError("expected a contiguous float64 [ny][nx] tensor")
         return h.data_ptr(), (1 if h.is_cuda else 0), h
+
+
+class _Rect(ctypes.Structure):
+    _fields_ = [("row0", ctypes.c_int), ("nrows", ctypes.c_int), ("col0", ctypes.c_int), ("ncols", ctypes.c_int),
+                ("offset", ctypes.c_longlong)]
+
+
+def make_rects(blocks):
+    """[(row0, nrows, col0, ncols, offset), ...] -> the tf_rect array tf_blocks_gather / tf_blocks_scatter take"""
+    arr = (_Rect * len(blocks))()
+    for k, b in enumerate(blocks):
+        arr[k] = _Rect(*[int(v) for v in b])
+    return arr
+
+
+def blocks_gather(field, rects, buf, stream=None):
+    """tf_blocks_gather: every block of the 2-D CUDA tensor `field` into the flat send buffer `buf` (one kernel)."""
+    torch = _torch()
+    assert field.is_cuda and buf.is_cuda and field.dtype == buf.dtype == torch.float64 and field.stride(1) == 1
+    stream = torch.cuda.current_stream(field.device) if stream is None else stream
+    st = lib().tf_blocks_gather(field.data_ptr(), field.stride(0), rects, len(rects), buf.data_ptr(), stream.cuda_stream)
+    if st != OK:
+        _err(None, st, "tf_blocks_gather")
+
+
+def blocks_scatter(buf, rects, field, reflect_left=False, reflect_right_at=-1, stream=None):
+    """tf_blocks_scatter: the receive buffer into `field`, ghost columns of (2.28) filled in the same pass."""
+    torch = _torch()
+    assert field.is_cuda and buf.is_cuda and field.dtype == buf.dtype == torch.float64 and field.stride(1) == 1
+    stream = torch.cuda.current_stream(field.device) if stream is None else stream
+    st = lib().tf_blocks_scatter(buf.data_ptr(), rects, len(rects), field.data_ptr(), field.stride(0),
+                                 1 if reflect_left else 0, int(reflect_right_at), stream.cuda_stream)
+    if st != OK:
+        _err(None, st, "tf_blocks_scatter")
+
+
+def block_copy(src, srow0, scol0, dst, drow0, dcol0, nrows, ncols, reflect_left=False, reflect_right_at=-1, stream=None):
+    """tf_block_copy: one block from the 2-D CUDA tensor `src` straight into `dst` (ghost columns as in blocks_scatter)."""
+    torch = _torch()
+    assert src.is_cuda and dst.is_cuda and src.dtype == dst.dtype == torch.float64 and src.stride(1) == dst.stride(1) == 1
+    stream = torch.cuda.current_stream(src.device) if stream is None else stream
+    st = lib().tf_block_copy(src.data_ptr(), src.stride(0), int(srow0), int(scol0), dst.data_ptr(), dst.stride(0), int(drow0),
+                             int(dcol0), int(nrows), int(ncols), 1 if reflect_left else 0, int(reflect_right_at),
+                             stream.cuda_stream)
+    if st != OK:
+        _err(None, st, "tf_block_copy")
 
 
 class _Adaptive(ctypes.Structure):

@@ -98,6 +98,38 @@ def test_ranks_as_threads_equal_the_oracle(tf, world, nx, ny):
     assert np.max(np.abs(h3 - ref_h3)) <= 1e-10 * np.max(np.abs(ref_h3))     # three converged steps (tol 1e-10 each)
 
 
+def test_block_kernels_equal_the_cpu_statement(tf):
+    """tf_blocks_gather / tf_blocks_scatter (incl. the ghost reflection of (2.28)) against the plain CPU statement of
+    the two calls in tests/test_multirank_redistribution.py, on ragged blocks."""
+    import torch
+    from test_multirank_redistribution import CpuBlocks
+    rng = np.random.default_rng(3)
+    ny, nx = 57, 203
+    F = torch.from_numpy(rng.uniform(0, 1, (ny, nx)))
+    blocks, off = [], 0
+    for (r0, nr, c0, nc) in ((0, 10, 0, 203), (10, 47, 5, 101), (3, 1, 200, 3), (20, 0, 0, 7), (56, 1, 0, 1)):
+        blocks.append((r0, nr, c0, nc, off))
+        off += nr * nc
+    buf_c, buf_g = torch.zeros(off, dtype=torch.float64), torch.zeros(off, dtype=torch.float64, device="cuda")
+    CpuBlocks.blocks_gather(F, CpuBlocks.make_rects(blocks), buf_c)
+    tf.blocks_gather(F.cuda(), tf.make_rects(blocks), buf_g)
+    assert torch.equal(buf_g.cpu(), buf_c)
+    n = 40                                                     # a halo'd column block of 40 own columns at both domain edges
+    blocks = [(0, 30, 2, n, 0), (30, 27, 2, n, 30 * n)]
+    src = torch.from_numpy(rng.uniform(0, 1, ny * n))
+    for lrefl, rrefl in ((True, n + 2), (False, -1), (True, -1), (False, n + 2)):
+        dst_c = torch.full((ny, n + 4), -1.0, dtype=torch.float64)
+        dst_g = dst_c.clone().cuda()
+        CpuBlocks.blocks_scatter(src, CpuBlocks.make_rects(blocks), dst_c, lrefl, rrefl)
+        tf.blocks_scatter(src.cuda(), tf.make_rects(blocks), dst_g, lrefl, rrefl)
+        assert torch.equal(dst_g.cpu(), dst_c), (lrefl, rrefl)
+        dst_c = torch.full((ny, n + 4), -1.0, dtype=torch.float64)          # the same block straight from a field
+        dst_g = dst_c.clone().cuda()
+        CpuBlocks.block_copy(F, 0, 17, dst_c, 0, 2, ny, n, lrefl, rrefl)
+        tf.block_copy(F.cuda(), 0, 17, dst_g, 0, 2, ny, n, lrefl, rrefl)
+        assert torch.equal(dst_g.cpu(), dst_c), (lrefl, rrefl)
+
+
 def test_rejected_step_leaves_the_distributed_state_unchanged(tf):
     import local_comm
     from paper_1806_10550_b200 import dist_step as ds

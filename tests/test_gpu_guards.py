@@ -29,6 +29,7 @@ def test_workspace_guards_stay_intact(nx, ny):
                                     buf.data_ptr() + off + GUARD, nbytes, stream.cuda_stream)
     assert st == 0
     try:
+        assert L.tf_set_newton(h, 1e-10, 64, 3) == 0
         film = torch.from_numpy(inputs.noise_ic(nx, ny, seed=nx)).cuda()
         assert L.tf_set_state(h, film.data_ptr(), 1) == 0
         it, res, m = ctypes.c_int(0), ctypes.c_double(0.0), ctypes.c_double(0.0)

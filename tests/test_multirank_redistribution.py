@@ -20,21 +20,53 @@ def field(nx, ny):
     return (1000.0 * j + i).astype(np.float64)              # every cell knows where it came from
 
 
+class CpuBlocks:
+    """Stand-in for the library's tf_blocks_gather / tf_blocks_scatter on CPU tensors, written from include/tf.h's
+    statement of the two calls (the CUDA kernels are compared with it in tests/test_gpu_distributed_step.py)."""
+
+    @staticmethod
+    def make_rects(blocks):
+        return [tuple(int(v) for v in b) for b in blocks]
+
+    @staticmethod
+    def blocks_gather(field, rects, buf):
+        for row0, nrows, col0, ncols, off in rects:
+            buf[off:off + nrows * ncols] = field[row0:row0 + nrows, col0:col0 + ncols].reshape(-1)
+
+    @staticmethod
+    def block_copy(src, srow0, scol0, dst, drow0, dcol0, nrows, ncols, reflect_left=False, reflect_right_at=-1):
+        dst[drow0:drow0 + nrows, dcol0:dcol0 + ncols] = src[srow0:srow0 + nrows, scol0:scol0 + ncols]
+        CpuBlocks.blocks_scatter(None, [], dst, reflect_left, reflect_right_at)
+
+    @staticmethod
+    def blocks_scatter(buf, rects, field, reflect_left=False, reflect_right_at=-1):
+        for row0, nrows, col0, ncols, off in rects:
+            field[row0:row0 + nrows, col0:col0 + ncols] = buf[off:off + nrows * ncols].view(nrows, ncols)
+        if reflect_left:
+            field[:, 1] = field[:, 2]
+            field[:, 0] = field[:, 3]
+        g = reflect_right_at
+        if g >= 0:
+            field[:, g] = field[:, g - 1]
+            field[:, g + 1] = field[:, g - 2]
+
+
 def check_rank(lay, r, comm, nx, ny):
     from paper_1806_10550_b200 import dist_step as ds
+    ex = ds.Exchange(lay, r, CpuBlocks, device="cpu")
     F = field(nx, ny)
     j0, j1 = lay.rows[r]
     i0, i1 = lay.cols[r]
     f_rows = torch.from_numpy(F[j0:j1].copy())
     f_cols = torch.full((ny, lay.local_width(r)), -1.0, dtype=torch.float64)
-    ds.rows_to_cols(lay, r, comm, f_rows, f_cols)
+    ex.rows_to_cols(comm, f_rows, f_cols)
     n = i1 - i0
     assert np.array_equal(f_cols[:, 2:2 + n].numpy(), F[:, i0:i1])                        # the block itself
     left = F[:, [1, 0]] if r == 0 else F[:, i0 - 2:i0]                                   # reflection: h_-2 = h_1, h_-1 = h_0
     right = F[:, [nx - 1, nx - 2]] if r == lay.world - 1 else F[:, i1:i1 + 2]
     assert np.array_equal(f_cols[:, :2].numpy(), left) and np.array_equal(f_cols[:, n + 2:].numpy(), right)
     back = torch.full((j1 - j0, nx), -1.0, dtype=torch.float64)
-    ds.cols_to_rows(lay, r, comm, f_cols, back)
+    ex.cols_to_rows(comm, f_cols, back)
     assert np.array_equal(back.numpy(), F[j0:j1])                                         # round trip
     return True
 
