@@ -140,6 +140,19 @@ tf_status tf_advance_adaptive(tf_ctx* ctx, tf_adaptive* ctl, int n_accept, int m
                               double* t_advanced, tf_step_record* hist, int hist_cap, int* nhist);
 
 /*
+ * The same controller with every decision taken ON THE DEVICE (the paper's controller is host
+ * code that reads a flag array after every iteration): attempts are enqueued in chunks without a
+ * host round trip -- per attempt a control kernel opens the attempt and publishes dt/2, max_iter gated iterations run
+ * (those past the deciding one return at once), a control kernel takes the decision of Fig. 1 from the residual
+ * records (accept / shrink / grow, dt_min, attempt cap) and a copy kernel commits u^{n+1} if the step was accepted.
+ * The host reads the control block once per chunk.  Same arguments, same results as tf_advance_adaptive: the sequence
+ * of (dt, status, iterations, residual) and the films are identical bit for bit.  At most 1024 attempts per call.
+ * TF_ERR_UNSUPPORTED with fixed_iters > 0 or the extra solution criterion switched on.
+ */
+tf_status tf_advance_adaptive_device(tf_ctx* ctx, tf_adaptive* ctl, int n_accept, int max_attempts,
+                                     double* t_advanced, tf_step_record* hist, int hist_cap, int* nhist);
+
+/*
  * The rows of the path one at a time, for callers that put an exchange step between the sweeps (a film distributed over
  * several devices).  tf_step is: for k = 0, 1, ...: tf_sweep(ctx, dt, k, 3); decide on
  * tf_residual(ctx, k); on acceptance tf_accept(ctx).

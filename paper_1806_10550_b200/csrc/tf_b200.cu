@@ -9,6 +9,7 @@
 #include "tf_topo.cuh"
 #include "tf_spectrum.cuh"
 #include "tf_blocks.cuh"
+#include "tf_control.cuh"
 #include <dlfcn.h>
 
 #include <algorithm>
@@ -33,7 +34,7 @@ thread_local std::string g_err;
 
 size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 size_t field_bytes(int nx, int ny) { return align_up((size_t)nx * ny * sizeof(double)); }
-size_t scratch_bytes() { return align_up(sizeof(double) * (2 * (MAX_ITERS + 1) + RED_BLOCKS + 8)); }
+size_t scratch_bytes() { return align_up(sizeof(double) * (2 * (MAX_ITERS + 1) + RED_BLOCKS + 8 + CT_SIZE + 4 * CT_HIST_CAP)); }
 constexpr int NFIELDS = 7;   // u, uk, bn, w, alpha, beta, z
 
 }  // namespace
@@ -51,6 +52,7 @@ struct tf_ctx {
     double *red;                               // [2*(MAX_ITERS+1)] residual / bad flag per iteration
     double *part;                              // [RED_BLOCKS]
     double *scal;                              // [8] : scal[0] mass, (int*)(scal+1) flag
+    double *ctl, *ctl_hist;                    // on-device adaptive controller: control block [CT_SIZE], history [4 * CT_HIST_CAP]
     double *pinned;                            // [4] host pinned readback
     double *pinned_red;                        // [2*MAX_ITERS] host pinned copy of the residual records
     double last_change;                        // max |u^{n+1} - u^n| / u^n of the last converged step (criterion on)
@@ -301,11 +303,14 @@ cudaError_t launch_xfwd(tf_ctx* c, const Params& P, const Dir& DX, const double*
 // one pseudo-Newton iteration k: reads src (u^n if k == 0 else uk), writes uk, red[2k..2k+1].  gated: the four
 // kernels return at once if iteration k-1's record says the step is already decided (speculative launch-ahead).
 // which: 1 = the y-sweep (S1-S4: y forward + y backward -> w), 2 = the x-sweep (S5-S7 -> uk, red[2k]), 3 = both
+// sdev != nullptr (on-device controller): s is read by the kernels from device memory, and iteration 0 is gated on gate0
 template <int N, int M>
-cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, int which = 3)
+cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, int which = 3, const double* sdev = nullptr,
+                             const double* gate0 = nullptr)
 {
     const Params& P = c->P;
-    const Gate gate = (gated && k > 0) ? Gate{c->red + 2 * (k - 1), c->tol} : Gate{nullptr, 0.0};
+    Gate gate = (gated && k > 0) ? Gate{c->red + 2 * (k - 1), c->tol, sdev} : Gate{nullptr, 0.0, sdev};
+    if (k == 0 && gate0) gate = Gate{gate0, c->tol, sdev};
     const Dir DX = make_dir(s, P.dx), DY = make_dir(s, P.dy);
     const double* src = (k == 0) ? c->u : c->uk;
     // one CTA = NSUB sub-problems: two strips x two halves, or one strip x two halves when that still leaves SMs idle
@@ -345,14 +350,15 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, i
     return cudaGetLastError();
 }
 
-cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, int which = 3)
+cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, int which = 3, const double* sdev = nullptr,
+                             const double* gate0 = nullptr)
 {
 #ifndef TF_ONLY_POWER32                      /* experiment builds instantiate the (3,2) power law only */
-    if (c->model == TF_PI_NLC) return launch_iteration<MODEL_NLC, 0>(c, s, k, slot, gated, which);
-    if (c->model == TF_PI_POLYMER) return launch_iteration<MODEL_POLYMER, 0>(c, s, k, slot, gated, which);
-    if (!(c->P.n == 3 && c->P.m == 2)) return launch_iteration<0, 0>(c, s, k, slot, gated, which);
+    if (c->model == TF_PI_NLC) return launch_iteration<MODEL_NLC, 0>(c, s, k, slot, gated, which, sdev, gate0);
+    if (c->model == TF_PI_POLYMER) return launch_iteration<MODEL_POLYMER, 0>(c, s, k, slot, gated, which, sdev, gate0);
+    if (!(c->P.n == 3 && c->P.m == 2)) return launch_iteration<0, 0>(c, s, k, slot, gated, which, sdev, gate0);
 #endif
-    return launch_iteration<3, 2>(c, s, k, slot, gated, which);
+    return launch_iteration<3, 2>(c, s, k, slot, gated, which, sdev, gate0);
 }
 
 // after a stream sync: fold the event intervals of `niter` profiled iterations into the totals
@@ -423,6 +429,8 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
     c->red = (double*)sc;
     c->part = c->red + 2 * (MAX_ITERS + 1);
     c->scal = c->part + RED_BLOCKS;
+    c->ctl = c->scal + 8;
+    c->ctl_hist = c->ctl + CT_SIZE;
     e = cudaMallocHost((void**)&c->pinned, (4 + 2 * (size_t)MAX_ITERS) * sizeof(double));
     if (e != cudaSuccess) {
         if (own) cudaFree(c->ws);
@@ -671,6 +679,69 @@ tf_status tf_advance_adaptive(tf_ctx* c, tf_adaptive* ctl, int n_accept, int max
     tf_status st = tf_adaptive_run(step_of_ctx, c, ctl, n_accept, max_attempts, t_advanced, hist, hist_cap, nhist);
     if (st != TF_OK && c->err.empty()) c->err = g_err;
     return st;
+}
+
+// Fig. 1 with every decision on the device (tf_control.cuh): attempts are enqueued a chunk at a time, each with max_iter
+// gated iterations; the host reads the control block and the history once per chunk.
+tf_status tf_advance_adaptive_device(tf_ctx* c, tf_adaptive* ctl, int n_accept, int max_attempts, double* t_advanced,
+                                     tf_step_record* hist, int hist_cap, int* nhist)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    if (!ctl || n_accept < 0 || hist_cap < 0 || (hist_cap > 0 && !hist))
+        return fail(c, TF_ERR_INVALID_ARG, "tf_advance_adaptive_device: NULL ctl or negative count");
+    if (!(ctl->dt > 0) || !(ctl->shrink > 0 && ctl->shrink < 1) || !(ctl->grow >= 1) || ctl->grow_after < 1 ||
+        !(ctl->dt_min > 0) || !(ctl->dt_max >= ctl->dt_min) || !std::isfinite(ctl->dt) || !std::isfinite(ctl->grow) ||
+        !std::isfinite(ctl->dt_max))
+        return fail(c, TF_ERR_INVALID_ARG, "tf_advance_adaptive_device: need dt > 0, 0 < shrink < 1, grow >= 1, grow_after >= 1, 0 < dt_min <= dt_max");
+    if (!c->have_state) return fail(c, TF_ERR_STATE, "no state set");
+    if (c->fixed_iters > 0 || c->max_rel_change > 0.0)
+        return fail(c, TF_ERR_UNSUPPORTED, "tf_advance_adaptive_device: fixed_iters and the extra solution criterion need the host controller");
+    if (max_attempts <= 0) max_attempts = 50 * std::max(n_accept, 1);
+    if (max_attempts > CT_HIST_CAP) max_attempts = CT_HIST_CAP;          // one run records at most CT_HIST_CAP attempts
+    CtlParams P;
+    P.shrink = ctl->shrink; P.grow = ctl->grow; P.dt_min = ctl->dt_min; P.dt_max = ctl->dt_max; P.tol = c->tol;
+    P.grow_after = ctl->grow_after; P.n_accept = n_accept; P.max_attempts = max_attempts; P.kmax = c->max_iter;
+    double init[CT_SIZE] = {0};
+    init[CT_DT] = std::min(ctl->dt, ctl->dt_max);
+    TF_CUDA(c, cudaMemcpyAsync(c->ctl, init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
+    TF_CUDA(c, cudaStreamSynchronize(c->stream));                        // `init` is on the stack
+    const size_t n = (size_t)c->P.nx * c->P.ny;
+    const unsigned gcopy = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)c->num_sms * 16);
+    std::vector<double> host(CT_SIZE + 4 * (size_t)CT_HIST_CAP);
+    double* hc = host.data();
+    int done = 0, attempts = 0, accepted = 0;
+    while (!done) {
+        const int chunk = std::max(1, std::min({n_accept - accepted + 1, 16, max_attempts - attempts + 1}));
+        for (int a = 0; a < chunk; ++a) {
+            ctl_begin_kernel<<<1, 256, 0, c->stream>>>(c->ctl, c->red, P);
+            for (int k = 0; k < c->max_iter; ++k)
+                TF_CUDA(c, launch_iteration(c, 1.0, k, -1, true, 3, c->ctl + CT_S, c->ctl + CT_GATE_RES));
+            ctl_end_kernel<<<1, 1, 0, c->stream>>>(c->ctl, c->red, c->ctl_hist, P);
+            ctl_commit_kernel<<<gcopy, 256, 0, c->stream>>>(n, c->uk, c->u, c->ctl);
+            count_launch(3);
+        }
+        TF_CUDA(c, cudaGetLastError());
+        TF_CUDA(c, cudaMemcpyAsync(hc, c->ctl, sizeof(double) * CT_SIZE, cudaMemcpyDeviceToHost, c->stream));
+        TF_CUDA(c, cudaStreamSynchronize(c->stream));
+        attempts = (int)hc[CT_ATTEMPTS];
+        accepted = (int)hc[CT_ACCEPTED];
+        done = (int)hc[CT_DONE];
+        if (!done && accepted >= n_accept) done = 1;
+        if (!done && attempts >= max_attempts) done = 3;
+    }
+    TF_CUDA(c, cudaMemcpyAsync(hc + CT_SIZE, c->ctl_hist, sizeof(double) * 4 * (size_t)std::min(attempts, CT_HIST_CAP),
+                               cudaMemcpyDeviceToHost, c->stream));
+    TF_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int a = 0; a < attempts && a < hist_cap && a < CT_HIST_CAP; ++a) {
+        const double* r = hc + CT_SIZE + 4 * a;
+        hist[a].dt = r[0]; hist[a].status = (int)r[1]; hist[a].newton_iters = (int)r[2]; hist[a].residual = r[3];
+    }
+    ctl->dt = hc[CT_DT];
+    if (t_advanced) *t_advanced = hc[CT_T];
+    if (nhist) *nhist = attempts;
+    if (done == 2) return fail(c, TF_NOT_CONVERGED, "tf_advance_adaptive_device: dt fell below dt_min");
+    if (done == 3 && accepted < n_accept) return fail(c, TF_NOT_CONVERGED, "tf_advance_adaptive_device: too many attempts");
+    return TF_OK;
 }
 
 tf_status tf_set_launch_ahead(tf_ctx* c, int batch)

@@ -1,0 +1,78 @@
+// tf_control.cuh -- the adaptive time-step controller of Fig. 1 taken ON THE DEVICE.
+//
+// The paper's controller runs on the host and reads a flag array after every iteration.
+// Here a whole run of attempts is enqueued without a host round trip: per attempt
+//   ctl_begin   (1 CTA)   : opens or closes the attempt (done / enough accepted steps), publishes s = dt/2, clears records
+//   K x 4 sweep kernels   : iteration k is gated on iteration k-1's record, iteration 0 on the attempt's gate record;
+//                           the forward kernels read s from device memory (Gate::s)
+//   ctl_end     (1 thread): reads the records in order -- the decision of S8 -- then accept / shrink / grow exactly as
+//                           tf_adaptive_run does on the host (same operations in the same order: same dt sequence, bit for bit)
+//   ctl_commit  (grid)    : u <- u_(k+1) if the attempt was accepted (the host path swaps pointers instead)
+// The host reads the control block and the attempt history once per enqueued chunk.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace tf {
+
+// control block, doubles: the layout the host reads back
+enum { CT_DT = 0, CT_S, CT_T, CT_ACCEPTED, CT_STREAK, CT_DONE, CT_GATE_RES, CT_GATE_BAD, CT_ATTEMPTS, CT_COMMIT, CT_SIZE = 16 };
+constexpr int CT_HIST_CAP = 1024;        // attempts recorded per run chunk: {dt, status, iters, res}
+// CT_DONE: 0 running, 1 n_accept reached, 2 dt fell below dt_min, 3 attempt cap reached
+
+struct CtlParams {
+    double shrink, grow, dt_min, dt_max, tol;
+    int grow_after, n_accept, max_attempts, kmax;
+};
+
+__global__ void ctl_begin_kernel(double* ctl, double* red, CtlParams P)
+{
+    for (int k = threadIdx.x; k < 2 * P.kmax; k += blockDim.x) red[k] = 0.0;
+    if (threadIdx.x == 0) {
+        if (ctl[CT_DONE] == 0.0 && ctl[CT_ACCEPTED] >= (double)P.n_accept) ctl[CT_DONE] = 1.0;
+        if (ctl[CT_DONE] == 0.0 && ctl[CT_ATTEMPTS] >= (double)P.max_attempts) ctl[CT_DONE] = 3.0;
+        ctl[CT_S] = 0.5 * ctl[CT_DT];
+        ctl[CT_GATE_RES] = __longlong_as_double(0x7ff0000000000000LL);   // +inf >= tol: open unless "bad"
+        ctl[CT_GATE_BAD] = ctl[CT_DONE] != 0.0 ? 1.0 : 0.0;
+        ctl[CT_COMMIT] = 0.0;
+    }
+}
+
+__global__ void ctl_end_kernel(double* ctl, const double* red, double* hist, CtlParams P)
+{
+    if (ctl[CT_GATE_BAD] != 0.0) return;                  // the attempt never ran
+    int k = 0, status = 1;                                // TF_NOT_CONVERGED
+    double res = 0.0;
+    for (int it = 0; it < P.kmax; ++it) {
+        k = it + 1;
+        res = red[2 * it];
+        const bool bad = red[2 * it + 1] != 0.0;
+        if (bad || res != res) break;
+        if (res < P.tol) { status = 0; break; }
+    }
+    const double dt = ctl[CT_DT];
+    const int a = (int)ctl[CT_ATTEMPTS];
+    if (a < CT_HIST_CAP) { hist[4 * a] = dt; hist[4 * a + 1] = (double)status; hist[4 * a + 2] = (double)k; hist[4 * a + 3] = res; }
+    ctl[CT_ATTEMPTS] = (double)(a + 1);
+    if (status == 0) {
+        ctl[CT_ACCEPTED] += 1.0;
+        ctl[CT_T] += dt;
+        ctl[CT_COMMIT] = 1.0;
+        const double streak = ctl[CT_STREAK] + 1.0;
+        if (streak >= (double)P.grow_after) { ctl[CT_DT] = fmin(dt * P.grow, P.dt_max); ctl[CT_STREAK] = 0.0; }
+        else ctl[CT_STREAK] = streak;
+    } else {
+        ctl[CT_STREAK] = 0.0;
+        const double nd = dt * P.shrink;
+        ctl[CT_DT] = nd;
+        if (nd < P.dt_min) ctl[CT_DONE] = 2.0;
+    }
+}
+
+__global__ void __launch_bounds__(256) ctl_commit_kernel(size_t n, const double* __restrict__ uk, double* __restrict__ u,
+                                                          const double* __restrict__ ctl)
+{
+    if (__ldcg(ctl + CT_COMMIT) == 0.0) return;
+    for (size_t p = (size_t)blockIdx.x * 256 + threadIdx.x; p < n; p += (size_t)gridDim.x * 256) u[p] = uk[p];
+}
+
+}  // namespace tf

@@ -232,7 +232,16 @@ __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefe
 // Every kernel of iteration k+1 first looks at iteration k's record {res, bad} (final: the writing kernel has
 // completed in stream order) and returns at once if that iteration already converged (res < tol), produced a bad
 // iterate, or a NaN -- so the iterate of the deciding iteration is left untouched.  p == nullptr: no gate.
-struct Gate { const double* p; double tol; };
+// s != nullptr (on-device adaptive controller): the kernels take s = dt/2 of the current attempt from device memory
+// and form their direction constants themselves, with the divisions of the host's make_dir (same bits).
+struct Gate { const double* p; double tol; const double* s; };
+__device__ __forceinline__ Dir dir_of(double s, double d)
+{
+    Dir D;
+    D.ca = s / (2.0 * d * d * d * d);
+    D.cb = s / (2.0 * d * d);
+    return D;
+}
 __device__ __forceinline__ bool gate_closed(const Gate& g)
 {
     if (g.p == nullptr) return false;

@@ -137,6 +137,7 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
                double* __restrict__ al, double* __restrict__ be, double* __restrict__ zz, Gate gate)
 {
     if (gate_closed(gate)) return;
+    if (gate.s) { const double sdev = __ldcg(gate.s); DX = dir_of(sdev, P.dx); DY = dir_of(sdev, P.dy); }
     // One CTA per SM: NSUB = 4 sub-problems q = warp % 4 (two adjacent strips x two halves), each with its own
     // ring and its own consumer + NP producers.  Warps w, w+4, w+8, ... share an SM sub-partition, so every
     // sub-partition gets exactly one consumer and NP producers (the consumers' dependent chains and the
@@ -444,6 +445,7 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
                double* __restrict__ alT, double* __restrict__ beT, double* __restrict__ zzT, Gate gate)
 {
     if (gate_closed(gate)) return;
+    if (gate.s) DX = dir_of(__ldcg(gate.s), P.dx);
     constexpr int SV = XW_CK * XW_LD;                 // doubles per value plane of a slot
     constexpr int NPL = 4;                            // planes per slot: A, p1, p2 of the forward face, right-hand side
     constexpr size_t RING = (size_t)NCH * NPL * SV * 8 + 16 * NCH;

@@ -37,6 +37,8 @@ SYMBOLS = {
                                        ctypes.POINTER(ctypes.c_int)]),
     "tf_advance_adaptive": (ctypes.c_int, [_vp, _vp, ctypes.c_int, ctypes.c_int, _dp, _vp, ctypes.c_int,
                                            ctypes.POINTER(ctypes.c_int)]),
+    "tf_advance_adaptive_device": (ctypes.c_int, [_vp, _vp, ctypes.c_int, ctypes.c_int, _dp, _vp, ctypes.c_int,
+                                                  ctypes.POINTER(ctypes.c_int)]),
     "tf_set_state": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
     "tf_get_state": (ctypes.c_int, [_vp, _vp, ctypes.c_int]),
     "tf_step": (ctypes.c_int, [_vp, ctypes.c_double, ctypes.POINTER(ctypes.c_int), _dp]),
@@ -335,18 +337,22 @@ class _StepRecord(ctypes.Structure):
 _STEP_FN = ctypes.CFUNCTYPE(ctypes.c_int, _vp, ctypes.c_double, ctypes.POINTER(ctypes.c_int), _dp)
 
 
-def advance_adaptive(ctx, dt, n_accept, grow=1.1, shrink=0.5, dt_max=0.1, dt_min=1e-12, max_attempts=None, grow_after=1):
+def advance_adaptive(ctx, dt, n_accept, grow=1.1, shrink=0.5, dt_max=0.1, dt_min=1e-12, max_attempts=None, grow_after=1,
+                     on_device=False, return_status=False):
     """Adaptive time stepping of Fig. 1 until `n_accept` steps were accepted: tf_advance_adaptive
     for a ThinFilm, tf_adaptive_run (the same controller, driven through a callback) for any object with a
     step(dt) -> (status, newton_iters, residual) method.  The controller itself is in the library; this marshals.
-    Returns (t, dt_next, history) with history = [(dt, status, newton_iters, residual), ...]."""
+    on_device=True: tf_advance_adaptive_device, the same controller with its decisions taken on the device.
+    Returns (t, dt_next, history) with history = [(dt, status, newton_iters, residual), ...]; with return_status=True a
+    fourth value, the status, is returned and a soft failure (dt below dt_min, attempt cap) does not raise."""
     L = lib()
     ctl = _Adaptive(float(dt), float(shrink), float(grow), int(grow_after), float(dt_min), float(dt_max))
     cap = int(max_attempts or 50 * max(n_accept, 1))
     hist = (_StepRecord * cap)()
     nh, t = ctypes.c_int(0), ctypes.c_double(0.0)
     if isinstance(ctx, ThinFilm):
-        st = L.tf_advance_adaptive(ctx._h, ctypes.byref(ctl), n_accept, cap, ctypes.byref(t), hist, cap, ctypes.byref(nh))
+        run = L.tf_advance_adaptive_device if on_device else L.tf_advance_adaptive
+        st = run(ctx._h, ctypes.byref(ctl), n_accept, cap, ctypes.byref(t), hist, cap, ctypes.byref(nh))
         handle = ctx._h
     else:
         def cb(_user, dt_, it_p, res_p):
@@ -357,10 +363,10 @@ def advance_adaptive(ctx, dt, n_accept, grow=1.1, shrink=0.5, dt_max=0.1, dt_min
         st = L.tf_adaptive_run(ctypes.cast(fn, _vp), None, ctypes.byref(ctl), n_accept, cap, ctypes.byref(t), hist, cap,
                                ctypes.byref(nh))
         handle = None
-    if st != OK:
+    if st != OK and not (return_status and st == NOT_CONVERGED):
         _err(handle, st, "advance_adaptive")
     out = [(hist[k].dt, hist[k].status, hist[k].newton_iters, hist[k].residual) for k in range(min(nh.value, cap))]
-    return t.value, ctl.dt, out
+    return (t.value, ctl.dt, out, st) if return_status else (t.value, ctl.dt, out)
 
 
 PENTA_LU, PENTA_PARTITION = 0, 1

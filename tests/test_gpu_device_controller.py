@@ -1,0 +1,121 @@
+"""tf_advance_adaptive_device (Fig. 1, with every decision on the device)
+against (a) the oracle's transcription of the flow chart on a run that DOES reject and (b) the host-side controller
+tf_advance_adaptive, which it must equal bit for bit."""
+import numpy as np
+import pytest
+
+from paper_1806_10550_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+K, HS = 100.0, 0.1
+
+
+@pytest.fixture(scope="module")
+def tf():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1806_10550_b200 import tf as tfmod
+    tfmod.lib()
+    return tfmod
+
+
+@pytest.fixture(scope="module")
+def tfo():
+    from oracle import tfo as o
+    o.build()
+    return o
+
+
+def rough_film(nx, ny, seed):
+    """grid-scale noise of 5 %: with max_iter = 10 a step of 0.08 does not converge, 0.01 does"""
+    rng = np.random.default_rng(seed)
+    return np.ascontiguousarray(1.0 + 0.05 * rng.uniform(-1, 1, (ny, nx)))
+
+
+@pytest.mark.parametrize("nx,ny,grow_after", [(96, 80, 1), (160, 128, 2), (61, 45, 1)])
+def test_device_controller_equals_flow_chart_and_host_controller(tf, tfo, nx, ny, grow_after):
+    cfg = inputs.config(0)
+    h = rough_film(nx, ny, seed=nx)
+    kw = dict(grow=1.6, shrink=0.5, dt_max=0.3, dt_min=1e-9, grow_after=grow_after)
+    o = tfo.ThinFilmOracle(nx, ny, cfg["dx"], cfg["dy"], K, HS, 3, 2)
+    o.set_newton(1e-10, 10, 0)
+    o.set_state(h)
+    t_o, dt_o, hist_o, failed = tfo.advance_adaptive(o, 0.08, 14, **kw)
+    assert not failed
+    runs = []
+    for on_device in (True, False):
+        g = tf.ThinFilm(nx, ny, cfg["dx"], cfg["dy"], K, HS, 3, 2)
+        g.set_newton(1e-10, 10, 0)
+        g.set_state(h)
+        t, dt, hist = tf.advance_adaptive(g, 0.08, 14, on_device=on_device, **kw)
+        runs.append((t, dt, hist, g.get_state(), g.mass()))
+        g.close()
+    dev, host = runs
+    # (b) bit for bit the host controller
+    assert dev[0] == host[0] and dev[1] == host[1] and dev[2] == host[2]
+    assert np.array_equal(dev[3], host[3])
+    # (a) the flow chart: the run rejects, shrinks, accepts, grows
+    st = [x[1] for x in dev[2]]
+    assert st == [x[1] for x in hist_o] and st.count(tf.NOT_CONVERGED) >= 2 and st.count(tf.OK) == 14
+    assert st[0] == tf.NOT_CONVERGED
+    assert [x[0] for x in dev[2]] == [x[0] for x in hist_o]                   # the dt sequence, exactly
+    assert [x[2] for x in dev[2]] == [x[2] for x in hist_o]                   # Newton counts
+    assert all(abs(a[3] - b[3]) <= 1e-4 * abs(b[3]) + 1e-15 for a, b in zip(dev[2], hist_o))   # residuals near tol carry rounding noise
+    assert (dev[0], dev[1]) == (t_o, dt_o)
+    assert np.max(np.abs(dev[3] - o.get_state())) <= 1e-8 * np.max(np.abs(dev[3]))
+    assert abs(dev[4] - o.mass()) <= 1e-13 * o.mass()
+
+
+def test_device_controller_halts_below_dt_min_with_the_last_accepted_state(tf, tfo):
+    """"if the new reduced time step is below some minimum, the numerical scheme halts and ends in a failed state"
+    (PAPER.md:254): dt_min above the step that would converge."""
+    cfg = inputs.config(0)
+    nx, ny = 96, 80
+    h = rough_film(nx, ny, seed=3)
+    outs = []
+    for on_device in (True, False):
+        g = tf.ThinFilm(nx, ny, cfg["dx"], cfg["dy"], K, HS, 3, 2)
+        g.set_newton(1e-10, 10, 0)
+        g.set_state(h)
+        t, dt, hist, st = tf.advance_adaptive(g, 0.08, 5, grow=1.1, shrink=0.5, dt_max=0.3, dt_min=0.03, on_device=on_device,
+                                              return_status=True)
+        outs.append((t, dt, hist, st, g.get_state()))
+        g.close()
+    dev, host = outs
+    assert dev[3] == host[3] == tf.NOT_CONVERGED
+    assert dev[:3] == host[:3] and dev[0] == 0.0 and dev[1] < 0.03
+    assert all(x[1] == tf.NOT_CONVERGED for x in dev[2]) and len(dev[2]) == 2         # 0.08, 0.04, then 0.02 < dt_min
+    assert np.array_equal(dev[4], h) and np.array_equal(host[4], h)
+
+
+def test_device_controller_attempt_cap_and_refusals(tf):
+    cfg = inputs.config(0)
+    g = tf.ThinFilm(96, 80, cfg["dx"], cfg["dy"], K, HS, 3, 2)
+    g.set_newton(1e-10, 10, 0)
+    g.set_state(rough_film(96, 80, seed=4))
+    t, dt, hist, st = tf.advance_adaptive(g, 0.08, 50, grow=1.0, shrink=0.9, dt_max=0.3, dt_min=1e-9, max_attempts=3,
+                                          on_device=True, return_status=True)
+    assert st == tf.NOT_CONVERGED and len(hist) == 3
+    g.set_newton(1e-10, 10, 4)                                                       # parity mode: host controller only
+    with pytest.raises(tf.TfError) as e:
+        tf.advance_adaptive(g, 0.01, 2, on_device=True)
+    assert e.value.status == tf.ERR_UNSUPPORTED
+    g.close()
+
+
+def test_config2_on_device_equals_host(tf):
+    """Config 2 as stated (4096^2, adaptive from 1e-3, x0.5 / x1.1, cap 0.1): 40 accepted steps with the decisions on the
+    device, identical to the host-driven run."""
+    cfg = inputs.config(2)
+    h = inputs.initial_condition(cfg)
+    outs = []
+    for on_device in (True, False):
+        g = tf.ThinFilm(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["kappa"], cfg["hstar"], cfg["n"], cfg["m"])
+        g.set_newton(cfg["tol"], cfg["max_iter"], 0)
+        g.set_state(h)
+        t, dt, hist = tf.advance_adaptive(g, cfg["dt"], 40, cfg["grow"], cfg["shrink"], cfg["dt_max"], cfg["dt_min"],
+                                          on_device=on_device)
+        outs.append((t, dt, hist, g.get_state()))
+        g.close()
+    assert outs[0][:3] == outs[1][:3] and np.array_equal(outs[0][3], outs[1][3])
+    assert len(outs[0][2]) == 40
