@@ -122,6 +122,23 @@ tf_status tf_step(tf_ctx* ctx, double dt, int* newton_iters, double* residual);
 tf_status tf_set_solution_criteria(tf_ctx* ctx, double max_rel_change);
 
 /*
+ * The criterion the paper names (PAPER.md:252 Note 2: "e.g. sufficiently small truncation error"), reading R25 of
+ * the local truncation error of the Crank-Nicolson / trapezoidal step (2.14) is -(dt^3/12) u_ttt.  It is
+ * estimated from quantities the step already holds: with u_t^n = -D(u^n) = 2 (b^n - u^n)/dt and the scheme's own relation
+ * u_t^{n+1} = 2 (u^{n+1} - u^n)/dt - u_t^n, the second time derivative at the middle of the step is
+ *     a_{n+1/2} = (u_t^{n+1} - u_t^n)/dt = 2 (u^{n+1} + u^n - 2 b^n)/dt^2,
+ * and u_ttt ~ (a_{n+1/2} - a_{n-1/2}) / ((dt + dt_prev)/2), a_{n-1/2} being kept from the previous accepted step (one
+ * field of the workspace).  A converged step is accepted only if
+ *     max_ij (dt^3/12) |u_ttt| / |u^{n+1}|  <=  max_rel_truncation,
+ * else tf_step returns TF_REJECTED with the state (and the stored a_{n-1/2}) untouched.  The first step after
+ * tf_set_state, tf_accept or tf_advance_adaptive_device has no history and is not tested.  0 = off (default).
+ * tf_last_truncation_estimate: the estimate of the last converged step that was tested (0 if none).
+ * One fused pass over four fields per step (40 B per grid point), order-independent max.
+ */
+tf_status tf_set_truncation_criterion(tf_ctx* ctx, double max_rel_truncation);
+tf_status tf_last_truncation_estimate(tf_ctx* ctx, double* estimate);
+
+/*
  * Adaptive time stepping of Fig. 1: take a step of size dt; if the solution criteria are met
  * (status TF_OK) advance time and, after `grow_after` consecutive accepted steps, multiply dt by `grow` (bounded by
  * dt_max); otherwise multiply dt by `shrink` and retry; fail (TF_NOT_CONVERGED) when dt falls below dt_min or after

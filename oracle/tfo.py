@@ -204,6 +204,38 @@ class CriteriaStepper:
         return st, it, res
 
 
+class TruncationStepper:
+    """step(dt) of a ThinFilmOracle with the criterion PAPER.md:252 Note 2 names ("sufficiently small truncation
+    error"), reading R25 of DESIGN.md, written out step by step:
+        u_t^n     = -D(u^n)                                     (the equation, PAPER.md:134 (2.1), with the oracle's D)
+        u_t^{n+1} = 2 (u^{n+1} - u^n)/dt - u_t^n                (the trapezoidal rule (2.14) solved for u_t^{n+1})
+        a_{n+1/2} = (u_t^{n+1} - u_t^n)/dt                      (second time derivative at the middle of the step)
+        u_ttt     = (a_{n+1/2} - a_{n-1/2}) / ((dt + dt_prev)/2)
+        estimate  = max (dt^3/12) |u_ttt| / |u^{n+1}|           (local error of the trapezoidal rule, relative to h)
+    A converged step whose estimate exceeds `limit` is undone (REJECTED); the first step has no a_{n-1/2} and is not
+    tested.  a_{n-1/2} is only replaced when a step is accepted."""
+    def __init__(self, oracle, limit):
+        self.o, self.limit, self.a_prev, self.dt_prev, self.last = oracle, limit, None, None, 0.0
+
+    def step(self, dt):
+        before = self.o.get_state()
+        st, it, res = self.o.step(dt)
+        if st != OK:
+            return st, it, res
+        after = self.o.get_state()
+        ut0 = -self.o.operator_D(before)
+        ut1 = 2.0 * (after - before) / dt - ut0
+        a = (ut1 - ut0) / dt
+        if self.a_prev is not None:
+            uttt = (a - self.a_prev) / (0.5 * (dt + self.dt_prev))
+            self.last = float(np.max(dt ** 3 / 12.0 * np.abs(uttt) / np.abs(after)))
+            if self.limit > 0 and not (self.last <= self.limit):
+                self.o.set_state(before)
+                return REJECTED, it, res
+        self.a_prev, self.dt_prev = a, dt
+        return st, it, res
+
+
 def advance_adaptive(stepper, dt, n_accept, grow, shrink, dt_max, dt_min, grow_after=1, max_attempts=None):
     """Flow chart of Fig. 1 over any object with step(dt) -> (status, iters, residual).  Returns
     (t, dt_next, history, failed) with history = [(dt, status, iters, residual), ...]."""

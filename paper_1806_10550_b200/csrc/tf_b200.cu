@@ -35,7 +35,7 @@ thread_local std::string g_err;
 size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 size_t field_bytes(int nx, int ny) { return align_up((size_t)nx * ny * sizeof(double)); }
 size_t scratch_bytes() { return align_up(sizeof(double) * (2 * (MAX_ITERS + 1) + RED_BLOCKS + 8 + CT_SIZE + 4 * CT_HIST_CAP)); }
-constexpr int NFIELDS = 7;   // u, uk, bn, w, alpha, beta, z
+constexpr int NFIELDS = 8;   // u, uk, bn, w, alpha, beta, z, a (second time derivative kept for the truncation criterion)
 
 }  // namespace
 
@@ -57,6 +57,9 @@ struct tf_ctx {
     double *pinned_red;                        // [2*MAX_ITERS] host pinned copy of the residual records
     double last_change;                        // max |u^{n+1} - u^n| / u^n of the last converged step (criterion on)
     double max_rel_change;                     // extra solution criterion (0 = off): reject a converged step that changed h by more
+    double *acc;                               // a_{n-1/2} of the last accepted step (truncation criterion; swaps with w on acceptance)
+    double max_trunc, last_trunc, dt_prev;     // truncation criterion: limit (0 = off), last estimate, step of the stored a
+    bool have_acc;                             // acc holds a_{n-1/2} of the step that led to the current state
     int spec_batch, last_iters;                // speculative launch-ahead: batch size (0 = off), iterations of the last accepted step
     int mid_y, mid_x;                          // split rows / columns of the two-sided sweeps
     int num_sms;
@@ -423,7 +426,7 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
         c->ws = (char*)dev_ws;
     }
     const size_t fb = field_bytes(nx, ny);
-    double** f[NFIELDS] = {&c->u, &c->uk, &c->bn, &c->w, &c->al, &c->be, &c->zz};
+    double** f[NFIELDS] = {&c->u, &c->uk, &c->bn, &c->w, &c->al, &c->be, &c->zz, &c->acc};
     for (int k = 0; k < NFIELDS; ++k) *f[k] = (double*)(c->ws + (size_t)k * fb);
     char* sc = c->ws + (size_t)NFIELDS * fb;
     c->red = (double*)sc;
@@ -440,6 +443,7 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
     c->pinned_red = c->pinned + 4;
     c->spec_batch = 2; c->last_iters = 1;
     c->max_rel_change = 0.0;
+    c->max_trunc = 0.0; c->last_trunc = 0.0; c->dt_prev = 0.0; c->have_acc = false;
     c->ubuf[0] = c->u; c->ubuf[1] = c->uk;
     {
         int dev = 0, sms = 148;
@@ -633,6 +637,22 @@ tf_status tf_set_solution_criteria(tf_ctx* c, double max_rel_change)
     return TF_OK;
 }
 
+tf_status tf_set_truncation_criterion(tf_ctx* c, double max_rel_truncation)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    if (!(max_rel_truncation >= 0.0) || !std::isfinite(max_rel_truncation))
+        return fail(c, TF_ERR_INVALID_ARG, "max_rel_truncation must be >= 0 and finite (0 = off)");
+    c->max_trunc = max_rel_truncation;
+    return TF_OK;
+}
+
+tf_status tf_last_truncation_estimate(tf_ctx* c, double* estimate)
+{
+    if (!c || !estimate) return TF_ERR_INVALID_ARG;
+    *estimate = c->last_trunc;
+    return TF_OK;
+}
+
 tf_status tf_adaptive_run(tf_step_fn step, void* user, tf_adaptive* ctl, int n_accept, int max_attempts, double* t_advanced,
                           tf_step_record* hist, int hist_cap, int* nhist)
 {
@@ -694,7 +714,7 @@ tf_status tf_advance_adaptive_device(tf_ctx* c, tf_adaptive* ctl, int n_accept, 
         !std::isfinite(ctl->dt_max))
         return fail(c, TF_ERR_INVALID_ARG, "tf_advance_adaptive_device: need dt > 0, 0 < shrink < 1, grow >= 1, grow_after >= 1, 0 < dt_min <= dt_max");
     if (!c->have_state) return fail(c, TF_ERR_STATE, "no state set");
-    if (c->fixed_iters > 0 || c->max_rel_change > 0.0)
+    if (c->fixed_iters > 0 || c->max_rel_change > 0.0 || c->max_trunc > 0.0)
         return fail(c, TF_ERR_UNSUPPORTED, "tf_advance_adaptive_device: fixed_iters and the extra solution criterion need the host controller");
     if (max_attempts <= 0) max_attempts = 50 * std::max(n_accept, 1);
     if (max_attempts > CT_HIST_CAP) max_attempts = CT_HIST_CAP;          // one run records at most CT_HIST_CAP attempts
@@ -737,6 +757,7 @@ tf_status tf_advance_adaptive_device(tf_ctx* c, tf_adaptive* ctl, int n_accept, 
         hist[a].dt = r[0]; hist[a].status = (int)r[1]; hist[a].newton_iters = (int)r[2]; hist[a].residual = r[3];
     }
     ctl->dt = hc[CT_DT];
+    c->have_acc = false;
     if (t_advanced) *t_advanced = hc[CT_T];
     if (nhist) *nhist = attempts;
     if (done == 2) return fail(c, TF_NOT_CONVERGED, "tf_advance_adaptive_device: dt fell below dt_min");
@@ -799,6 +820,7 @@ tf_status tf_set_state(tf_ctx* c, const double* h, int is_device_ptr)
     if (flag) return fail(c, TF_ERR_INVALID_ARG, "state has non-finite or non-positive values");
     std::swap(c->u, c->uk);
     c->have_state = true;
+    c->have_acc = false;                             // a new film has no time-derivative history
     return TF_OK;
 }
 
@@ -882,6 +904,25 @@ tf_status tf_step(tf_ctx* c, double dt, int* newton_iters, double* residual)
         c->last_change = c->pinned[0];
         if (!(c->last_change <= c->max_rel_change)) status = TF_REJECTED;
     }
+    bool commit_acc = false;
+    if (status == TF_OK && c->max_trunc > 0.0) {
+        // second criterion (reading R25): estimated local truncation error of the trapezoidal rule, relative to h
+        const size_t n = (size_t)c->P.nx * c->P.ny;
+        const int have = c->have_acc ? 1 : 0;
+        const double scale = have ? (dt * dt * dt / 12.0) / (0.5 * (dt + c->dt_prev)) : 0.0;
+        TF_CUDA(c, cudaMemsetAsync(c->scal + 3, 0, sizeof(double), c->stream));
+        truncation_kernel<<<RED_BLOCKS, RED_THREADS, 0, c->stream>>>(n, c->u, c->uk, c->bn, c->acc, c->w, 2.0 / (dt * dt), scale,
+                                                                     have, c->scal + 3);
+        count_launch(1);
+        TF_CUDA(c, cudaGetLastError());
+        TF_CUDA(c, cudaMemcpyAsync(c->pinned, c->scal + 3, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        TF_CUDA(c, cudaStreamSynchronize(c->stream));
+        c->last_trunc = have ? c->pinned[0] : 0.0;
+        if (have && !(c->last_trunc <= c->max_trunc)) status = TF_REJECTED;
+        else commit_acc = true;
+    }
+    if (status == TF_OK && commit_acc) { std::swap(c->acc, c->w); c->dt_prev = dt; c->have_acc = true; }
+    else if (status == TF_OK) c->have_acc = false;   // a step taken with the criterion off breaks the history
     if (status == TF_OK) std::swap(c->u, c->uk);     // pointer swap
     if (newton_iters) *newton_iters = k;
     if (residual) *residual = res;
@@ -925,6 +966,7 @@ tf_status tf_accept(tf_ctx* c)
     if (!c) return TF_ERR_INVALID_ARG;
     if (!c->have_state) return fail(c, TF_ERR_STATE, "no state set");
     std::swap(c->u, c->uk);
+    c->have_acc = false;
     return TF_OK;
 }
 

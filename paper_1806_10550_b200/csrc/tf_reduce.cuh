@@ -52,6 +52,32 @@ max_rel_change_kernel(size_t n, const double* __restrict__ u_old, const double* 
     if ((threadIdx.x & 31) == 0) atomic_max_nonneg(out, acc);
 }
 
+// Truncation-error estimate of the trapezoidal rule (PAPER.md:252 Note 2 "sufficiently small truncation error"; reading
+// R25 of DESIGN.md): the local error of (2.14) is -(dt^3/12) u_ttt.  With u_t^n = -D(u^n) = 2 (b^n - u^n)/dt and the
+// Crank-Nicolson relation u_t^{n+1} = 2 (u^{n+1} - u^n)/dt - u_t^n, the second time derivative at the midpoint of the step is
+//   a_{n+1/2} = (u_t^{n+1} - u_t^n)/dt = 2 (u^{n+1} + u^n - 2 b^n)/dt^2,
+// and u_ttt ~ (a_{n+1/2} - a_{n-1/2}) / ((dt + dt_prev)/2) with a_{n-1/2} kept from the previous accepted step.
+// Writes a_{n+1/2} to a_new (committed by the host only if the step is accepted) and max |tau| / |u^{n+1}| to out.
+// have_prev == 0 (first step after tf_set_state): only a_new is written.
+__global__ void __launch_bounds__(RED_THREADS)
+truncation_kernel(size_t n, const double* __restrict__ u_old, const double* __restrict__ u_new, const double* __restrict__ bn,
+                  const double* __restrict__ a_prev, double* __restrict__ a_new, double two_over_dt2, double scale,
+                  int have_prev, double* __restrict__ out)
+{
+    double acc = 0.0;
+    for (size_t p = (size_t)blockIdx.x * RED_THREADS + threadIdx.x; p < n; p += (size_t)RED_BLOCKS * RED_THREADS) {
+        const double un = u_new[p];
+        const double a = two_over_dt2 * ((un + u_old[p]) - 2.0 * bn[p]);
+        a_new[p] = a;
+        if (have_prev) {
+            const double r = scale * fabs(a - a_prev[p]) / fabs(un);     // scale = (dt^3/12) / ((dt + dt_prev)/2)
+            acc = (r != r) ? __longlong_as_double(0x7ff8000000000000LL) : ((acc != acc) ? acc : fmax(acc, r));
+        }
+    }
+    acc = warp_max_nonneg(acc);
+    if ((threadIdx.x & 31) == 0) atomic_max_nonneg(out, acc);
+}
+
 __global__ void __launch_bounds__(1024)
 sum_final_kernel(const double* __restrict__ part, double scale, double* __restrict__ out)
 {

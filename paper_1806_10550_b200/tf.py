@@ -33,6 +33,8 @@ SYMBOLS = {
     "tf_set_pressure": (ctypes.c_int, [_vp, ctypes.c_int, _dp, ctypes.c_int]),
     "tf_set_launch_ahead": (ctypes.c_int, [_vp, ctypes.c_int]),
     "tf_set_solution_criteria": (ctypes.c_int, [_vp, ctypes.c_double]),
+    "tf_set_truncation_criterion": (ctypes.c_int, [_vp, ctypes.c_double]),
+    "tf_last_truncation_estimate": (ctypes.c_int, [_vp, _dp]),
     "tf_adaptive_run": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, ctypes.c_int, _dp, _vp, ctypes.c_int,
                                        ctypes.POINTER(ctypes.c_int)]),
     "tf_advance_adaptive": (ctypes.c_int, [_vp, _vp, ctypes.c_int, ctypes.c_int, _dp, _vp, ctypes.c_int,
@@ -163,6 +165,20 @@ class ThinFilm:
         st = lib().tf_set_solution_criteria(self._h, float(max_rel_change))
         if st != OK:
             _err(self._h, st, "tf_set_solution_criteria")
+
+    def set_truncation_criterion(self, max_rel_truncation=0.0):
+        """tf_set_truncation_criterion: accept a converged step only if the estimated local truncation error of the
+        trapezoidal rule, relative to h, is <= max_rel_truncation (0 = off)."""
+        st = lib().tf_set_truncation_criterion(self._h, float(max_rel_truncation))
+        if st != OK:
+            _err(self._h, st, "tf_set_truncation_criterion")
+
+    def last_truncation_estimate(self):
+        v = ctypes.c_double(0.0)
+        st = lib().tf_last_truncation_estimate(self._h, ctypes.byref(v))
+        if st != OK:
+            _err(self._h, st, "tf_last_truncation_estimate")
+        return v.value
 
     def set_pressure(self, kind, params=()):
         """tf_set_pressure: PI_POWER (), PI_NLC (cap0, cap1, K, b, N, beta, w), PI_POLYMER (cap0, cap1, C, A_SiOx, A_Si, d)."""

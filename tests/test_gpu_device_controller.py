@@ -119,3 +119,51 @@ def test_config2_on_device_equals_host(tf):
         g.close()
     assert outs[0][:3] == outs[1][:3] and np.array_equal(outs[0][3], outs[1][3])
     assert len(outs[0][2]) == 40
+
+
+# ------------------------------------------------------------------ the truncation-error criterion (PAPER.md:252 Note 2, R25)
+def test_truncation_criterion_against_the_oracle_transcription(tf, tfo):
+    """tf_set_truncation_criterion + tf_advance_adaptive against oracle/tfo.py's TruncationStepper under the same flow
+    chart: same accept / REJECTED sequence, same time steps, same Newton counts, estimates equal to 1e-3, same film.
+    The limit is taken from a first oracle run so that the growing step is rejected several times."""
+    cfg = inputs.config(0)
+    nx, ny = 96, 80
+    x = (np.arange(nx) + 0.5) / nx
+    y = (np.arange(ny) + 0.5) / ny
+    h = np.ascontiguousarray(1.0 + 0.2 * np.cos(2 * np.pi * x)[None, :] * np.cos(np.pi * y)[:, None])   # smooth: a clean u_ttt
+    kw = dict(grow=1.5, shrink=0.5, dt_max=1.0, dt_min=1e-9, grow_after=1)
+    DT0 = 0.05
+    o = tfo.ThinFilmOracle(nx, ny, cfg["dx"], cfg["dy"], K, HS, 3, 2)
+    o.set_newton(1e-14, 200, 0)                               # the estimate divides differences of iterates by dt^2
+    o.set_state(h)
+    probe = tfo.TruncationStepper(o, 0.0)
+    ests = []
+    for _ in range(4):
+        assert probe.step(DT0)[0] == 0
+        ests.append(probe.last)
+    limit = 2.0 * ests[-1]                                    # a step 1.5x longer (tau ~ dt^3: x3.4) violates it
+    assert ests[-1] > 1e-11, ests
+    o.set_state(h)
+    stepper = tfo.TruncationStepper(o, limit)
+    t_o, dt_o, hist_o, failed = tfo.advance_adaptive(stepper, DT0, 12, **kw)
+    assert not failed
+    g = tf.ThinFilm(nx, ny, cfg["dx"], cfg["dy"], K, HS, 3, 2)
+    g.set_newton(1e-14, 200, 0)
+    g.set_truncation_criterion(limit)
+    g.set_state(h)
+    t_g, dt_g, hist_g = tf.advance_adaptive(g, DT0, 12, **kw)
+    st = [x_[1] for x_ in hist_g]
+    assert st == [x_[1] for x_ in hist_o] and st.count(tf.REJECTED) >= 2 and st[0] == tf.OK
+    assert [x_[0] for x_ in hist_g] == [x_[0] for x_ in hist_o] and (t_g, dt_g) == (t_o, dt_o)
+    assert [x_[2] for x_ in hist_g] == [x_[2] for x_ in hist_o]
+    assert abs(g.last_truncation_estimate() - stepper.last) <= 1e-3 * stepper.last
+    assert np.max(np.abs(g.get_state() - o.get_state())) <= 1e-9 * np.max(np.abs(h))
+    # one estimate on its own: two equal steps from the same film, GPU against the oracle's transcription
+    g.set_truncation_criterion(1.0)
+    g.set_state(h)
+    o.set_state(h)
+    s2 = tfo.TruncationStepper(o, 1.0)
+    for _ in range(2):
+        assert g.step(DT0)[0] == 0 and s2.step(DT0)[0] == 0
+    assert abs(g.last_truncation_estimate() - s2.last) <= 1e-3 * s2.last and s2.last > 0
+    g.close()
