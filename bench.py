@@ -42,7 +42,9 @@ def parse():
                     help="power: BASELINE.json's Pi (headline); nlc: the paper's NLC pressure (1.8)-(1.9) with (1.11), on the "
                          "same grid with the paper's spacing 0.05 and a 0.2 film (side measurement, row f-1)")
     ap.add_argument("--nsys", type=int, default=0, help="config 4 only: number of systems (0: the config's 16384)")
-    ap.add_argument("--variant", default="lu", choices=["lu", "partition"], help="config 4 only: tf_penta_solve_ex variant")
+    ap.add_argument("--variant", default="lu", choices=["lu", "partition", "pcr"],
+                    help="config 4 only: tf_penta_solve_ex variant (pcr: parallel cyclic reduction, systems along rows, length <= 2048)")
+    ap.add_argument("--length", type=int, default=0, help="config 4 only: unknowns per system (0: the config's 16384)")
     ap.add_argument("--nparts", type=int, default=0, help="config 4 only: chunks per system of the partition variant (0: automatic)")
     ap.add_argument("--cusparse", action="store_true", help="config 4 only: also time cuSPARSE's interleaved-batch routine (context)")
     ap.add_argument("--slabs", action="store_true",
@@ -473,15 +475,17 @@ def run_penta(args, cfg):
     if int(os.environ.get("RANK", "0")) != 0:
         return
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
-    n = cfg["nrow"]
-    nsys = args.nsys or n
-    variant = tf.PENTA_PARTITION if args.variant == "partition" else tf.PENTA_LU
+    n = args.length or cfg["nrow"]
+    nsys = args.nsys or cfg["nrow"]
+    variant = {"partition": tf.PENTA_PARTITION, "pcr": tf.PENTA_PCR}.get(args.variant, tf.PENTA_LU)
     gen = torch.Generator(device="cuda").manual_seed(cfg["seed"])
     peak, peak_src = measured_peak()
     small = 7 * nsys * n * 8 < 4 * 126e6          # working set not far above L2: flush between timed solves
     flush = torch.empty(64 * 1024 * 1024, dtype=torch.float64, device="cuda") if small else None
     res = {}
     for direction, name in ((1, "along_columns_y"), (0, "along_rows_x")):
+        if variant == tf.PENTA_PCR and direction == 1:
+            continue                                    # the cyclic-reduction variant exists for the x-sweep shape only
         nrow, ncol = (nsys, n) if direction == 0 else (n, nsys)
         U = lambda lo, hi: torch.rand(nrow, ncol, dtype=torch.float64, device="cuda", generator=gen) * (hi - lo) + lo
         e, c, a, b, y = U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1)
@@ -514,6 +518,8 @@ def run_penta(args, cfg):
             torch.cuda.synchronize()
             ms = ev0.elapsed_time(ev1) / args.steps
         bpu = 104 if chunks == 1 else 200          # partition: 2 x 48 B interface pass + 104 B chunk solves
+        if variant == tf.PENTA_PCR:
+            bpu = 56                                # six arrays in, one out: the compulsory traffic
         res[name] = {"ms": ms, "chunks": chunks, "unknowns_per_s": nsys * n / (ms * 1e-3), "alg_bytes_per_unknown": bpu,
                      "alg_gbs": bpu * nsys * n / (ms * 1e-3) / 1e9, "frac_of_peak": bpu * nsys * n / (ms * 1e-3) / 1e9 / peak}
         if args.cusparse and direction == 1:

@@ -248,12 +248,18 @@ tf_status tf_penta_solve(int nrow, int ncol, int dir,
  *                       four end unknowns and the four unknowns outside it, (2) the reduced system of 4*nparts end
  *                       unknowns per system is solved, (3) all chunks are solved independently with corrected
  *                       right-hand sides.  Same solution up to rounding; for few, long systems (nsys << 20 000).
+ *   TF_PENTA_PCR        parallel cyclic reduction (PAPER.md:647 names "cyclical reduction"), systems along rows only
+ *                       (dir = 0): one CTA holds one system in shared memory as a block-tridiagonal system of 2 x 2
+ *                       blocks, one thread per pair of unknowns, ceil(log2(len/2)) levels; global traffic is the
+ *                       compulsory 56 B per unknown, ~76 fp64 operations per pair and level.  64 <= ncol <= 2048, ncol
+ *                       even, 16-byte aligned arrays; TF_ERR_UNSUPPORTED otherwise.  The x-sweep alternative measured
+ *                       against the LU; not used by tf_step.
  * tf_penta_partition_chunks returns the chunk count that will be used (1 = the shape falls back to TF_PENTA_LU:
  * odd nrow or ncol, fewer than 32 systems, or systems shorter than 192); 0 for invalid arguments.
  * dev_ws needs tf_penta_workspace_bytes_ex(nrow, ncol, dir, variant, nparts) bytes.  Arrays must be 16-byte
  * aligned for TF_PENTA_PARTITION (TF_ERR_UNSUPPORTED otherwise).
  */
-typedef enum { TF_PENTA_LU = 0, TF_PENTA_PARTITION = 1 } tf_penta_variant;
+typedef enum { TF_PENTA_LU = 0, TF_PENTA_PARTITION = 1, TF_PENTA_PCR = 2 } tf_penta_variant;
 int       tf_penta_partition_chunks(int nrow, int ncol, int dir, int nparts);
 size_t    tf_penta_workspace_bytes_ex(int nrow, int ncol, int dir, int variant, int nparts);
 tf_status tf_penta_solve_ex(int nrow, int ncol, int dir, int variant, int nparts,

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtf_b200.so")
 SOURCES = [os.path.join(CSRC, "tf_b200.cu")]
-HEADERS = [os.path.join(CSRC, f) for f in ("tf_device.cuh", "tf_reduce.cuh", "tf_penta.cuh", "tf_async.cuh", "tf_bwd.cuh", "tf_tma.cuh", "tf_fwd.cuh", "tf_partition.cuh", "tf_topo.cuh", "tf_spectrum.cuh", "tf_blocks.cuh", "tf_control.cuh")] + \
+HEADERS = [os.path.join(CSRC, f) for f in ("tf_device.cuh", "tf_reduce.cuh", "tf_penta.cuh", "tf_async.cuh", "tf_bwd.cuh", "tf_tma.cuh", "tf_fwd.cuh", "tf_partition.cuh", "tf_topo.cuh", "tf_spectrum.cuh", "tf_blocks.cuh", "tf_control.cuh", "tf_pcr.cuh")] + \
           [os.path.join(os.path.dirname(HERE), "include", "tf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--fmad=true", "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v", "-ldl"]

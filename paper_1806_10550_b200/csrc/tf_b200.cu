@@ -10,6 +10,7 @@
 #include "tf_spectrum.cuh"
 #include "tf_blocks.cuh"
 #include "tf_control.cuh"
+#include "tf_pcr.cuh"
 #include <dlfcn.h>
 
 #include <algorithm>
@@ -400,7 +401,6 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
     Params& P = c->P;
     P.nx = nx; P.ny = ny; P.dx = dx; P.dy = dy;
     P.rdx2 = 1.0 / (dx * dx); P.rdy2 = 1.0 / (dy * dy);
-    P.m2r = -2.0 * (P.rdx2 + P.rdy2);
     P.n = n; P.m = m;
     double hm = 1.0, hn = 1.0;
     for (int k = 0; k < m; ++k) hm *= hstar;
@@ -1172,9 +1172,32 @@ tf_status tf_penta_solve_ex(int nrow, int ncol, int dir, int variant, int nparts
     if (nrow < 1 || ncol < 1 || (dir != 0 && dir != 1)) return fail(nullptr, TF_ERR_INVALID_ARG, "bad shape or dir");
     if ((dir ? nrow : ncol) < 3) return fail(nullptr, TF_ERR_INVALID_ARG, "system length must be >= 3");
     if (!e || !c || !d || !a || !b || !rhs || !x || !dev_ws) return fail(nullptr, TF_ERR_INVALID_ARG, "NULL pointer");
-    if (variant != TF_PENTA_LU && variant != TF_PENTA_PARTITION) return fail(nullptr, TF_ERR_UNSUPPORTED, "unknown variant");
+    if (variant != TF_PENTA_LU && variant != TF_PENTA_PARTITION && variant != TF_PENTA_PCR)
+        return fail(nullptr, TF_ERR_UNSUPPORTED, "unknown variant");
     if (nparts < 0) return fail(nullptr, TF_ERR_INVALID_ARG, "nparts < 0");
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (variant == TF_PENTA_PCR) {
+        const double* in6[6] = {e, c, d, a, b, rhs};
+        bool ok = dir == 0 && ncol % 2 == 0 && ncol >= 64 && ncol <= 2048 && ((uintptr_t)x % 16 == 0);
+        for (int k = 0; k < 6; ++k) ok = ok && ((uintptr_t)in6[k] % 16 == 0);
+        if (!ok) return fail(nullptr, TF_ERR_UNSUPPORTED, "TF_PENTA_PCR: dir = 0, even 64 <= ncol <= 2048, 16-byte aligned arrays");
+        const int nb = ncol / 2;
+        const size_t sm = (size_t)PCR_VALS * nb * sizeof(double);
+        static DevOnce ready;
+        if (!ready.done()) {
+            cudaError_t ee = opt_in_smem(penta_row_pcr_kernel<512>, (size_t)PCR_VALS * 512 * sizeof(double));
+            if (ee == cudaSuccess) ee = opt_in_smem(penta_row_pcr_kernel<1024>, (size_t)PCR_VALS * 1024 * sizeof(double));
+            if (ee != cudaSuccess) return cuda_fail(nullptr, ee, "cudaFuncSetAttribute");
+            ready.mark();
+        }
+        const unsigned nthr = (unsigned)((nb + 31) / 32 * 32);
+        if (nb <= 512) penta_row_pcr_kernel<512><<<(unsigned)nrow, nthr, sm, st>>>(ncol, e, c, d, a, b, rhs, x);
+        else penta_row_pcr_kernel<1024><<<(unsigned)nrow, nthr, sm, st>>>(ncol, e, c, d, a, b, rhs, x);
+        count_launch(1);
+        cudaError_t le = cudaGetLastError();
+        if (le != cudaSuccess) return cuda_fail(nullptr, le, "penta_row_pcr launch");
+        return TF_OK;
+    }
     const size_t fb = align_up((size_t)nrow * ncol * sizeof(double));
     if (variant == TF_PENTA_PARTITION) {
         const int P = tf_penta_partition_chunks(nrow, ncol, dir, nparts);

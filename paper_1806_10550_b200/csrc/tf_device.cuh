@@ -18,7 +18,6 @@ struct Params {
     int nx, ny;
     double dx, dy;
     double rdx2, rdy2;      // 1/dx^2, 1/dy^2
-    double m2r;             // -2 (rdx2 + rdy2)
     int n, m;               // Pi exponents, n > m >= 1
     double cm, cn;          // kappa*m*hstar^m, kappa*n*hstar^n
     double mp[10];          // constants of the NLC / polymer pressures (tf_set_pressure), see cell_functions

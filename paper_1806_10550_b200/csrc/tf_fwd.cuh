@@ -22,15 +22,9 @@ namespace tf {
 #ifndef TF_ROTATE_Y
 #define TF_ROTATE_Y 1
 #endif
-#ifndef TF_WAIT_HINT_NS
-#define TF_WAIT_HINT_NS 0
-#endif
-#ifndef TF_Y_TRIM
-#define TF_Y_TRIM 0
-#endif
-#ifndef TF_Y_ELIM1
-#define TF_Y_ELIM1 0
-#endif
+// Probe builds (-DTF_EXP_NOSTORE / TF_EXP_STORE_L2 / TF_EXP_NOCONS / TF_EXP_NOPROD / TF_EXP_NOZ / TF_PERT_SHFL / TF_PERT_FMA /
+// TF_PERT_INT): timing-only variants of the y forward kernel that leave out or add one ingredient; they compute wrong
+// results on purpose.  DESIGN.md section 6 quotes what they measured; no product build defines them.
 constexpr int YW_VALID = 28;     // columns per strip (lanes 2..29; lanes 0,1,30,31 are x-halo)
 
 // rolling state of a thread marching down a column
@@ -53,12 +47,7 @@ __device__ __forceinline__ void y_advance(YState& S, int j, double hp2, const Pa
     const unsigned FULL = 0xffffffffu;
     const int ny = P.ny;
     const double hL = __shfl_up_sync(FULL, S.hp1, 1), hR = __shfl_down_sync(FULL, S.hp1, 1);
-#if TF_Y_TRIM
-    // 5 fp64 instead of 6: lap h = rdx2 (hL + hR) + rdy2 (h(j+2) + h(j)) - 2 (rdx2 + rdy2) h(j+1)
-    const double Lp = fma(P.rdy2, hp2 + S.h0, fma(P.rdx2, hL + hR, P.m2r * S.hp1));
-#else
     const double Lp = fma((hL + hR) - 2.0 * S.hp1, P.rdx2, ((hp2 + S.h0) - 2.0 * S.hp1) * P.rdy2);
-#endif
     const Cell cp = cell_functions<N, M>(S.hp1, P);
     Face fp = {0.0, 0.0, 0.0};
     double phip = 0.0;
@@ -240,11 +229,7 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
             }
             __syncwarp();
             issue_tma(c + NP);                                  // staging is free again: fetch my next chunk
-#if TF_WAIT_HINT_NS
-            mbar_wait_hint(empty + s, ((c / NCH) & 1) ^ 1, TF_WAIT_HINT_NS);
-#else
             mbar_wait(empty + s, ((c / NCH) & 1) ^ 1);
-#endif
             // slot row of chunk row r: r (half 0), RP-1-r (half 1)
             double* st = sm + (size_t)s * 5 * SV + (dir ? RP - 1 : 0) * 32 + lane;
             const int sstep = dir ? -32 : 32;
@@ -301,47 +286,6 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
         }
     } else {
         // ------------------------------------------------------------------ consumer: the recurrence.
-#if TF_Y_ELIM1
-        // textbook row elimination (12 fp64 + 1 MUFU per row, 75-cycle chain): with four teams per SM the kernel is
-        // bound by instruction throughput, not by the chain, and elim2_row's shorter chain costs 4 more fp64 per row
-        Elim S = {0, 0, 0, 0, 0, 0};
-        double e = 0.0;
-        const int step = dir ? -nx : nx;
-        int o = (dir ? ny - 1 : 0) * nx + i;
-        const int offc = dir ? 3 * SV : SV, offa = dir ? SV : 3 * SV;
-        for (int c = 0; c < nchunk; ++c) {
-            const int s = c % NCH;
-            mbar_wait(full + s, (c / NCH) & 1);
-            const double* st = sm + (size_t)s * 5 * SV + lane;
-            const double* stc = st + offc;
-            const double* sta = st + offa;
-            const int nrow = min(RP, nrows - c * RP);
-            if (nrow == RP) {
-#pragma unroll
-                for (int r = 0; r < RP; ++r) {
-                    const double A = st[r * 32], cc = stc[r * 32], q = st[2 * SV + r * 32], a = sta[r * 32];
-                    const double R = st[4 * SV + r * 32];
-                    double va, vb, vz;
-                    elim_row(S, e, cc, q, a, A, R, va, vb, vz);
-                    e = A;
-                    st3_if(outl, al + o, va, be + o, vb, zz + o, vz);
-                    o += step;
-                }
-            } else {
-                for (int r = 0; r < nrow; ++r) {
-                    const double A = st[r * 32], cc = stc[r * 32], q = st[2 * SV + r * 32], a = sta[r * 32];
-                    const double R = st[4 * SV + r * 32];
-                    double va, vb, vz;
-                    elim_row(S, e, cc, q, a, A, R, va, vb, vz);
-                    e = A;
-                    st3_if(outl, al + o, va, be + o, vb, zz + o, vz);
-                    o += step;
-                }
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(empty + s);
-        }
-#else
         // elim2_row emits the coefficients of the PREVIOUS row, so every store goes one row behind.
         Elim2 S = elim2_init();
         double e = 0.0;
@@ -398,7 +342,6 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
         if (xacc == 0x12345) vz = 1.0;
 #endif
         st3_if(outl, al + o, va, be + o, vb, zz + o, vz);
-#endif
     }
 }
 
@@ -509,13 +452,8 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
             }
 #endif
             const int g0 = 2 * t, g1 = 2 * t + 1;             // global slot numbers of this tile
-#if TF_WAIT_HINT_NS
-            mbar_wait_hint(empty + g0 % NCH, ((g0 / NCH) & 1) ^ 1, TF_WAIT_HINT_NS);
-            mbar_wait_hint(empty + g1 % NCH, ((g1 / NCH) & 1) ^ 1, TF_WAIT_HINT_NS);
-#else
             mbar_wait(empty + g0 % NCH, ((g0 / NCH) & 1) ^ 1);
             mbar_wait(empty + g1 % NCH, ((g1 / NCH) & 1) ^ 1);
-#endif
             double* st = sm + (size_t)((slot_sel ? g1 : g0) % NCH) * NPL * SV + kc * XW_LD;
             // one row of the tile; INTERIOR: every face of the tile is an interior, unfolded face and every
             // column belongs to this half -- no boundary selects (all tiles but the first, last and the split one)

@@ -46,21 +46,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 {
     while (!mbar_try_wait(bar, parity)) __nanosleep(TF_WAIT_SLEEP_NS);
 }
-// The same wait with a suspend-time hint: the hardware parks the thread until the phase completes or `ns` have
-// passed, so a long wait costs a handful of probes instead of one every TF_WAIT_SLEEP_NS.
-__device__ __forceinline__ void mbar_wait_hint(uint64_t* bar, uint32_t parity, uint32_t ns)
-{
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n"
-            ".reg .pred p;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n"
-            "selp.u32 %0, 1, 0, p;\n"
-            "}\n" : "=r"(ok) : "r"(s_addr(bar)), "r"(parity), "r"(ns) : "memory");
-    } while (!ok);
-}
-
 // global -> shared, 2-D box at (c0 = inner/contiguous coordinate, c1 = outer coordinate)
 __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar)
 {

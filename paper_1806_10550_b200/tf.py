@@ -385,7 +385,7 @@ def advance_adaptive(ctx, dt, n_accept, grow=1.1, shrink=0.5, dt_max=0.1, dt_min
     return (t.value, ctl.dt, out, st) if return_status else (t.value, ctl.dt, out)
 
 
-PENTA_LU, PENTA_PARTITION = 0, 1
+PENTA_LU, PENTA_PARTITION, PENTA_PCR = 0, 1, 2
 
 
 def penta_partition_chunks(nrow, ncol, direction, nparts=0):

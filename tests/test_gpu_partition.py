@@ -109,3 +109,38 @@ def test_partition_full_length_few_systems(tf, tfo, direction):
         x, ref = solve_both(tf, tfo, arrs, direction, 0)
         assert rel_inf(x, ref) <= TOL[kind]
         assert backward_error(arrs, x) <= 2e-14
+
+
+@pytest.mark.parametrize("nsys,length", [(37, 64), (8, 1024), (5, 2048), (16, 130), (3, 1000)])
+def test_cyclic_reduction_variant_rows(tf, nsys, length):
+    """TF_PENTA_PCR (parallel cyclic reduction on 2 x 2 blocks, systems along rows): config-4 systems against the
+    oracle's LU (<= 1e-12) and by backward error (needs no oracle); weakly dominant bending systems by backward error."""
+    import torch
+    from oracle import tfo
+    for gen, tol in ((lambda: inputs.penta_system(nsys, length, seed=length), 1e-12),
+                     (lambda: inputs.penta_system_bending(nsys, length, seed=length, sigma=1e2), None)):
+        e, c, d, a, b, y = gen()
+        x = tf.penta_solve(0, *[torch.from_numpy(t).cuda() for t in (e, c, d, a, b, y)], variant=tf.PENTA_PCR)
+        torch.cuda.synchronize()
+        x = x.cpu().numpy()
+        if tol is not None:
+            ref = tfo.penta_solve(0, e, c, d, a, b, y)
+            assert np.max(np.abs(x - ref)) <= tol * np.max(np.abs(ref))
+        Ax = d * x
+        Ax[:, 1:] += c[:, 1:] * x[:, :-1]
+        Ax[:, 2:] += e[:, 2:] * x[:, :-2]
+        Ax[:, :-1] += a[:, :-1] * x[:, 1:]
+        Ax[:, :-2] += b[:, :-2] * x[:, 2:]
+        normA = np.max(np.abs(e) + np.abs(c) + np.abs(d) + np.abs(a) + np.abs(b))
+        assert np.max(np.abs(Ax - y)) / (normA * np.max(np.abs(x)) + np.max(np.abs(y))) <= 1e-13
+
+
+def test_cyclic_reduction_variant_refuses_other_shapes(tf):
+    import torch
+    t = [torch.ones(8, 4096, dtype=torch.float64, device="cuda") for _ in range(6)]
+    with pytest.raises(tf.TfError) as err:
+        tf.penta_solve(0, *t, variant=tf.PENTA_PCR)
+    assert err.value.status == tf.ERR_UNSUPPORTED
+    t = [torch.ones(256, 64, dtype=torch.float64, device="cuda") for _ in range(6)]
+    with pytest.raises(tf.TfError):
+        tf.penta_solve(1, *t, variant=tf.PENTA_PCR)
