@@ -105,14 +105,14 @@ def measured_peak():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-NCU_SUMMARY = os.path.join("profiles", "r01_v7_ncu_full_summary.csv")
+NCU_SUMMARY = os.path.join("profiles", "r02_ncu_full_summary.csv")
 NCU_KERNEL = {"y_forward": "yfwd_ws_kernel", "y_backward": "ybwd2_tma_kernel", "x_forward": "xfwd_ws_kernel",
               "x_backward_update": "xbwd2_tma_kernel"}
 
 
 def ncu_traffic(kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` at 8192^2, from the committed
-    ncu --set full summary (profiles/r01_v7_ncu.md names the command), or None."""
+    ncu --set full summary (profiles/r02_ncu.md names the command), or None."""
     import csv
     p = os.path.join(ROOT, NCU_SUMMARY)
     try:

@@ -273,9 +273,10 @@ cudaError_t launch_yfwd(tf_ctx* c, const CUtensorMap& mu, int tma, const Params&
 {
     // producers per team: YW_NP with four teams per CTA; grids with two teams per CTA (sides <= ~4100) have SM capacity to spare
     constexpr int NP = NSUB == 2 ? TF_YW_NP2 : YW_NP;
-    constexpr size_t SM = NSUB * (size_t)YW_NSTG * 5 * YW_RP * 32 * 8 + NSUB * NP * (size_t)(2 * YW_RP + 4) * 32 * 8 +
-                          (2 * NSUB * YW_NSTG + NSUB * NP) * 8;
-    auto kern = yfwd_ws_kernel<N, M, FIRST, NP, YW_RP, YW_NSTG, NSUB>;
+    constexpr int NSTG = NP > YW_NSTG ? NP : YW_NSTG;                  // ring slots >= producers (see the kernel)
+    constexpr size_t SM = NSUB * (size_t)NSTG * 5 * YW_RP * 32 * 8 + NSUB * NP * (size_t)(2 * YW_RP + 4) * 32 * 8 +
+                          (2 * NSUB * NSTG + NSUB * NP) * 8;
+    auto kern = yfwd_ws_kernel<N, M, FIRST, NP, YW_RP, NSTG, NSUB>;
     static DevOnce ready;
     if (!ready.done()) {
         cudaError_t e = opt_in_smem(kern, SM);
