@@ -93,6 +93,15 @@ tf_status tf_set_newton(tf_ctx* ctx, double tol, int max_iter, int fixed_iters);
  * those of batch = 0.  0 <= batch <= 64. */
 tf_status tf_set_launch_ahead(tf_ctx* ctx, int batch);
 
+/* Launch-ahead batches through CUDA graphs (default on): a batch {first iteration, count, which buffer holds u^n, dt}
+ * that recurs is captured once (at its second occurrence) and replayed from then on -- the same launches with the same
+ * arguments, so results are bit-identical; what changes is the launch cost (per step on a 128^2 grid: about a dozen
+ * iterations of four ~10 us kernels).  Setters that change a launch argument (tf_set_newton, tf_set_pressure) drop the
+ * captured graphs; profiled steps (tf_set_profiling) and fixed_iters steps are launched plainly.  At most 16 graphs are
+ * kept per context (least recently used goes).  tf_graph_replays: how many batches were replayed so far. */
+tf_status tf_set_cuda_graphs(tf_ctx* ctx, int on);
+tf_status tf_graph_replays(tf_ctx* ctx, unsigned long long* replays);
+
 /* Copy nx*ny doubles into the context as u^n.  `h` is a device pointer if is_device_ptr != 0,
  * else a host pointer.  Rejects non-finite or non-positive values (Pi is singular at h = 0)
  * with TF_ERR_INVALID_ARG; the previous state is then kept. */

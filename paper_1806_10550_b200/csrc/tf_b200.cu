@@ -70,6 +70,15 @@ struct tf_ctx {
     bool tma_yf;                               // y forward producers stage their inputs by TMA
     CUtensorMap mUy[2], mBn;                   // state buffers / b^n as [ny][nx], boxes (RP+4) x 32 and RP x 32
     double* ubuf[2];                           // buffer addresses mU[0], mU[1] were encoded for
+    // CUDA graphs of launch-ahead batches (small grids are launch-bound): a batch {first iteration, count, which buffer
+    // holds u^n, dt/2} that comes back is captured once and replayed; any setter that changes a launch argument clears them
+    struct GraphEntry { int k0, n, parity; double s; cudaGraphExec_t exec; unsigned long long stamp; };
+    std::vector<GraphEntry> graphs;
+    std::vector<GraphEntry> misses;            // keys seen once (u and u_k swap every step, so keys alternate)
+    bool use_graphs;
+    cudaStream_t gstream;                      // capture stream (the caller's may be the legacy default stream)
+    double* w0;                                // the buffer w started in (w and a swap when the truncation criterion accepts)
+    unsigned long long gstamp, graph_replays;
     bool profiling;
     cudaEvent_t ev[65 * 5];                    // 5 events per iteration, up to 65 iterations in flight
     double prof_ms[TF_PROFILE_SLOTS];
@@ -380,6 +389,82 @@ void collect_profile(tf_ctx* c, int niter)
         }
 }
 
+void clear_graphs(tf_ctx* c)
+{
+    for (auto& g : c->graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
+    c->graphs.clear();
+    c->misses.clear();
+}
+
+// one launch-ahead batch: [clear the records] + iterations k0 .. k1-1 (gated) + the records of the batch to the host
+cudaError_t enqueue_batch(tf_ctx* c, double s, int k0, int k1, int kmax)
+{
+    cudaError_t e = cudaSuccess;
+    if (k0 == 0) e = cudaMemsetAsync(c->red, 0, sizeof(double) * 2 * (size_t)kmax, c->stream);
+    for (int k = k0; k < k1 && e == cudaSuccess; ++k) e = launch_iteration(c, s, k, -1, true);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(c->pinned_red + 2 * k0, c->red + 2 * k0, 2 * sizeof(double) * (size_t)(k1 - k0),
+                            cudaMemcpyDeviceToHost, c->stream);
+    return e;
+}
+
+// the same batch through a CUDA graph when its key {k0, count, buffer parity, s} has been seen before: captured on the
+// second occurrence (the first ran plainly, so every kernel attribute is set), replayed from the third on
+cudaError_t enqueue_batch_graphed(tf_ctx* c, double s, int k0, int k1, int kmax)
+{
+    const int n = k1 - k0, parity = ((c->u == c->ubuf[0]) ? 0 : 1) + ((c->w == c->w0) ? 0 : 2);
+    if (!c->use_graphs) return enqueue_batch(c, s, k0, k1, kmax);
+    for (auto& g : c->graphs)
+        if (g.k0 == k0 && g.n == n && g.parity == parity && g.s == s) {
+            g.stamp = ++c->gstamp;
+            ++c->graph_replays;
+            count_launch(4 * n);
+            return cudaGraphLaunch(g.exec, c->stream);
+        }
+    size_t mi = 0;
+    for (; mi < c->misses.size(); ++mi) {
+        const auto& m = c->misses[mi];
+        if (m.k0 == k0 && m.n == n && m.parity == parity && m.s == s) break;
+    }
+    if (mi == c->misses.size()) {                        // first occurrence: remember the key, launch plainly
+        if (c->misses.size() >= 16) c->misses.erase(c->misses.begin());
+        c->misses.push_back(tf_ctx::GraphEntry{k0, n, parity, s, nullptr, 0});
+        return enqueue_batch(c, s, k0, k1, kmax);
+    }
+    c->misses.erase(c->misses.begin() + (long)mi);
+    if (!c->gstream && cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking) != cudaSuccess) {
+        c->gstream = nullptr;
+        c->use_graphs = false;
+        return enqueue_batch(c, s, k0, k1, kmax);
+    }
+    cudaStream_t user = c->stream;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    cudaError_t e = cudaStreamBeginCapture(c->gstream, cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) {
+        c->stream = c->gstream;
+        e = enqueue_batch(c, s, k0, k1, kmax);
+        c->stream = user;
+        const cudaError_t e2 = cudaStreamEndCapture(c->gstream, &graph);
+        if (e == cudaSuccess) e = e2;
+    }
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&exec, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    if (e != cudaSuccess) {                              // no graphs on this setup: fall back for good, run the batch plainly
+        cudaGetLastError();
+        c->use_graphs = false;
+        return enqueue_batch(c, s, k0, k1, kmax);
+    }
+    if (c->graphs.size() >= 16) {                        // evict the least recently used
+        size_t lru = 0;
+        for (size_t i = 1; i < c->graphs.size(); ++i) if (c->graphs[i].stamp < c->graphs[lru].stamp) lru = i;
+        cudaGraphExecDestroy(c->graphs[lru].exec);
+        c->graphs.erase(c->graphs.begin() + (long)lru);
+    }
+    c->graphs.push_back(tf_ctx::GraphEntry{k0, n, parity, s, exec, ++c->gstamp});
+    return cudaGraphLaunch(exec, c->stream);
+}
+
 tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, double kappa, double hstar,
                         int n, int m, tf_bc bc, void* dev_ws, size_t bytes, void* stream, bool own)
 {
@@ -471,6 +556,8 @@ tf_status create_common(tf_ctx** out, int nx, int ny, double dx, double dy, doub
         c->tma_yf = c->tma_yf && make_map2d(&c->mBn, c->bn, nx, ny, 32, YW_RP, false);
     }
     if (!c->tma_yf) { memset(&c->mUy, 0, sizeof(c->mUy)); memset(&c->mBn, 0, sizeof(c->mBn)); }
+    c->w0 = c->w;
+    c->use_graphs = true; c->gstream = nullptr; c->gstamp = 0; c->graph_replays = 0;
     c->profiling = false;
     for (auto& ev : c->ev) ev = nullptr;
     for (int q = 0; q < TF_PROFILE_SLOTS; ++q) { c->prof_ms[q] = 0.0; c->prof_n[q] = 0; }
@@ -613,6 +700,8 @@ void tf_destroy(tf_ctx* c)
 {
     if (!c) return;
     cudaStreamSynchronize(c->stream);
+    clear_graphs(c);
+    if (c->gstream) cudaStreamDestroy(c->gstream);
     if (c->owns_ws) cudaFree(c->ws);
     for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
     cudaFreeHost(c->pinned);
@@ -626,6 +715,7 @@ tf_status tf_set_newton(tf_ctx* c, double tol, int max_iter, int fixed_iters)
     if (max_iter < 1 || max_iter > MAX_ITERS || fixed_iters < 0 || fixed_iters > MAX_ITERS)
         return fail(c, TF_ERR_INVALID_ARG, "max_iter in [1,4096], fixed_iters in [0,4096]");
     c->tol = tol; c->max_iter = max_iter; c->fixed_iters = fixed_iters;
+    clear_graphs(c);
     return TF_OK;
 }
 
@@ -775,11 +865,27 @@ tf_status tf_set_launch_ahead(tf_ctx* c, int batch)
     return TF_OK;
 }
 
+tf_status tf_set_cuda_graphs(tf_ctx* c, int on)
+{
+    if (!c) return TF_ERR_INVALID_ARG;
+    c->use_graphs = on != 0;
+    if (!on) clear_graphs(c);
+    return TF_OK;
+}
+
+tf_status tf_graph_replays(tf_ctx* c, unsigned long long* replays)
+{
+    if (!c || !replays) return TF_ERR_INVALID_ARG;
+    *replays = c->graph_replays;
+    return TF_OK;
+}
+
 tf_status tf_set_pressure(tf_ctx* c, tf_pressure kind, const double* p, int np)
 {
     if (!c) return TF_ERR_INVALID_ARG;
     double* mp = c->P.mp;
     const double PI = 3.14159265358979323846;
+    clear_graphs(c);
     auto finite_pos = [](double v) { return v > 0 && std::isfinite(v); };
     if (kind == TF_PI_POWER) {
         c->model = TF_PI_POWER;
@@ -845,11 +951,11 @@ tf_status tf_step(tf_ctx* c, double dt, int* newton_iters, double* residual)
     const double s = 0.5 * dt;
     const bool fixed = c->fixed_iters > 0;
     const int kmax = fixed ? c->fixed_iters : c->max_iter;
-    TF_CUDA(c, cudaMemsetAsync(c->red, 0, sizeof(double) * 2 * (size_t)kmax, c->stream));
     int k = 0;
     double res = 0.0;
     tf_status status = TF_NOT_CONVERGED;
     if (fixed) {
+        TF_CUDA(c, cudaMemsetAsync(c->red, 0, sizeof(double) * 2 * (size_t)kmax, c->stream));
         // parity mode: no host decision inside the step, one read at the end
         const bool prof = c->profiling && kmax <= 64;
         for (; k < kmax; ++k) TF_CUDA(c, launch_iteration(c, s, k, prof ? k : -1, false));
@@ -876,9 +982,15 @@ tf_status tf_step(tf_ctx* c, double dt, int* newton_iters, double* residual)
         bool decided = false;
         while (!decided && done < kmax) {
             const int upto = std::min(kmax, enq + batch);
-            for (; enq < upto; ++enq) TF_CUDA(c, launch_iteration(c, s, enq, prof ? enq - done : -1, true));
-            TF_CUDA(c, cudaMemcpyAsync(c->pinned_red + 2 * done, c->red + 2 * done, 2 * sizeof(double) * (size_t)(enq - done),
-                                       cudaMemcpyDeviceToHost, c->stream));
+            if (prof) {
+                if (enq == 0) TF_CUDA(c, cudaMemsetAsync(c->red, 0, sizeof(double) * 2 * (size_t)kmax, c->stream));
+                for (; enq < upto; ++enq) TF_CUDA(c, launch_iteration(c, s, enq, enq - done, true));
+                TF_CUDA(c, cudaMemcpyAsync(c->pinned_red + 2 * done, c->red + 2 * done, 2 * sizeof(double) * (size_t)(enq - done),
+                                           cudaMemcpyDeviceToHost, c->stream));
+            } else {
+                TF_CUDA(c, enqueue_batch_graphed(c, s, enq, upto, kmax));
+                enq = upto;
+            }
             TF_CUDA(c, cudaStreamSynchronize(c->stream));
             const int first = done;
             for (; done < enq && !decided; ++done) {

@@ -32,6 +32,8 @@ SYMBOLS = {
     "tf_set_newton": (ctypes.c_int, [_vp, ctypes.c_double, ctypes.c_int, ctypes.c_int]),
     "tf_set_pressure": (ctypes.c_int, [_vp, ctypes.c_int, _dp, ctypes.c_int]),
     "tf_set_launch_ahead": (ctypes.c_int, [_vp, ctypes.c_int]),
+    "tf_set_cuda_graphs": (ctypes.c_int, [_vp, ctypes.c_int]),
+    "tf_graph_replays": (ctypes.c_int, [_vp, ctypes.POINTER(ctypes.c_ulonglong)]),
     "tf_set_solution_criteria": (ctypes.c_int, [_vp, ctypes.c_double]),
     "tf_set_truncation_criterion": (ctypes.c_int, [_vp, ctypes.c_double]),
     "tf_last_truncation_estimate": (ctypes.c_int, [_vp, _dp]),
@@ -159,6 +161,19 @@ class ThinFilm:
         st = lib().tf_set_launch_ahead(self._h, int(batch))
         if st != OK:
             _err(self._h, st, "tf_set_launch_ahead")
+
+    def set_cuda_graphs(self, on=True):
+        """tf_set_cuda_graphs: replay recurring launch-ahead batches as CUDA graphs (default on; bit-identical results)."""
+        st = lib().tf_set_cuda_graphs(self._h, 1 if on else 0)
+        if st != OK:
+            _err(self._h, st, "tf_set_cuda_graphs")
+
+    def graph_replays(self):
+        n = ctypes.c_ulonglong(0)
+        st = lib().tf_graph_replays(self._h, ctypes.byref(n))
+        if st != OK:
+            _err(self._h, st, "tf_graph_replays")
+        return int(n.value)
 
     def set_solution_criteria(self, max_rel_change=0.0):
         """tf_set_solution_criteria: accept a converged step only if max|u^{n+1}-u^n|/u^n <= max_rel_change (0 = off)."""

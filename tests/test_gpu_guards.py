@@ -65,3 +65,31 @@ def test_steps_are_bitwise_reproducible_run_to_run(nx, ny):
         else:
             assert out[0] == ref[0]
             assert np.array_equal(out[1], ref[1])
+
+
+@pytest.mark.parametrize("nx,ny", [(128, 128), (300, 167), (1024, 1024)])
+def test_cuda_graph_replay_is_bit_identical(nx, ny):
+    """Launch-ahead batches replayed as CUDA graphs (tf_set_cuda_graphs, default on) against plain launches: 40 steps,
+    every (status, iterations, residual) and the final film identical to the last bit; graphs were actually replayed;
+    a change of dt, of the Newton controls or a rejected step in between does not confuse the cache."""
+    from paper_1806_10550_b200 import tf
+    cfg = inputs.config(0)
+    h = inputs.noise_ic(nx, ny, seed=9)
+    outs = []
+    for graphs in (True, False):
+        g = tf.ThinFilm(nx, ny, cfg["dx"], cfg["dy"])
+        g.set_cuda_graphs(graphs)
+        g.set_newton(1e-10, 64, 0)
+        g.set_state(h)
+        log = [g.step(1e-2) for _ in range(25)]
+        log += [g.step(5e-3) for _ in range(5)]              # another dt: other graphs
+        g.set_newton(1e-10, 3, 0)                            # too few iterations: rejected, state kept
+        log.append(g.step(1e-2))
+        g.set_newton(1e-10, 64, 0)
+        log += [g.step(1e-2) for _ in range(40)]             # the iteration count settles: keys recur
+        outs.append((log, g.get_state(), g.graph_replays()))
+        g.close()
+    assert outs[0][0] == outs[1][0]
+    assert np.array_equal(outs[0][1], outs[1][1])
+    assert outs[0][2] >= 3 and outs[1][2] == 0           # (the count falls from step to step early on: few keys recur)
+    assert any(st == tf.NOT_CONVERGED for st, _, _ in outs[0][0])
