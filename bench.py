@@ -54,6 +54,7 @@ def parse():
                     help="ONE film spread over the ranks (paper_1806_10550_b200/dist_step.py: two all-to-alls and one "
                          "all-reduce per Newton iteration) instead of one replica per rank; strong scaling")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-side", action="store_true", help="skip the short side measurements of configs 0, 1, 2 and 4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -183,6 +184,72 @@ def whole_job_value(npts, steps, world, seconds):
     return world * npts * steps / seconds
 
 
+# ----------------------------------------------------------------------------------------- side measurements
+def side_measurements():
+    """Short runs of the other BASELINE.json configs (parity-test cases, not the headline), so that the driver's own
+    bench run records them: ms per step and per Newton iteration of configs 0 and 1 (fixed dt, 50 steps after 30),
+    config 2 (40 accepted adaptive steps, decisions on the device), and the isolated solver of config 4."""
+    import torch
+    from paper_1806_10550_b200 import tf
+    out = {}
+
+    def timed(fn):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        ev0.record()
+        r = fn()
+        ev1.record()
+        torch.cuda.synchronize()
+        return ev0.elapsed_time(ev1), r
+
+    for idx in (0, 1):
+        cfg = inputs.config(idx)
+        g = tf.ThinFilm(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["kappa"], cfg["hstar"], cfg["n"], cfg["m"])
+        g.set_newton(cfg["tol"], cfg["max_iter"], 0)
+        g.set_state(torch.from_numpy(inputs.initial_condition(cfg)).cuda())
+        for _ in range(30):
+            g.step(cfg["dt"])
+        ms, its = timed(lambda: sum(g.step(cfg["dt"])[1] for _ in range(50)))
+        out[cfg["name"]] = {"ms_per_step": ms / 50, "newton_iters_per_step": its / 50, "ms_per_iteration": ms / its,
+                            "grid_point_steps_per_s": cfg["nx"] * cfg["ny"] * 50 / (ms * 1e-3), "graph_replays": g.graph_replays(),
+                            "note": "steps 31-80 of the config's run (L2-resident: time to solution, no roofline)"}
+        g.close()
+    cfg = inputs.config(2)
+    g = tf.ThinFilm(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["kappa"], cfg["hstar"], cfg["n"], cfg["m"])
+    g.set_newton(cfg["tol"], cfg["max_iter"], 0)
+    h2 = torch.from_numpy(inputs.initial_condition(cfg)).cuda()
+    for dev in (False, True):
+        g.set_state(h2)
+        ms, r = timed(lambda: tf.advance_adaptive(g, cfg["dt"], 40, cfg["grow"], cfg["shrink"], cfg["dt_max"], cfg["dt_min"],
+                                                  on_device=dev))
+        its = sum(x[2] for x in r[2])
+        out[cfg["name"] + ("_device_controller" if dev else "_host_controller")] = {
+            "ms_per_accepted_step": ms / 40, "attempts": len(r[2]), "newton_iters_total": its, "ms_per_iteration": ms / its,
+            "point_iterations_per_s": cfg["nx"] * cfg["ny"] * its / (ms * 1e-3)}
+    g.close()
+    del h2
+    cfg = inputs.config(4)
+    n = cfg["nrow"]
+    gen = torch.Generator(device="cuda").manual_seed(cfg["seed"])
+    peak, _ = measured_peak()
+    for direction, name in ((1, "columns_y"), (0, "rows_x")):
+        U = lambda lo, hi: torch.rand(n, n, dtype=torch.float64, device="cuda", generator=gen) * (hi - lo) + lo
+        e, c, a, b, y = U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1)
+        d = 1 + e.abs() + c.abs() + a.abs() + b.abs() + U(0, 1)
+        ws = torch.empty(tf.lib().tf_penta_workspace_bytes(n, n), dtype=torch.uint8, device="cuda")
+        x = torch.empty_like(e)
+        solve = lambda: tf.penta_solve(direction, e, c, d, a, b, y, out=x, workspace=ws)
+        for _ in range(3):
+            solve()
+        ms, _ = timed(lambda: [solve() for _ in range(5)])
+        ms /= 5
+        out[cfg["name"] + "_" + name] = {"ms": ms, "unknowns_per_s": n * n / (ms * 1e-3), "alg_bytes_per_unknown": 104,
+                                         "alg_gbs": 104 * n * n / (ms * 1e-3) / 1e9, "frac_of_peak": 104 * n * n / (ms * 1e-3) / 1e9 / peak}
+        del e, c, a, b, y, d, ws, x
+    torch.cuda.empty_cache()
+    return out
+
+
 # ----------------------------------------------------------------------------------------- B200 arm
 def run_b200(args, cfg):
     import torch
@@ -296,11 +363,20 @@ def run_b200(args, cfg):
         "penta_unknowns_per_s": 2 * world * npts * iters / sec,
         "iteration_model": {"bytes_per_point_iter": 152, "gbs": 152 * npts * iters / sec / 1e9,
                             "frac_of_peak": 152 * npts * iters / sec / 1e9 / peak,
-                            "compulsory_48B_gbs": 48 * npts * iters / sec / 1e9},
+                            "compulsory_48B_gbs": 48 * npts * iters / sec / 1e9,
+                            "compulsory_48B_frac_of_peak": 48 * npts * iters / sec / 1e9 / peak},
         "kernels": kern, "kernel_time_share_of_step": ksum / (sec * 1e3) if kern else None,
         "roofline": roofline, "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
         "mass_rel_drift": mass_drift,
     }
+    if world == 1 and not args.no_side and args.pressure == "power" and (nx, ny) == (8192, 8192):
+        ctx.close()
+        del h_dev
+        torch.cuda.empty_cache()
+        try:
+            line["side"] = side_measurements()
+        except Exception as exc:                         # a side measurement must never cost the headline line
+            line["side"] = {"error": repr(exc)}
     if world == 1 and not args.no_cpu_baseline and args.pressure == "power":
         n = 2048 if min(nx, ny) >= 2048 else min(nx, ny)
         r = oracle_sample_run(cfg, n, 1, 0, args.fixed_iters)
