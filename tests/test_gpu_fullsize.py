@@ -244,3 +244,40 @@ def test_large_nonsquare_grids_sampled(tf, tfo, nx, ny):
         ia, ib = (0 if i0 == 0 else MARGIN), (W if i0 + W == nx else W - MARGIN)
         d = np.max(np.abs(u[j0 + ja:j0 + jb, i0 + ia:i0 + ib] - uo[ja:jb, ia:ib])) / np.max(np.abs(uo))
         assert d <= 1e-11, (nx, ny, j0, i0, d)
+
+
+# ------------------------------------------------------------------ fields beyond 4 GiB (element offsets up to ~6e8)
+def test_field_larger_than_4GiB_sampled(tf, tfo):
+    """30000 x 20000: 4.8 GB per field, 38 GB of workspace -- byte offsets beyond 2^32 in every kernel, 1072 strips and
+    715 row blocks (four teams per CTA in both forward kernels), dx != dy.  One step of two fixed iterations; sampled
+    windows against the oracle (corners, the split rows / columns, far ends of the arrays), mass to 1e-13."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 60e9:
+        pytest.skip("needs ~45 GB of device memory")
+    nx, ny = 30000, 20000
+    cfg = inputs.config(3)
+    dx, dy = cfg["dx"], 1.03 * cfg["dx"]
+    h = inputs.noise_ic(nx, ny, seed=31)
+    g = tf.ThinFilm(nx, ny, dx, dy)
+    g.set_newton(1e-10, 64, 2)
+    g.set_state(h)
+    m0 = g.mass()
+    ref = float(np.sum(h, dtype=np.float64)) * dx * dy
+    assert abs(m0 - ref) <= 1e-13 * ref
+    assert g.step(cfg["dt"])[:2] == (0, 2)
+    m1 = g.mass()
+    assert abs(m1 - m0) <= 1e-13 * m0
+    u = g.get_state()
+    g.close()
+    midx, midy = (nx // 2) // 16 * 16, (ny // 2) // 16 * 16
+    o = tfo.ThinFilmOracle(W, W, dx, dy)
+    o.set_newton(1e-10, 64, 2)
+    for (j0, i0) in ((0, 0), (ny - W, nx - W), (midy - W // 2, midx - W // 2), (ny - W, 0), (0, nx - W), (ny - W, midx - W // 2)):
+        o.set_state(np.ascontiguousarray(h[j0:j0 + W, i0:i0 + W]))
+        assert o.step(cfg["dt"])[:2] == (0, 2)
+        uo = o.get_state()
+        ja, jb = (0 if j0 == 0 else MARGIN), (W if j0 + W == ny else W - MARGIN)
+        ia, ib = (0 if i0 == 0 else MARGIN), (W if i0 + W == nx else W - MARGIN)
+        d = np.max(np.abs(u[j0 + ja:j0 + jb, i0 + ia:i0 + ib] - uo[ja:jb, ia:ib])) / np.max(np.abs(uo))
+        assert d <= 1e-11, (j0, i0, d)
