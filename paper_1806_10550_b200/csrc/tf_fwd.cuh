@@ -23,7 +23,7 @@ namespace tf {
 #define TF_ROTATE_Y 1
 #endif
 // Probe builds (-DTF_EXP_NOSTORE / TF_EXP_STORE_L2 / TF_EXP_NOCONS / TF_EXP_NOPROD / TF_EXP_NOZ / TF_PERT_SHFL / TF_PERT_FMA /
-// TF_PERT_INT): timing-only variants of the y forward kernel that leave out or add one ingredient; they compute wrong
+// TF_PERT_INT / TF_PERT_LESS_SHFL): timing-only variants of the y forward kernel that leave out or add one ingredient; they compute wrong
 // results on purpose.  DESIGN.md section 6 quotes what they measured; no product build defines them.
 constexpr int YW_VALID = 28;     // columns per strip (lanes 2..29; lanes 0,1,30,31 are x-halo)
 
@@ -85,8 +85,12 @@ __device__ __forceinline__ void y_advance(YState& S, int j, double hp2, const Pa
             if (t == 0x7fffffff) S.phim += 1.0;
         }
 #endif
+#ifdef TF_PERT_LESS_SHFL                              /* probe: what halving the shuffles would be worth (wrong results) */
+        const double f0R = S.c0.f0 * 1.0000001, f1R = S.c0.f1, LR = S.L0 + 1e-9;
+#else
         const double f0R = __shfl_down_sync(FULL, S.c0.f0, 1), f1R = __shfl_down_sync(FULL, S.c0.f1, 1);
         const double LR = __shfl_down_sync(FULL, S.L0, 1);
+#endif
         double phixp = DX.cb * fma(S.c0.f0 + f0R, LR - S.L0, (S.c0.f1 + f1R) * (S.hR0 - S.h0));
         if (!xface) phixp = 0.0;
         const double phixm = __shfl_up_sync(FULL, phixp, 1);
