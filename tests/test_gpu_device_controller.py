@@ -167,3 +167,21 @@ def test_truncation_criterion_against_the_oracle_transcription(tf, tfo):
         assert g.step(DT0)[0] == 0 and s2.step(DT0)[0] == 0
     assert abs(g.last_truncation_estimate() - s2.last) <= 1e-3 * s2.last and s2.last > 0
     g.close()
+
+
+def test_device_controller_with_the_nlc_pressure_equals_host(tf):
+    """The device controller with the paper's NLC pressure (1.8)-(1.9), (1.11): same run as the host controller."""
+    nx, ny = 128, 96
+    C = 0.0857
+    h = 0.2 * (1.0 + 0.05 * np.random.default_rng(8).uniform(-1, 1, (ny, nx)))
+    outs = []
+    for on_device in (True, False):
+        g = tf.ThinFilm(nx, ny, 0.05, 0.05)
+        g.set_pressure(tf.PI_NLC, (C, 1.0 / C, 36.0, 0.01, 1.67, 1.0, 0.05))
+        g.set_newton(1e-10, 10, 0)
+        g.set_state(np.ascontiguousarray(h))
+        t, dt, hist = tf.advance_adaptive(g, 1e-3, 10, grow=1.5, shrink=0.5, dt_max=0.1, dt_min=1e-12, on_device=on_device)
+        outs.append((t, dt, hist, g.get_state()))
+        g.close()
+    assert outs[0][:3] == outs[1][:3] and np.array_equal(outs[0][3], outs[1][3])
+    assert sum(1 for x in outs[0][2] if x[1] == 0) == 10
