@@ -23,7 +23,7 @@ namespace tf {
 #define TF_ROTATE_Y 1
 #endif
 // Probe builds (-DTF_EXP_NOSTORE / TF_EXP_STORE_L2 / TF_EXP_NOCONS / TF_EXP_NOPROD / TF_EXP_NOZ / TF_PERT_SHFL / TF_PERT_FMA /
-// TF_PERT_INT / TF_PERT_LESS_SHFL): timing-only variants of the y forward kernel that leave out or add one ingredient; they compute wrong
+// TF_PERT_INT / TF_PERT_LESS_SHFL; TF_EXP_X_NOSTORE / TF_EXP_X_NOCONS / TF_EXP_X_NOPROD for the x forward kernel): timing-only variants of the y forward kernel that leave out or add one ingredient; they compute wrong
 // results on purpose.  DESIGN.md section 6 quotes what they measured; no product build defines them.
 constexpr int YW_VALID = 28;     // columns per strip (lanes 2..29; lanes 0,1,30,31 are x-halo)
 
@@ -491,6 +491,16 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
                 }
             };
             const bool interior = (ilo >= 3) && (ilo + XW_CT + 2 <= nx - 2) && (ilo >= imin) && (ilo + XW_CT <= imax);
+#ifdef TF_EXP_X_NOPROD
+            if (interior) {
+#pragma unroll
+                for (int k = 0; k < NRMAX; ++k)
+                    if (pw + k * NP < XW_R && lane_ok) {
+                        const int r = pw + k * NP;
+                        st[r] = hq[k] * 0.1; st[SV + r] = 0.5 * hq[k]; st[2 * SV + r] = -0.2 * hq[k]; st[3 * SV + r] = wq[k];
+                    }
+            } else
+#endif
             if (interior) {
 #pragma unroll
                 for (int k = 0; k < NRMAX; ++k)
@@ -508,6 +518,9 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
         const int j = j0 + lane;
         const int rowok = (lane < XW_R && j < ny) ? 1 : 0;
         Elim2 S = elim2_init();
+#ifdef TF_EXP_X_NOSTORE
+        int xacc = 0;
+#endif
         double Ba = 0.0, B1 = 0.0, B2 = 0.0;              // backward face: the boundary face before the first column carries nothing
         const int step = dir ? -ny : ny;
         int o = (dir ? nx : -1) * ny + j;                 // the column before the first one
@@ -525,9 +538,16 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
                 double va, vb, vz;
                 elim2_row(S, Ba, cc, qq, a, Fa, R, va, vb, vz);
                 Ba = Fa; B1 = F1; B2 = F2;
+#ifdef TF_EXP_X_NOSTORE
+                xacc ^= __double2hiint(va) ^ __double2hiint(vb) ^ __double2hiint(vz);
+#else
                 st3_if(pred, alT + o, va, beT + o, vb, zzT + o, vz);
+#endif
                 o += step;
             };
+#ifdef TF_EXP_X_NOCONS
+            if (ncol == XW_CK && g > 0) { o += XW_CK * step; } else
+#endif
             if (ncol == XW_CK && g > 0) {
 #pragma unroll
                 for (int c = 0; c < XW_CK; ++c) column(c, rowok);
@@ -539,6 +559,9 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
         }
         double va, vb, vz;
         elim2_flush(S, va, vb, vz);
+#ifdef TF_EXP_X_NOSTORE
+        if (xacc == 0x12345) vz = 1.0;
+#endif
         st3_if(rowok, alT + o, va, beT + o, vb, zzT + o, vz);
     }
 }
