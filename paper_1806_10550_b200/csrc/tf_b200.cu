@@ -265,6 +265,15 @@ constexpr int PR_NST = 2;                 // isolated solver, rows: 2 stages x 6
 #ifndef TF_XW_NP2
 #define TF_XW_NP2 7
 #endif
+#ifndef TF_YW_NP1
+#define TF_YW_NP1 6
+#endif
+#ifndef TF_XW_NP1
+#define TF_XW_NP1 7
+#endif
+#ifndef TF_NSUB1
+#define TF_NSUB1 1
+#endif
 constexpr int YW_NP = 3, YW_RP = 8, YW_NSTG = 4;   // yfwd: consumer warp 0 + 3 producer warps, chunks of 8 rows, ring of 4 chunk slots (40 KiB)
 
 #ifndef TF_XW_NP
@@ -281,7 +290,7 @@ cudaError_t launch_yfwd(tf_ctx* c, const CUtensorMap& mu, int tma, const Params&
                         const double* src, int grid, Gate gate)
 {
     // producers per team: YW_NP with four teams per CTA; grids with two teams per CTA (sides <= ~4100) have SM capacity to spare
-    constexpr int NP = NSUB == 2 ? TF_YW_NP2 : YW_NP;
+    constexpr int NP = NSUB == 2 ? TF_YW_NP2 : (NSUB == 1 ? TF_YW_NP1 : YW_NP);
     constexpr int NSTG = NP > YW_NSTG ? NP : YW_NSTG;                  // ring slots >= producers (see the kernel)
     constexpr size_t SM = NSUB * (size_t)NSTG * 5 * YW_RP * 32 * 8 + NSUB * NP * (size_t)(2 * YW_RP + 4) * 32 * 8 +
                           (2 * NSUB * NSTG + NSUB * NP) * 8;
@@ -292,7 +301,7 @@ cudaError_t launch_yfwd(tf_ctx* c, const CUtensorMap& mu, int tma, const Params&
         if (e != cudaSuccess) return e;
         ready.mark();
     }
-    kern<<<grid, 32 * NSUB * (NP + 1), SM, c->stream>>>(mu, c->mBn, tma, P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz, gate);
+    kern<<<grid, 32 * fwd_warps(NSUB, NP), SM, c->stream>>>(mu, c->mBn, tma, P, DX, DY, c->mid_y, src, c->bn, c->al, c->be, c->zz, gate);
     return cudaGetLastError();
 }
 
@@ -302,7 +311,7 @@ cudaError_t launch_xfwd(tf_ctx* c, const Params& P, const Dir& DX, const double*
     constexpr size_t SM = NSUB * ((size_t)XW_NSTG * 4 * XW_CK * XW_LD * 8 + 16 * XW_NSTG);
     // two teams per CTA (sides <= ~4100, the paper's domain sizes): 7 producers of 4 rows each per team instead of 4 of 7
     // (measured at 4096^2: x forward 0.168 -> 0.153 ms; 6, 8, 9, 10 producers: 0.162 - 0.167; y forward with 4: slower)
-    constexpr int NP = NSUB == 2 ? TF_XW_NP2 : XW_NP;
+    constexpr int NP = NSUB == 2 ? TF_XW_NP2 : (NSUB == 1 ? TF_XW_NP1 : XW_NP);
     auto kern = xfwd_ws_kernel<N, M, NP, XW_NSTG, NSUB>;
     static DevOnce ready;
     if (!ready.done()) {
@@ -310,7 +319,7 @@ cudaError_t launch_xfwd(tf_ctx* c, const Params& P, const Dir& DX, const double*
         if (e != cudaSuccess) return e;
         ready.mark();
     }
-    kern<<<grid, 32 * NSUB * (NP + 1), SM, c->stream>>>(P, DX, c->mid_x, src, c->w, c->al, c->be, c->zz, gate);
+    kern<<<grid, 32 * fwd_warps(NSUB, NP), SM, c->stream>>>(P, DX, c->mid_x, src, c->w, c->al, c->be, c->zz, gate);
     return cudaGetLastError();
 }
 
@@ -338,6 +347,9 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, i
         if (nstrip > c->num_sms)
             e = k == 0 ? launch_yfwd<N, M, true, 4>(c, mu, tma, P, DX, DY, src, (nstrip + 1) / 2, gate)
                        : launch_yfwd<N, M, false, 4>(c, mu, tma, P, DX, DY, src, (nstrip + 1) / 2, gate);
+        else if (TF_NSUB1 && 2 * nstrip <= c->num_sms)      // one team per SM (sides <= ~2070): a whole SM per half line
+            e = k == 0 ? launch_yfwd<N, M, true, 1>(c, mu, tma, P, DX, DY, src, 2 * nstrip, gate)
+                       : launch_yfwd<N, M, false, 1>(c, mu, tma, P, DX, DY, src, 2 * nstrip, gate);
         else
             e = k == 0 ? launch_yfwd<N, M, true, 2>(c, mu, tma, P, DX, DY, src, nstrip, gate)
                        : launch_yfwd<N, M, false, 2>(c, mu, tma, P, DX, DY, src, nstrip, gate);
@@ -351,7 +363,8 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, i
     if (which & 2) {
         const int nblk = (P.ny + XW_R - 1) / XW_R;
         cudaError_t e = nblk > c->num_sms ? launch_xfwd<N, M, 4>(c, P, DX, src, (nblk + 1) / 2, gate)
-                                          : launch_xfwd<N, M, 2>(c, P, DX, src, nblk, gate);
+                        : (TF_NSUB1 && 2 * nblk <= c->num_sms) ? launch_xfwd<N, M, 1>(c, P, DX, src, 2 * nblk, gate)
+                                                               : launch_xfwd<N, M, 2>(c, P, DX, src, nblk, gate);
         if (e != cudaSuccess) return e;
     }
     if (ev) cudaEventRecord(ev[3], c->stream);

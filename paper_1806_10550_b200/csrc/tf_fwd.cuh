@@ -27,6 +27,25 @@ namespace tf {
 // results on purpose.  DESIGN.md section 6 quotes what they measured; no product build defines them.
 constexpr int YW_VALID = 28;     // columns per strip (lanes 2..29; lanes 0,1,30,31 are x-halo)
 
+// Warps of a forward CTA.  With one team per CTA (NSUB = 1, small grids) the consumer keeps SM sub-partition 0 to itself:
+// warps 4, 8, ... (which would share it) are launched idle, the producers are the warps with warp % 4 != 0.
+#ifndef TF_N1_SKIP0
+#define TF_N1_SKIP0 1
+#endif
+#ifndef TF_N2_SKIP0
+#define TF_N2_SKIP0 0
+#endif
+// the same for two teams per CTA (both consumers on sub-partition 0, warps 0 and 4) was measured slower (4096^2: y forward
+// 0.155 -> 0.163 ms, x forward 0.152 -> 0.167 ms) and is off
+__host__ __device__ constexpr bool fwd_sp0(int nsub) { return (nsub == 1 && TF_N1_SKIP0) || (nsub == 2 && TF_N2_SKIP0); }
+__host__ __device__ constexpr int fwd_warps(int nsub, int np)
+{
+    if (!fwd_sp0(nsub)) return nsub * (np + 1);
+    int w = 4 * (nsub - 1) + 1;                       // the last consumer warp
+    while (w - (w + 3) / 4 < nsub * np) ++w;           // warps 0 .. w-1 hold w - ceil(w/4) producers
+    return w;
+}
+
 // rolling state of a thread marching down a column
 struct YState {
     double hm1, h0, hp1;         // h(j-1), h(j), h(j+1)
@@ -124,7 +143,7 @@ __device__ __forceinline__ void y_advance(YState& S, int j, double hp2, const Pa
 // stays small.  Inputs arrive by TMA, one box per chunk, issued a chunk ahead (see the producer loop).
 // ---------------------------------------------------------------------------------------------
 template <int N, int M, bool FIRST, int NP, int RP, int NCH, int NSUB>
-__global__ void __launch_bounds__(32 * NSUB * (NP + 1), 1)
+__global__ void __launch_bounds__(32 * fwd_warps(NSUB, NP), 1)
 yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ CUtensorMap mB, int use_tma,
                Params P, Dir DX, Dir DY, int mid, const double* __restrict__ u, double* __restrict__ bn,
                double* __restrict__ al, double* __restrict__ be, double* __restrict__ zz, Gate gate)
@@ -149,9 +168,17 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
     // role 0: consumer, 1..NP: producers.  Warp w runs on SM sub-partition w % 4: consumer q sits on sub-partition q,
     // its producers (TF_ROTATE_Y) on the sub-partitions after it, so that a team's assembly burst uses several fp64
     // pipes while the other teams' consumers (dependent chains, mostly idle issue slots) share them
-    const int role = warp / NSUB;
-    // (not for the NLC cells, whose exp and extra reciprocals make the producers the fp64-heavier side: measured +1.5 %)
-    const int q = (TF_ROTATE_Y && N != MODEL_NLC) ? (warp % NSUB + NSUB * NP - role) % NSUB : warp % NSUB;
+    // (rotation not for the NLC cells, whose exp and extra reciprocals make the producers the fp64-heavier side: +1.5 %)
+    int role, q;
+    bool idle = false;
+    if (fwd_sp0(NSUB)) {                              // consumers: warps 0, 4, ..; producers: the warps with warp % 4 != 0
+        if (warp % 4 == 0) { role = 0; q = warp / 4; idle = warp / 4 >= NSUB; }
+        else { const int p = warp - warp / 4 - 1; q = p % NSUB; role = 1 + p / NSUB; idle = role > NP; }
+        if (idle) { role = 1; q = 0; }
+    } else {
+        role = warp / NSUB;
+        q = (TF_ROTATE_Y && N != MODEL_NLC) ? (warp % NSUB + NSUB * NP - role) % NSUB : warp % NSUB;
+    }
     double* sm = reinterpret_cast<double*>(raw + q * RING);          // [NCH][5][RP][32]
     uint64_t* bars = reinterpret_cast<uint64_t*>(raw + NSUB * RING + NSUB * NP * STG);
     uint64_t* full = bars + q * 2 * NCH;
@@ -163,10 +190,13 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
         mbar_fence_init();
     }
     __syncthreads();
-    const int strip = (NSUB / 2) * blockIdx.x + (q % (NSUB / 2));
+    if (idle) return;
+    // NSUB = 1 (grids with at most one team per SM: sides <= ~2070): one team per CTA, blockIdx.x = 2 strip + half
+    constexpr int SPC = NSUB >= 2 ? NSUB / 2 : 1;     // strips per CTA
+    const int strip = NSUB >= 2 ? SPC * (int)blockIdx.x + (q % SPC) : (int)blockIdx.x / 2;
     if (strip * YW_VALID >= nx) return;               // odd strip count: the last CTA has one strip
     const int i = strip * YW_VALID - 2 + lane;
-    const int dir = q / (NSUB / 2);                   // 0: rows 0 .. mid-1 downwards, 1: rows ny-1 .. mid upwards
+    const int dir = NSUB >= 2 ? q / SPC : (int)blockIdx.x % 2;   // 0: rows 0 .. mid-1 downwards, 1: rows ny-1 .. mid upwards
     const int nrows = dir ? ny - mid : mid;           // rows of this half
     const int nchunk = (nrows + RP - 1) / RP;
     const int jmin = dir ? mid : 0, jmax = dir ? ny : mid;    // this half owns rows [jmin, jmax)
@@ -387,7 +417,7 @@ constexpr int XW_R = 28;             // rows per block
 constexpr int XW_LD = 29;            // slot row pitch in doubles (odd)
 
 template <int N, int M, int NP, int NCH, int NSUB>
-__global__ void __launch_bounds__(32 * NSUB * (NP + 1), 1)
+__global__ void __launch_bounds__(32 * fwd_warps(NSUB, NP), 1)
 xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const double* __restrict__ w,
                double* __restrict__ alT, double* __restrict__ beT, double* __restrict__ zzT, Gate gate)
 {
@@ -401,8 +431,16 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
     const unsigned FULL = 0xffffffffu;
     const int nx = P.nx, ny = P.ny;
     const int warp = uniform_warp_idx(), lane = threadIdx.x & 31;
-    const int role = warp / NSUB;                     // role 0: consumer, 1..NP: producers (NSUB, rotation: see yfwd_ws_kernel)
-    const int q = TF_ROTATE_X ? (warp % NSUB + NSUB * NP - role) % NSUB : warp % NSUB;
+    int role, q;                                      // 0: consumer, 1..NP: producers; team q (see yfwd_ws_kernel)
+    bool idle = false;
+    if (fwd_sp0(NSUB)) {
+        if (warp % 4 == 0) { role = 0; q = warp / 4; idle = warp / 4 >= NSUB; }
+        else { const int p = warp - warp / 4 - 1; q = p % NSUB; role = 1 + p / NSUB; idle = role > NP; }
+        if (idle) { role = 1; q = 0; }
+    } else {
+        role = warp / NSUB;
+        q = TF_ROTATE_X ? (warp % NSUB + NSUB * NP - role) % NSUB : warp % NSUB;
+    }
     double* sm = reinterpret_cast<double*>(raw + q * RING);          // [NCH][NPL][CK][LD]
     uint64_t* full = reinterpret_cast<uint64_t*>(raw + q * RING + (size_t)NCH * NPL * SV * 8);
     uint64_t* empty = full + NCH;
@@ -412,9 +450,11 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
         mbar_fence_init();
     }
     __syncthreads();
-    const int j0 = ((NSUB / 2) * blockIdx.x + (q % (NSUB / 2))) * XW_R;
+    if (idle) return;
+    constexpr int SPC = NSUB >= 2 ? NSUB / 2 : 1;     // row blocks per CTA; NSUB = 1: blockIdx.x = 2 block + half
+    const int j0 = (NSUB >= 2 ? SPC * (int)blockIdx.x + (q % SPC) : (int)blockIdx.x / 2) * XW_R;
     if (j0 >= ny) return;
-    const int dir = q / (NSUB / 2);
+    const int dir = NSUB >= 2 ? q / SPC : (int)blockIdx.x % 2;
     const int ncols = dir ? nx - mid : mid;           // columns of this half
     const int ntile = (ncols + XW_CT - 1) / XW_CT;
     const int imin = dir ? mid : 0, imax = dir ? nx : mid;
