@@ -556,7 +556,7 @@ def run_penta(args, cfg):
     if int(os.environ.get("RANK", "0")) != 0:
         return
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
-    n = args.length or cfg["nrow"]
+    n = args.length or (1024 if args.variant == "pcr" else cfg["nrow"])     # the cyclic-reduction variant holds a system in shared memory
     nsys = args.nsys or cfg["nrow"]
     variant = {"partition": tf.PENTA_PARTITION, "pcr": tf.PENTA_PCR}.get(args.variant, tf.PENTA_LU)
     gen = torch.Generator(device="cuda").manual_seed(cfg["seed"])
