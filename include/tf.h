@@ -248,6 +248,40 @@ tf_status tf_penta_solve(int nrow, int ncol, int dir,
                          void* dev_ws, void* cuda_stream);
 
 /*
+ * tf_penta_solve for callers that have no device scratch to hand over and no way to get any.
+ *
+ * tf_penta_solve needs three scratch arrays (the LU factors alpha, beta and the intermediate z of (A.5),
+ * PAPER.md:729-734) and leaves their allocation to the caller.  Some callers cannot allocate at the moment of the call:
+ *   - a service that, at start-up, gave all free HBM to its own memory pool: a later cudaMalloc fails for lack of memory;
+ *   - a latency-bound loop: cudaMalloc / cudaFree synchronise the whole device and take an unbounded time, which stalls
+ *     the work other streams have in flight;
+ *   - a plug-in inside a host application whose rules forbid CUDA allocations after initialisation.
+ * For them the library itself carries the scratch: one fixed array in the device image of libtf_b200.so
+ * (3 * TF_PENTA_STATIC_MAX_ELEMS doubles = 24 MiB).  The price is paid by everybody: every GPU on which this library's
+ * device code gets loaded holds those 24 MiB from then until the process exits, whether or not this call is ever made.
+ *
+ * Same arguments, same kernels, same result (bit for bit) as tf_penta_solve without dev_ws; e ... rhs and x are DEVICE
+ * arrays on the CURRENT device, owned by the caller, x may not alias an input.
+ *   Limit:     nrow * ncol <= TF_PENTA_STATIC_MAX_ELEMS (tf_penta_static_max_elems() returns it at run time); a larger
+ *              shape is refused with TF_ERR_INVALID_ARG and a message naming the limit, before any CUDA call.
+ *   No allocation: neither this call nor anything below it calls cudaMalloc, cudaFree or a library routine that allocates.
+ *   First call on each device: looks up the device address of the array (once per device, that device being current)
+ *              and raises the shared-memory limit of the kernels it launches.  Make this first call during set-up,
+ *              before any stream capture is started; later calls only enqueue kernels on cuda_stream and return.
+ *   Sharing:   every call on a device uses the SAME array and finds in it whatever the previous call left.  Nothing in
+ *              it has to start at zero -- the forward elimination writes every entry before the back substitution
+ *              reads it -- so no clearing is done.  Two calls whose kernels can overlap on the GPU (different streams,
+ *              or different host threads, without an ordering between them) race on the array and both results are
+ *              garbage: keep all calls on one stream or order them with events.
+ */
+#define TF_PENTA_STATIC_MAX_ELEMS (1u << 20)
+size_t    tf_penta_static_max_elems(void);
+tf_status tf_penta_solve_static(int nrow, int ncol, int dir,
+                                const double* e, const double* c, const double* d,
+                                const double* a, const double* b, const double* rhs, double* x,
+                                void* cuda_stream);
+
+/*
  * The same solve with a selectable algorithm (PAPER.md:647 names "the SPIKE method or
  * cyclical reduction" as the way to parallelise a single system):
  *   TF_PENTA_LU         one thread per system, two-sided LU (what tf_penta_solve runs);

@@ -1406,6 +1406,61 @@ tf_status tf_penta_solve_ex(int nrow, int ncol, int dir, int variant, int nparts
     return TF_OK;
 }
 
+// ---- tf_penta_solve_static: the isolated solve for callers that cannot allocate device memory (include/tf.h).
+// The scratch (alpha, beta, z) is part of this library's device image.  Every device that loads the image keeps the
+// array until the process ends, and every call on a device shares it.
+static __device__ __align__(256) double g_penta_static_scratch[3 * (size_t)TF_PENTA_STATIC_MAX_ELEMS];
+
+namespace {
+
+// In host code `g_penta_static_scratch` is only a handle for the runtime, NOT a device address: a kernel given
+// `&g_penta_static_scratch[0]` from the host would fault (or, on a system where the GPU can reach host memory, quietly
+// work on the wrong bytes).  The device address is asked for once per device, with that device current, and kept.
+std::mutex g_penta_static_mu;
+double* g_penta_static_addr[64];      // by device ordinal; written under the mutex
+
+tf_status penta_static_scratch(double** out)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "tf_penta_solve_static: cudaGetDevice");
+    if (dev < 0 || dev >= 64) return fail(nullptr, TF_ERR_UNSUPPORTED, "tf_penta_solve_static: device ordinal above 63");
+    std::lock_guard<std::mutex> lock(g_penta_static_mu);
+    if (!g_penta_static_addr[dev]) {
+        double* p = nullptr;
+        e = cudaGetSymbolAddress((void**)&p, g_penta_static_scratch);
+        if (e != cudaSuccess) return cuda_fail(nullptr, e, "tf_penta_solve_static: cudaGetSymbolAddress");
+        if (!p || (uintptr_t)p % ALIGN) return fail(nullptr, TF_ERR_CUDA, "tf_penta_solve_static: scratch address is null or misaligned");
+        g_penta_static_addr[dev] = p;
+    }
+    *out = g_penta_static_addr[dev];
+    return TF_OK;
+}
+
+}  // namespace
+
+size_t tf_penta_static_max_elems(void) { return (size_t)TF_PENTA_STATIC_MAX_ELEMS; }
+
+tf_status tf_penta_solve_static(int nrow, int ncol, int dir, const double* e, const double* c, const double* d,
+                                const double* a, const double* b, const double* rhs, double* x, void* cuda_stream)
+{
+    // all argument checks come before the first CUDA call: a refused call touches no device
+    if (nrow < 1 || ncol < 1 || (dir != 0 && dir != 1)) return fail(nullptr, TF_ERR_INVALID_ARG, "bad shape or dir");
+    if ((unsigned long long)nrow * (unsigned long long)ncol > (unsigned long long)TF_PENTA_STATIC_MAX_ELEMS)
+        return fail(nullptr, TF_ERR_INVALID_ARG,
+                    "tf_penta_solve_static: nrow * ncol = " + std::to_string((unsigned long long)nrow * (unsigned long long)ncol) +
+                        " exceeds the built-in scratch of TF_PENTA_STATIC_MAX_ELEMS = " + std::to_string((unsigned long long)TF_PENTA_STATIC_MAX_ELEMS) +
+                        " elements; use tf_penta_solve with a caller-owned workspace");
+    if ((dir ? nrow : ncol) < 3) return fail(nullptr, TF_ERR_INVALID_ARG, "system length must be >= 3");
+    if (!e || !c || !d || !a || !b || !rhs || !x) return fail(nullptr, TF_ERR_INVALID_ARG, "NULL pointer");
+    double* scratch = nullptr;
+    const tf_status st = penta_static_scratch(&scratch);
+    if (st != TF_OK) return st;
+    // the three fields sit align_up(nrow * ncol * 8) <= 8 MiB apart: inside the array by the limit above.  The existing
+    // thread-per-system path does the rest; it enqueues kernels and sets function attributes, and allocates nothing.
+    return tf_penta_solve_ex(nrow, ncol, dir, TF_PENTA_LU, 0, e, c, d, a, b, rhs, x, scratch, cuda_stream);
+}
+
 size_t tf_betti_workspace_bytes(int nx, int ny, int nthr)
 {
     if (nx < 1 || ny < 1 || nthr < 1) return 0;

@@ -58,6 +58,8 @@ SYMBOLS = {
                                      ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp]),
     "tf_penta_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int, ctypes.c_int]),
     "tf_penta_solve": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int] + [_vp] * 9),
+    "tf_penta_static_max_elems": (ctypes.c_size_t, []),
+    "tf_penta_solve_static": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, ctypes.c_int] + [_vp] * 8),
     "tf_penta_partition_chunks": (ctypes.c_int, [ctypes.c_int] * 4),
     "tf_penta_slab_interface_doubles": (ctypes.c_size_t, [ctypes.c_int] * 4),
     "tf_penta_slab_workspace_bytes": (ctypes.c_size_t, [ctypes.c_int] * 5),
@@ -432,6 +434,33 @@ def penta_solve(direction, e, c, d, a, b, rhs, out=None, workspace=None, stream=
                              workspace.data_ptr(), st)
     if rc != OK:
         _err(None, rc, "tf_penta_solve_ex")
+    return out
+
+
+def penta_static_max_elems():
+    """tf_penta_static_max_elems: the largest nrow * ncol that penta_solve_static accepts."""
+    return int(lib().tf_penta_static_max_elems())
+
+
+def penta_solve_static(direction, e, c, d, a, b, rhs, out, stream=None):
+    """tf_penta_solve_static: penta_solve for a caller that may not allocate device memory when it calls -- all of
+    HBM already belongs to its own pool, or a cudaMalloc would stall its other streams, or its host application forbids
+    allocations after start-up.  The scratch is a fixed 24 MiB array inside libtf_b200.so, so this binding allocates
+    nothing either: `out` must be passed in.  nrow * ncol <= penta_static_max_elems(), else TfError (ERR_INVALID_ARG).
+    The first call on a device does one-time set-up.  All calls on a device share the one scratch array: keep them on
+    one stream (or order them), calls that overlap on the GPU corrupt each other.  Same kernels and bits as penta_solve.
+    The tensors must live on the current device.  Enqueues and returns `out` without synchronising."""
+    torch = _torch()
+    ts = (e, c, d, a, b, rhs, out)
+    nrow, ncol = e.shape
+    for t in ts:
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                and tuple(t.shape) == (nrow, ncol)):
+            raise ValueError("expected contiguous CUDA float64 tensors of one shape")
+    st = (torch.cuda.current_stream(e.device) if stream is None else stream).cuda_stream
+    rc = lib().tf_penta_solve_static(nrow, ncol, direction, *[t.data_ptr() for t in ts], st)
+    if rc != OK:
+        _err(None, rc, "tf_penta_solve_static")
     return out
 
 
