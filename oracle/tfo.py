@@ -80,7 +80,7 @@ class ThinFilmOracle:
     """Same call names as the CUDA binding (create/set_newton/set_state/step/get_state/mass)."""
 
     def __init__(self, nx, ny, dx, dy, kappa=100.0, hstar=0.1, n=3, m=2, bc=0, omp=False, library=None):
-        self.L = library if library is not None else lib(omp)   # library: a mutated build (tests/test_oracle_mutants.py)
+        self.L = library if library is not None else lib(omp)   # library: a mutated build (tests/mutation_sweep.py)
         self.nx, self.ny = nx, ny
         self._h = ctypes.c_void_p()
         _chk(self.L.tfo_create(ctypes.byref(self._h), nx, ny, dx, dy, kappa, hstar, n, m, bc), "tfo_create")

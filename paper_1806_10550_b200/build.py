@@ -29,10 +29,7 @@ def build(force=False, verbose=False):
     if not force and not stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    # TF_EXTRA_NVCC_FLAGS: extra flags, e.g. the -DTF_EXP_* / -DTF_PERT_* probe macros of csrc/tf_fwd.cuh (timing-only
-    # builds that profiles/r02_ncu.md quotes; rebuild with --force and without the variable afterwards)
-    extra = os.environ.get("TF_EXTRA_NVCC_FLAGS", "").split()
-    cmd = [nvcc, *NVCC_FLAGS, *extra, "-o", LIB, *SOURCES]
+    cmd = [nvcc, *NVCC_FLAGS, "-o", LIB, *SOURCES]
     r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if verbose or r.returncode != 0:
         print(" ".join(cmd))

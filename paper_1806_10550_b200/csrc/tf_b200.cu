@@ -380,11 +380,9 @@ cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, i
 cudaError_t launch_iteration(tf_ctx* c, double s, int k, int slot, bool gated, int which = 3, const double* sdev = nullptr,
                              const double* gate0 = nullptr)
 {
-#ifndef TF_ONLY_POWER32                      /* experiment builds instantiate the (3,2) power law only */
     if (c->model == TF_PI_NLC) return launch_iteration<MODEL_NLC, 0>(c, s, k, slot, gated, which, sdev, gate0);
     if (c->model == TF_PI_POLYMER) return launch_iteration<MODEL_POLYMER, 0>(c, s, k, slot, gated, which, sdev, gate0);
     if (!(c->P.n == 3 && c->P.m == 2)) return launch_iteration<0, 0>(c, s, k, slot, gated, which, sdev, gate0);
-#endif
     return launch_iteration<3, 2>(c, s, k, slot, gated, which, sdev, gate0);
 }
 

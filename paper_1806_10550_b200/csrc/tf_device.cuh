@@ -175,11 +175,7 @@ __device__ __forceinline__ void elim2_row(Elim2& S, double e, double c, double q
     const double T = fma(-S.b2, e, q);
     const double g = S.p1 * gam;
     const double bg = S.b1 * gam;
-#ifdef TF_EXP_NOZ
-    const double sy = y;
-#else
     const double sy = fma(-S.z2, e, y);
-#endif
     const double u1 = fma(-g, S.y1, T);
     const double G = g * S.y1;
     const double mu = fma(-G, S.t1, u1);             // the only op between t1 and the next seed
@@ -189,12 +185,8 @@ __device__ __forceinline__ void elim2_row(Elim2& S, double e, double c, double q
     const double tt = fma(ee, ee, ee);
     const double r1 = fma(S.y1, S.t1, S.y1);         // finish row i-1, off the critical path
     al = S.p1 * r1; be = S.b1 * r1;
-#ifdef TF_EXP_NOZ
-    zz = sy; const double s = sy;
-#else
     zz = S.s1 * r1;
     const double s = fma(-zz, gam, sy);
-#endif
     const double p = fma(-bg, r1, a);
     S.a2 = al; S.b2 = be; S.z2 = zz;
     S.y1 = y0; S.t1 = tt; S.p1 = p; S.b1 = b; S.s1 = s;

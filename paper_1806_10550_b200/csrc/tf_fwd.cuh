@@ -22,9 +22,8 @@ namespace tf {
 #ifndef TF_ROTATE_Y
 #define TF_ROTATE_Y 1
 #endif
-// Probe builds (-DTF_EXP_NOSTORE / TF_EXP_STORE_L2 / TF_EXP_NOCONS / TF_EXP_NOPROD / TF_EXP_NOZ / TF_PERT_SHFL / TF_PERT_FMA /
-// TF_PERT_INT / TF_PERT_LESS_SHFL; TF_EXP_X_NOSTORE / TF_EXP_X_NOCONS / TF_EXP_X_NOPROD for the x forward kernel): timing-only variants of the y forward kernel that leave out or add one ingredient; they compute wrong
-// results on purpose.  DESIGN.md section 6 quotes what they measured; no product build defines them.
+// What bounds these kernels was measured with timing-only probe builds (one ingredient left out or added at a time);
+// the results are in profiles/r02_ncu.md, the switches are gone from the source.
 constexpr int YW_VALID = 28;     // columns per strip (lanes 2..29; lanes 0,1,30,31 are x-halo)
 
 // Warps of a forward CTA.  With one team per CTA (NSUB = 1, small grids) the consumer keeps SM sub-partition 0 to itself:
@@ -83,33 +82,8 @@ __device__ __forceinline__ void y_advance(YState& S, int j, double hp2, const Pa
         }
     }
     if (MODE == 2) {
-#ifdef TF_PERT_SHFL
-        {   // perturbation probe: 4 extra 32-bit shuffles per row
-            int t = __double2loint(hp2);
-            t ^= __shfl_xor_sync(FULL, t, 1); t ^= __shfl_xor_sync(FULL, t, 2); t ^= __shfl_xor_sync(FULL, t, 4); t ^= __shfl_xor_sync(FULL, t, 8);
-            if (t == 0x7fffffff) S.phim += 1.0;
-        }
-#endif
-#ifdef TF_PERT_FMA
-        {   // perturbation probe: 4 extra independent DFMAs per row
-            const double a0 = fma(hp2, 1.25, S.h0), a1 = fma(hp2, 1.5, S.hm1), a2 = fma(S.h0, 1.75, S.hm1), a3 = fma(S.hp1, 2.25, S.hm1);
-            if (__double2hiint(a0) == 0x7ff12345 || __double2hiint(a1) == 0x7ff12345 || __double2hiint(a2) == 0x7ff12345 || __double2hiint(a3) == 0x7ff12345) S.phim += 1.0;
-        }
-#endif
-#ifdef TF_PERT_INT
-        {   // perturbation probe: 8 extra integer ops per row
-            int t = __double2loint(hp2);
-#pragma unroll
-            for (int k = 0; k < 8; ++k) t = t * 1664525 + j;
-            if (t == 0x7fffffff) S.phim += 1.0;
-        }
-#endif
-#ifdef TF_PERT_LESS_SHFL                              /* probe: what halving the shuffles would be worth (wrong results) */
-        const double f0R = S.c0.f0 * 1.0000001, f1R = S.c0.f1, LR = S.L0 + 1e-9;
-#else
         const double f0R = __shfl_down_sync(FULL, S.c0.f0, 1), f1R = __shfl_down_sync(FULL, S.c0.f1, 1);
         const double LR = __shfl_down_sync(FULL, S.L0, 1);
-#endif
         double phixp = DX.cb * fma(S.c0.f0 + f0R, LR - S.L0, (S.c0.f1 + f1R) * (S.hR0 - S.h0));
         if (!xface) phixp = 0.0;
         const double phixm = __shfl_up_sync(FULL, phixp, 1);
@@ -271,15 +245,6 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
             S.hm1 = 0.0; S.h0 = hq[0]; S.hp1 = hq[1]; S.hR0 = 0.0;
             S.c0 = {0, 0, 0, 0}; S.L0 = 0.0; S.fm = {0, 0, 0}; S.phim = 0.0;
             double o6[6], sD;
-#ifdef TF_EXP_NOPROD
-            if (interior) {
-#pragma unroll
-                for (int r = 0; r < RP; ++r) {
-                    double* sr = st + r * sstep;
-                    sr[0] = hq[r]; sr[SV] = hq[r + 1]; sr[2 * SV] = hq[r + 2] + 4.0; sr[3 * SV] = hq[r + 3]; sr[4 * SV] = bq[r];
-                }
-            } else
-#endif
             if (interior) {
                 y_advance<N, M, 0, true>(S, jlo - 2, hq[2], P, DX, DY, xface, 0.0, o6, sD);
                 y_advance<N, M, 1, true>(S, jlo - 1, hq[3], P, DX, DY, xface, 0.0, o6, sD);
@@ -323,9 +288,6 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
         // elim2_row emits the coefficients of the PREVIOUS row, so every store goes one row behind.
         Elim2 S = elim2_init();
         double e = 0.0;
-#ifdef TF_EXP_NOSTORE
-        int xacc = 0;
-#endif
         const int step = dir ? -nx : nx;
         int o = (dir ? ny : -1) * nx + i;                 // the row before the first one (32-bit element offset)
         const int offc = dir ? 3 * SV : SV, offa = dir ? SV : 3 * SV;   // half 1: c' = a, a' = c
@@ -336,9 +298,6 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
             const double* stc = st + offc;
             const double* sta = st + offa;
             const int nrow = min(RP, nrows - c * RP);
-#ifdef TF_EXP_NOCONS
-            if (nrow == RP && c > 0) { o += RP * step; } else
-#endif
             if (nrow == RP && c > 0) {
 #pragma unroll
                 for (int r = 0; r < RP; ++r) {
@@ -347,13 +306,7 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
                     double va, vb, vz;
                     elim2_row(S, e, cc, q, a, A, R, va, vb, vz);
                     e = A;
-#ifdef TF_EXP_NOSTORE
-                    xacc ^= __double2hiint(va) ^ __double2hiint(vb) ^ __double2hiint(vz);
-#elif defined(TF_EXP_STORE_L2)
-                    { const int o2 = (o & 0x3fffff); st3_if(outl, al + o2, va, be + o2, vb, zz + o2, vz); }   // 32 MB window per plane: stays in L2
-#else
                     st3_if(outl, al + o, va, be + o, vb, zz + o, vz);
-#endif
                     o += step;
                 }
             } else {
@@ -372,9 +325,6 @@ yfwd_ws_kernel(const __grid_constant__ CUtensorMap mU, const __grid_constant__ C
         }
         double va, vb, vz;
         elim2_flush(S, va, vb, vz);
-#ifdef TF_EXP_NOSTORE
-        if (xacc == 0x12345) vz = 1.0;
-#endif
         st3_if(outl, al + o, va, be + o, vb, zz + o, vz);
     }
 }
@@ -531,16 +481,6 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
                 }
             };
             const bool interior = (ilo >= 3) && (ilo + XW_CT + 2 <= nx - 2) && (ilo >= imin) && (ilo + XW_CT <= imax);
-#ifdef TF_EXP_X_NOPROD
-            if (interior) {
-#pragma unroll
-                for (int k = 0; k < NRMAX; ++k)
-                    if (pw + k * NP < XW_R && lane_ok) {
-                        const int r = pw + k * NP;
-                        st[r] = hq[k] * 0.1; st[SV + r] = 0.5 * hq[k]; st[2 * SV + r] = -0.2 * hq[k]; st[3 * SV + r] = wq[k];
-                    }
-            } else
-#endif
             if (interior) {
 #pragma unroll
                 for (int k = 0; k < NRMAX; ++k)
@@ -558,9 +498,6 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
         const int j = j0 + lane;
         const int rowok = (lane < XW_R && j < ny) ? 1 : 0;
         Elim2 S = elim2_init();
-#ifdef TF_EXP_X_NOSTORE
-        int xacc = 0;
-#endif
         double Ba = 0.0, B1 = 0.0, B2 = 0.0;              // backward face: the boundary face before the first column carries nothing
         const int step = dir ? -ny : ny;
         int o = (dir ? nx : -1) * ny + j;                 // the column before the first one
@@ -578,16 +515,9 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
                 double va, vb, vz;
                 elim2_row(S, Ba, cc, qq, a, Fa, R, va, vb, vz);
                 Ba = Fa; B1 = F1; B2 = F2;
-#ifdef TF_EXP_X_NOSTORE
-                xacc ^= __double2hiint(va) ^ __double2hiint(vb) ^ __double2hiint(vz);
-#else
                 st3_if(pred, alT + o, va, beT + o, vb, zzT + o, vz);
-#endif
                 o += step;
             };
-#ifdef TF_EXP_X_NOCONS
-            if (ncol == XW_CK && g > 0) { o += XW_CK * step; } else
-#endif
             if (ncol == XW_CK && g > 0) {
 #pragma unroll
                 for (int c = 0; c < XW_CK; ++c) column(c, rowok);
@@ -599,9 +529,6 @@ xfwd_ws_kernel(Params P, Dir DX, int mid, const double* __restrict__ u, const do
         }
         double va, vb, vz;
         elim2_flush(S, va, vb, vz);
-#ifdef TF_EXP_X_NOSTORE
-        if (xacc == 0x12345) vz = 1.0;
-#endif
         st3_if(rowok, alT + o, va, beT + o, vb, zzT + o, vz);
     }
 }

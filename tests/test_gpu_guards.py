@@ -1,4 +1,4 @@
-"""Out-of-bounds evidence without compute-sanitizer (closed on this GPU pool, profiles/r02_sanitizer.md): the context
+"""Out-of-bounds evidence without compute-sanitizer (closed on this GPU pool): the context
 gets a caller-supplied workspace that sits between two guard zones filled with a bit pattern, runs steps on grids with
 ragged strips / tiles / splits, and the guards must come back untouched.  (A write past one of the context's seven
 fields lands in the next field and shows up as a parity failure in tests/test_gpu_parity.py instead.)"""
