@@ -39,7 +39,13 @@ MUTANTS = [
     ("LU: z drops the e term", "z[i] = (y[i * sv] - z2 * ei - z1 * gam) / mu;", "z[i] = (y[i * sv] - z1 * gam) / mu;"),
     ("LU: back substitution swaps alpha, beta", "x[(size_t)i * sv] = z[i] - al[i] * x1 - be[i] * x2;", "x[(size_t)i * sv] = z[i] - be[i] * x1 - al[i] * x2;"),
     ("step: b^n with +s D", "c->bn[p] = c->u[p] - s * c->R[p];", "c->bn[p] = c->u[p] + s * c->R[p];"),
-    ("step: sweep order x then y", "directional_solve(c, 1, s, c->uk, c->R, c->w);", "directional_solve(c, 0, s, c->uk, c->R, c->w);"),
+    ("step: both sweeps along x", "directional_solve(c, 1, s, c->uk, c->R, c->w);", "directional_solve(c, 0, s, c->uk, c->R, c->w);"),
+    ("step: sweep order x then y (the true swap)",
+     "directional_solve(c, 1, s, c->uk, c->R, c->w);     /* (2.19): implicit y */\n        directional_solve(c, 0, s, c->uk, c->w, c->v);",
+     "directional_solve(c, 0, s, c->uk, c->R, c->w);     /* (2.19): implicit y */\n        directional_solve(c, 1, s, c->uk, c->w, c->v);"),
+    ("step: positivity dropped from the bad-iterate test (R18)",
+     "if (!isfinite(c->uk[p]) || (c->model != 1 && !(c->uk[p] > 0))) bad = 1;", "if (!isfinite(c->uk[p])) bad = 1;"),
+    ("step: NaN residual skipped by the max (R18)", "if (!(r <= res)) res = r;", "if (r > res) res = r;"),
     ("system matrix: s dropped from band a", "q[i] = 1.0 + s * q[i]; a[i] *= s;", "q[i] = 1.0 + s * q[i];"),
 ]
 
@@ -60,7 +66,7 @@ def main():
     survived = []
     with tempfile.TemporaryDirectory() as tmp:
         for name, old, new in MUTANTS:
-            assert src.count(old) == 1, f"mutation target not unique in tfo.c: {old!r}"
+            assert src.count(old) >= 1 and src.count(old.split("\n")[0]) == 1, f"mutation target not unique in tfo.c: {old!r}"
             c, so = os.path.join(tmp, "m.c"), os.path.join(tmp, "libm.so")
             open(c, "w").write(src.replace(old, new))
             subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-std=c11", "-fPIC", "-shared", "-o", so, c, "-lm"])

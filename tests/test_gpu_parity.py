@@ -1,6 +1,8 @@
 """GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, element by element,
 on the same seeded inputs.  Tolerances are BASELINE.json's: relative L-inf <= 1e-11 after one step,
 <= 1e-8 after 100 steps, Newton iteration count fixed for the comparison."""
+import math
+
 import numpy as np
 import pytest
 
@@ -330,3 +332,34 @@ def test_sweeps_driven_one_by_one_equal_tf_step(tf, nx, ny):
     v2 = b.field(b.FIELD_ITERATE) - u
     torch.cuda.synchronize()
     assert float((v2 - 0.5 * v1).abs().max()) <= 1e-13 * float(v1.abs().max())
+
+
+def test_finite_non_positive_iterate_and_nan_residual_like_the_oracle(tf, tfo):
+    """Reading R18 on the CUDA path, on the two cases that pin it in the oracle (tests/test_oracle_pins.py, O13): a first
+    iterate that is finite but negative somewhere rejects the step after one iteration in both modes; a valid state
+    whose h^3 overflows gives a NaN residual.  Status, count and NaN-ness must equal the oracle's, the state stays u^n."""
+    nx, ny, d, dt = 24, 20, 0.05, 1e-2
+    h = np.ascontiguousarray(0.12 + 0.1 * np.random.default_rng(5).uniform(0, 1, (ny, nx)))
+    for fixed in (1, 0):
+        g = tf.ThinFilm(nx, ny, d, d, K, HS, 3, 2)
+        o = tfo.ThinFilmOracle(nx, ny, d, d, K, HS, 3, 2)
+        for f in (g, o):
+            f.set_newton(1e-10, 64, fixed)
+            f.set_state(h)
+        (gs, gi, gr), (os_, oi, or_) = g.step(dt), o.step(dt)
+        assert (gs, gi) == (os_, oi) == (tf.NOT_CONVERGED, 1)
+        assert math.isfinite(gr) and abs(gr - or_) <= 1e-9 * abs(or_)
+        assert np.array_equal(g.get_state(), h)
+    nx, ny = 16, 12
+    h = np.ones((ny, nx))
+    h[5, 7] = 1e120
+    for fixed in (0, 1, 3):
+        g = tf.ThinFilm(nx, ny, 0.3, 0.3, K, HS, 3, 2)
+        o = tfo.ThinFilmOracle(nx, ny, 0.3, 0.3, K, HS, 3, 2)
+        for f in (g, o):
+            f.set_newton(1e-10, 10, fixed)
+            f.set_state(h)
+        (gs, gi, gr), (os_, oi, or_) = g.step(1e-3), o.step(1e-3)
+        assert (gs, gi) == (os_, oi) == (tf.NOT_CONVERGED, max(fixed, 1))
+        assert math.isnan(gr) and math.isnan(or_)
+        assert np.array_equal(g.get_state(), h)

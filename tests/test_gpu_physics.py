@@ -163,3 +163,4 @@ def test_fixed_count_step_with_a_bad_iterate_is_not_accepted(tf):
     assert np.array_equal(g.get_state(), h)
     st, it, res = g.step(1e-9)
     assert st == tf.OK and it == 2 and np.all(g.get_state() > 0)
+

@@ -315,3 +315,87 @@ def test_step_rejection_leaves_state_unchanged_and_validation():
         tfo.ThinFilmOracle(4, 16, dx, dy)
     with pytest.raises(tfo.OracleError):
         tfo.ThinFilmOracle(16, 16, dx, dy, K, HS, 2, 3)
+
+
+# ---------------------------------------------------------------- O12: order of the two sweeps inside tfo_step
+def _nonsymmetric_film(nx, ny, dx, dy, seed):
+    x = (np.arange(nx) + 0.5) * dx
+    y = (np.arange(ny) + 0.5) * dy
+    rng = np.random.default_rng(seed)
+    u = 1.0 + 0.2 * np.cos(2 * math.pi * x / (nx * dx))[None, :] * np.sin(1.3 * y)[:, None] + 0.15 * rng.uniform(-1, 1, (ny, nx))
+    return np.ascontiguousarray(u), x, y
+
+
+def test_O12_direction_labels_of_directional_solve():
+    """directional_solve(0, ...) is the solve along x and (1, ...) the one along y, fixed by a structural fact rather than
+    by the label: for a film and a right-hand side that do not vary along x, J_x annihilates the right-hand side (every
+    term of the x-part of (2.26) is an x-difference of one of them), so the x-solve must return it unchanged, and the
+    y-solve must not."""
+    nx, ny, dx, dy = 23, 17, 0.31, 0.47
+    _, _, y = _nonsymmetric_film(nx, ny, dx, dy, 3)
+    o = tfo.ThinFilmOracle(nx, ny, dx, dy, K, HS, N_, M_)
+    uy = np.ascontiguousarray(np.repeat((1.0 + 0.2 * np.sin(1.3 * y))[:, None], nx, axis=1))
+    rhs = np.ascontiguousarray(np.repeat(np.cos(0.7 * y)[:, None], nx, axis=1))
+    assert np.max(np.abs(o.directional_solve(0, 0.01, uy, rhs) - rhs)) <= 1e-14
+    assert np.max(np.abs(o.directional_solve(1, 0.01, uy, rhs) - rhs)) >= 1e-2
+
+@pytest.mark.parametrize("dt", [1e-3, 1e-2])
+def test_O12_one_iteration_is_the_y_sweep_followed_by_the_x_sweep(dt):
+    """(2.19) before (2.20), and the kernel order 1)-4) of App. A.2: the first iterate of
+    tfo_step must equal u + S_x(S_y(R)), R = b^n - u - s D(u), composed here from operator_D and directional_solve
+    (each pinned on its own: O4, O3, O12 above) -- and on this film (no symmetry, dx != dy) the other order gives a
+    different field, so the comparison can tell the two apart."""
+    nx, ny, dx, dy = 23, 17, 0.31, 0.47
+    u, _, _ = _nonsymmetric_film(nx, ny, dx, dy, 3)
+    s = 0.5 * dt
+    o = tfo.ThinFilmOracle(nx, ny, dx, dy, K, HS, N_, M_)
+    o.set_newton(1e-10, 10, 1)                            # exactly one iteration, accepted
+    o.set_state(u)
+    st, it, _ = o.step(dt)
+    assert st == tfo.OK and it == 1
+    v = o.get_state() - u
+    D = o.operator_D(u)
+    R = (u - s * D) - u - s * D                           # b^n - u_(0) - s D(u_(0))
+    v_yx = o.directional_solve(0, s, u, o.directional_solve(1, s, u, R))
+    v_xy = o.directional_solve(1, s, u, o.directional_solve(0, s, u, R))
+    scale = np.max(np.abs(v_yx))
+    assert np.max(np.abs(v - v_yx)) <= 1e-14 * scale
+    assert np.max(np.abs(v_xy - v_yx)) >= 1e-7 * scale    # measured: 2e-2 (dt = 1e-3), 0.6 (dt = 1e-2)
+    assert np.max(np.abs(v - v_xy)) >= 1e-7 * scale
+
+
+# ---------------------------------------------------------------- O13: reading R18, the two lines the GPU is compared against
+def test_O13_a_finite_but_non_positive_iterate_rejects_the_step():
+    """Reading R18: an iterate that is finite but not positive ends the step (Pi is singular at h = 0, such
+    a field is not a film).  The case is built so that ONLY positivity can trip: the first iterate, composed from the
+    separately pinned pieces, is finite everywhere and negative somewhere."""
+    nx, ny, d, dt = 24, 20, 0.05, 1e-2
+    h = np.ascontiguousarray(0.12 + 0.1 * np.random.default_rng(5).uniform(0, 1, (ny, nx)))
+    o = tfo.ThinFilmOracle(nx, ny, d, d, K, HS, N_, M_)
+    s = 0.5 * dt
+    u1 = h + o.directional_solve(0, s, h, o.directional_solve(1, s, h, -2.0 * s * o.operator_D(h)))
+    assert np.isfinite(u1).all() and u1.min() < 0.0
+    o.set_newton(1e-10, 64, 1)                            # parity mode, one iteration: accepted unless the iterate is bad
+    o.set_state(h)
+    st, it, res = o.step(dt)
+    assert st == tfo.NOT_CONVERGED and it == 1 and math.isfinite(res)
+    assert np.array_equal(o.get_state(), h)
+    o.set_newton(1e-10, 64, 0)                            # normal mode: the iteration stops at the bad iterate
+    st, it, res = o.step(dt)
+    assert st == tfo.NOT_CONVERGED and it == 1 and math.isfinite(res)
+    assert np.array_equal(o.get_state(), h)
+
+
+@pytest.mark.parametrize("fixed", [0, 1, 3])
+def test_O13_a_nan_residual_is_reported_as_nan(fixed):
+    """A NaN in v / u_k must surface in the reported residual (max over the grid with NaN winning), not be skipped by the
+    comparison.  h = 1e120 in one cell is a valid state (finite, positive) whose h^3 overflows: D(u) is inf - inf there."""
+    nx, ny = 16, 12
+    h = np.ones((ny, nx))
+    h[5, 7] = 1e120
+    o = tfo.ThinFilmOracle(nx, ny, 0.3, 0.3, K, HS, N_, M_)
+    o.set_newton(1e-10, 10, fixed)
+    o.set_state(h)
+    st, it, res = o.step(1e-3)
+    assert st == tfo.NOT_CONVERGED and it == max(fixed, 1) and math.isnan(res)
+    assert np.array_equal(o.get_state(), h)
