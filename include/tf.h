@@ -50,7 +50,8 @@ size_t tf_workspace_bytes(int nx, int ny);
 /*
  * Create a context (problem statement: PAPER.md:47 (1.1), 86-91 (1.7)-(1.8), 297-302 (2.28)).
  *   nx, ny >= 5 and (nx+1)*(ny+1) < 2^31 (the kernels index a field with 32-bit element offsets);
- *   dx, dy, kappa, hstar > 0; integer exponents n > m >= 1; bc = TF_BC_NOFLUX
+ *   dx, dy, kappa, hstar > 0; integer exponents 16 >= n > m >= 1 (the powers are formed by repeated multiplication;
+ *   a larger n is TF_ERR_INVALID_ARG); bc = TF_BC_NOFLUX
  *   (anything else: TF_ERR_UNSUPPORTED -- the paper defines no other boundary condition).
  * tf_create allocates tf_workspace_bytes() of device memory itself and uses the legacy
  * default stream.  tf_create_with_workspace borrows `dev_ws` (device pointer, 256-byte
@@ -172,7 +173,8 @@ tf_status tf_advance_adaptive(tf_ctx* ctx, tf_adaptive* ctl, int n_accept, int m
  * (those past the deciding one return at once), a control kernel takes the decision of Fig. 1 from the residual
  * records (accept / shrink / grow, dt_min, attempt cap) and a copy kernel commits u^{n+1} if the step was accepted.
  * The host reads the control block once per chunk.  Same arguments, same results as tf_advance_adaptive: the sequence
- * of (dt, status, iterations, residual) and the films are identical bit for bit.  At most 1024 attempts per call.
+ * of (dt, status, iterations, residual) and the films are identical bit for bit, for any number of attempts (the device
+ * records them in a ring of 1024 entries that the host drains between chunks).
  * TF_ERR_UNSUPPORTED with fixed_iters > 0 or the extra solution criterion switched on.
  */
 tf_status tf_advance_adaptive_device(tf_ctx* ctx, tf_adaptive* ctl, int n_accept, int max_attempts,

@@ -819,7 +819,6 @@ tf_status tf_advance_adaptive_device(tf_ctx* c, tf_adaptive* ctl, int n_accept, 
     if (c->fixed_iters > 0 || c->max_rel_change > 0.0 || c->max_trunc > 0.0)
         return fail(c, TF_ERR_UNSUPPORTED, "tf_advance_adaptive_device: fixed_iters and the extra solution criterion need the host controller");
     if (max_attempts <= 0) max_attempts = 50 * std::max(n_accept, 1);
-    if (max_attempts > CT_HIST_CAP) max_attempts = CT_HIST_CAP;          // one run records at most CT_HIST_CAP attempts
     CtlParams P;
     P.shrink = ctl->shrink; P.grow = ctl->grow; P.dt_min = ctl->dt_min; P.dt_max = ctl->dt_max; P.tol = c->tol;
     P.grow_after = ctl->grow_after; P.n_accept = n_accept; P.max_attempts = max_attempts; P.kmax = c->max_iter;
@@ -831,7 +830,24 @@ tf_status tf_advance_adaptive_device(tf_ctx* c, tf_adaptive* ctl, int n_accept, 
     const unsigned gcopy = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)c->num_sms * 16);
     std::vector<double> host(CT_SIZE + 4 * (size_t)CT_HIST_CAP);
     double* hc = host.data();
-    int done = 0, attempts = 0, accepted = 0;
+    int done = 0, attempts = 0, accepted = 0, drained = 0;
+    // the device keeps the attempt records in a ring of CT_HIST_CAP entries; records [drained, upto) are copied out
+    // before the next chunk (<= 16 attempts) could overwrite them, so a run may take any number of attempts
+    auto drain = [&](int upto) -> cudaError_t {
+        while (drained < upto) {
+            const int at = drained % CT_HIST_CAP, cnt = std::min(upto - drained, CT_HIST_CAP - at);
+            cudaError_t e = cudaMemcpyAsync(hc + CT_SIZE, c->ctl_hist + 4 * (size_t)at, sizeof(double) * 4 * (size_t)cnt,
+                                            cudaMemcpyDeviceToHost, c->stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+            if (e != cudaSuccess) return e;
+            for (int a = drained; a < drained + cnt && a < hist_cap; ++a) {
+                const double* r = hc + CT_SIZE + 4 * (size_t)(a - drained);
+                hist[a].dt = r[0]; hist[a].status = (int)r[1]; hist[a].newton_iters = (int)r[2]; hist[a].residual = r[3];
+            }
+            drained += cnt;
+        }
+        return cudaSuccess;
+    };
     while (!done) {
         const int chunk = std::max(1, std::min({n_accept - accepted + 1, 16, max_attempts - attempts + 1}));
         for (int a = 0; a < chunk; ++a) {
@@ -850,14 +866,9 @@ tf_status tf_advance_adaptive_device(tf_ctx* c, tf_adaptive* ctl, int n_accept, 
         done = (int)hc[CT_DONE];
         if (!done && accepted >= n_accept) done = 1;
         if (!done && attempts >= max_attempts) done = 3;
+        if (attempts - drained > CT_HIST_CAP - 32) TF_CUDA(c, drain(attempts));
     }
-    TF_CUDA(c, cudaMemcpyAsync(hc + CT_SIZE, c->ctl_hist, sizeof(double) * 4 * (size_t)std::min(attempts, CT_HIST_CAP),
-                               cudaMemcpyDeviceToHost, c->stream));
-    TF_CUDA(c, cudaStreamSynchronize(c->stream));
-    for (int a = 0; a < attempts && a < hist_cap && a < CT_HIST_CAP; ++a) {
-        const double* r = hc + CT_SIZE + 4 * a;
-        hist[a].dt = r[0]; hist[a].status = (int)r[1]; hist[a].newton_iters = (int)r[2]; hist[a].residual = r[3];
-    }
+    TF_CUDA(c, drain(attempts));
     ctl->dt = hc[CT_DT];
     c->have_acc = false;
     if (t_advanced) *t_advanced = hc[CT_T];

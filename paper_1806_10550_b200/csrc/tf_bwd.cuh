@@ -309,8 +309,8 @@ xbwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
                 const double uo = U[c];
                 const double un = uo + v;
                 const double rr = fabs(v) * rcp(uo);
-                res = fmax(res, rowok ? rr : 0.0);           // a NaN/inf iterate is caught by `bad`
-                bad |= (rowok && !(un > 0.0 && un <= 1.7976931348623157e308)) ? 1 : 0;
+                res = fmax(res, rowok ? rr : 0.0);           // fmax drops a NaN ratio: bit 1 of `bad` remembers it
+                bad |= (rowok && !(un > 0.0 && un <= 1.7976931348623157e308)) ? (un != un ? 3 : 1) : 0;
                 *pu = un;
             } else {
                 *pu = v;
@@ -340,7 +340,9 @@ xbwd2_tma_kernel(const __grid_constant__ CUtensorMap mA, const __grid_constant__
     }
     if (lane == 0) tma_store_wait_all<0>();
     if (!UPDATE) return;
-    if (res != res) res = __longlong_as_double(0x7ff8000000000000LL);
+    // (2.22) with a NaN winning the max, as in the definition written out: u_k is a finite positive film, so v / u_k is
+    // NaN exactly when v is, i.e. exactly when u_k + v is
+    if (bad & 2) res = __longlong_as_double(0x7ff8000000000000LL);
     res = warp_max_nonneg(res);
     bad = __any_sync(0xffffffffu, bad);
     if (lane == 0) {
@@ -381,12 +383,14 @@ xbwd2_plain_kernel(int nx, int ny, int mid, const double* __restrict__ alT, cons
         const double rr = fabs(v) * rcp(uo);
         if (rowok) {
             res = fmax(res, rr);
-            bad |= !(un > 0.0 && un <= 1.7976931348623157e308) ? 1 : 0;
+            bad |= !(un > 0.0 && un <= 1.7976931348623157e308) ? (un != un ? 3 : 1) : 0;
             unew[(size_t)j * nx + i] = un;
         }
         v2 = v1; v1 = v;
     }
-    if (res != res) res = __longlong_as_double(0x7ff8000000000000LL);
+    // (2.22) with a NaN winning the max, as in the definition written out: u_k is a finite positive film, so v / u_k is
+    // NaN exactly when v is, i.e. exactly when u_k + v is
+    if (bad & 2) res = __longlong_as_double(0x7ff8000000000000LL);
     res = warp_max_nonneg(res);
     bad = __any_sync(0xffffffffu, bad);
     if (lane == 0) {

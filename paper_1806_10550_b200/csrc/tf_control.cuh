@@ -16,7 +16,7 @@ namespace tf {
 
 // control block, doubles: the layout the host reads back
 enum { CT_DT = 0, CT_S, CT_T, CT_ACCEPTED, CT_STREAK, CT_DONE, CT_GATE_RES, CT_GATE_BAD, CT_ATTEMPTS, CT_COMMIT, CT_SIZE = 16 };
-constexpr int CT_HIST_CAP = 1024;        // attempts recorded per run chunk: {dt, status, iters, res}
+constexpr int CT_HIST_CAP = 1024;        // ring of attempt records {dt, status, iters, res}; the host drains it every <= CT_HIST_CAP - 16 attempts
 // CT_DONE: 0 running, 1 n_accept reached, 2 dt fell below dt_min, 3 attempt cap reached
 
 struct CtlParams {
@@ -51,7 +51,7 @@ __global__ void ctl_end_kernel(double* ctl, const double* red, double* hist, Ctl
     }
     const double dt = ctl[CT_DT];
     const int a = (int)ctl[CT_ATTEMPTS];
-    if (a < CT_HIST_CAP) { hist[4 * a] = dt; hist[4 * a + 1] = (double)status; hist[4 * a + 2] = (double)k; hist[4 * a + 3] = res; }
+    { double* h = hist + 4 * (a % CT_HIST_CAP); h[0] = dt; h[1] = (double)status; h[2] = (double)k; h[3] = res; }   // a ring: the host drains it before it wraps
     ctl[CT_ATTEMPTS] = (double)(a + 1);
     if (status == 0) {
         ctl[CT_ACCEPTED] += 1.0;

@@ -185,3 +185,23 @@ def test_device_controller_with_the_nlc_pressure_equals_host(tf):
         g.close()
     assert outs[0][:3] == outs[1][:3] and np.array_equal(outs[0][3], outs[1][3])
     assert sum(1 for x in outs[0][2] if x[1] == 0) == 10
+
+
+def test_device_controller_takes_more_attempts_than_its_record_ring_holds(tf):
+    """The device records attempts in a ring of 1024 entries that the host drains between chunks, so a run is not
+    limited to 1024 attempts (it was, silently, in round 2): 1100 accepted steps of a small film, with the default
+    attempt cap of 50 * n_accept, equal the host controller bit for bit -- every record, the time, the next dt, the film."""
+    nx, ny = 48, 40
+    h = rough_film(nx, ny, seed=2)
+    outs = []
+    for on_device in (True, False):
+        g = tf.ThinFilm(nx, ny, 0.4, 0.4, K, HS, 3, 2)
+        g.set_newton(1e-10, 10, 0)
+        g.set_state(h)
+        t, dt, hist = tf.advance_adaptive(g, 0.08, 1100, grow=1.3, shrink=0.5, dt_max=0.02, dt_min=1e-9, on_device=on_device)
+        outs.append((t, dt, hist, g.get_state()))
+        g.close()
+    dev, host = outs
+    assert len(dev[2]) > 1100 and sum(1 for x in dev[2] if x[1] == tf.OK) == 1100      # it rejected on the way
+    assert dev[0] == host[0] and dev[1] == host[1] and dev[2] == host[2]
+    assert np.array_equal(dev[3], host[3])

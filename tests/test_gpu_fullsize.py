@@ -172,6 +172,59 @@ def test_penta_solve_full_length_systems(tf, tfo, direction):
     assert np.max(np.abs(Ax - y)) / (normA * np.max(np.abs(xs)) + np.max(np.abs(y))) <= 1e-14
 
 
+@pytest.mark.parametrize("direction", [1, 0])
+def test_penta_solve_config4_as_timed_16384_systems(tf, tfo, direction):
+    """BASELINE.json config 4 as bench.py times it: ALL 16384 systems of 16384 unknowns in one tf_penta_solve per
+    direction (512 x 2 CTAs of the two-sided forward kernel, more than are resident at once), solver of App. A.2,
+    PAPER.md:729-738.  The 2 GiB arrays are drawn on the device by bench.py's recipe (the bands U[-1,1], strictly
+    dominant diagonal); 256 evenly spaced systems are overwritten by inputs.penta_system(rows=...), which the host can
+    reproduce row by row, and compared with the oracle (<= 1e-12); EVERY system is checked by its backward error
+    ||Ax - y||_inf / (||A||_inf ||x||_inf + ||y||_inf) <= 1e-14, evaluated with torch on the device (no oracle needed)."""
+    import torch
+    n = inputs.config(4)["nrow"]
+    assert n == 16384 and inputs.config(4)["ncol"] == n
+    gen = torch.Generator(device="cuda").manual_seed(inputs.config(4)["seed"] + direction)
+    U = lambda lo, hi: torch.rand(n, n, dtype=torch.float64, device="cuda", generator=gen) * (hi - lo) + lo
+    e, c, a, b, y = U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1), U(-1, 1)
+    d = 1 + e.abs() + c.abs() + a.abs() + b.abs() + U(0, 1)
+    sample = list(range(31, n, 64))                                # 256 systems, among them strip seams and both halves
+    rows = inputs.penta_system(n, n, seed=40 + direction, rows=sample)
+    idx = torch.tensor(sample, device="cuda")
+    for dev, host in zip((e, c, d, a, b, y), rows):
+        t = torch.from_numpy(host).cuda()
+        if direction == 0:
+            dev[idx, :] = t                                        # system s = row s
+        else:
+            dev[:, idx] = t.T                                      # system s = column s
+    ws = torch.empty(tf.lib().tf_penta_workspace_bytes(n, n), dtype=torch.uint8, device="cuda")
+    x = torch.full_like(e, float("nan"))
+    tf.penta_solve(direction, e, c, d, a, b, y, out=x, workspace=ws)
+    torch.cuda.synchronize()
+    del ws
+    assert bool(torch.isfinite(x).all())
+    # sampled systems against the oracle
+    ref = tfo.penta_solve(0, *rows, omp=True)
+    got = (x[idx, :] if direction == 0 else x[:, idx].T).cpu().numpy()
+    assert np.max(np.abs(got - ref)) / np.max(np.abs(ref)) <= 1e-12
+    # every system by backward error; `ax` = the dimension a system runs along
+    ax = 1 if direction == 0 else 0
+    L = lambda t, lo, hi: t.narrow(ax, lo, hi - lo)
+    r = d * x
+    L(r, 1, n).add_(L(c, 1, n) * L(x, 0, n - 1))
+    L(r, 2, n).add_(L(e, 2, n) * L(x, 0, n - 2))
+    L(r, 0, n - 1).add_(L(a, 0, n - 1) * L(x, 1, n))
+    L(r, 0, n - 2).add_(L(b, 0, n - 2) * L(x, 2, n))
+    r.sub_(y)
+    res = r.abs().amax(dim=ax)                                     # per system
+    del r
+    normA = (e.abs() + c.abs() + d.abs() + a.abs() + b.abs()).amax(dim=ax)
+    berr = res / (normA * x.abs().amax(dim=ax) + y.abs().amax(dim=ax))
+    assert berr.numel() == n
+    assert float(berr.max()) <= 1e-14, (int(berr.argmax()), float(berr.max()))
+    del e, c, d, a, b, y, x
+    torch.cuda.empty_cache()
+
+
 # ------------------------------------------------------------------ config 2 at full size: adaptive controller
 def test_config2_4096_adaptive_run(tf, tfo):
     """Config 2 (4096^2, uniform 0.12 film with 16 Gaussian depressions, adaptive dt from 1e-3): the controller of
