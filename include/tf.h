@@ -402,6 +402,16 @@ const char* tf_last_error(const tf_ctx* ctx);
 tf_status tf_set_profiling(tf_ctx* ctx, int on);
 tf_status tf_get_profile(tf_ctx* ctx, double ms[TF_PROFILE_SLOTS], unsigned long long launches[TF_PROFILE_SLOTS]);
 
+/*
+ * Measured fp64 arithmetic peak of the current device, the denominator of bench.py's "alu" roofline (SURVEY.md section 6:
+ * the fp64 peak is not in MEASURED_PEAKS.json and has to be measured).  Launches `launches` >= 1 times (after one untimed
+ * launch) a kernel in which every thread runs 8 independent chains of dependent DFMAs, 16 CTAs of 256 threads per SM
+ * (2048 threads, 16 384 chains per SM: the fp64 pipe is the only limit), each launch timed with CUDA events on
+ * cuda_stream.  *best_dfma_per_s / *mean_dfma_per_s: thread-level DFMA instructions per second of the fastest launch /
+ * over all launches (either may be NULL); 2 flops each.  A launch takes about 2 ms.  Synchronises the stream.
+ */
+tf_status tf_fp64_peak(int launches, double* best_dfma_per_s, double* mean_dfma_per_s, void* cuda_stream);
+
 /* Number of kernels this library has launched since load (all contexts); for bench.py's
  * gpu_launches claim. */
 unsigned long long tf_kernel_launches(void);

@@ -1470,6 +1470,59 @@ tf_status tf_penta_solve_static(int nrow, int ncol, int dir, const double* e, co
     return tf_penta_solve_ex(nrow, ncol, dir, TF_PENTA_LU, 0, e, c, d, a, b, rhs, x, scratch, cuda_stream);
 }
 
+// ---- tf_fp64_peak: DFMA micro-benchmark (the denominator of the "alu" roofline)
+namespace {
+
+constexpr int DFMA_CHAINS = 8, DFMA_ITERS = 16384;
+
+__global__ void __launch_bounds__(256) dfma_probe_kernel(double* sink, double a, double b)
+{
+    double x[DFMA_CHAINS];
+#pragma unroll
+    for (int k = 0; k < DFMA_CHAINS; ++k) x[k] = 1.0 + 1e-3 * (double)(threadIdx.x + k);
+#pragma unroll 4
+    for (int it = 0; it < DFMA_ITERS; ++it) {
+#pragma unroll
+        for (int k = 0; k < DFMA_CHAINS; ++k) x[k] = fma(x[k], a, b);      // a, b are run-time values: nothing folds
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < DFMA_CHAINS; ++k) s += x[k];
+    if (s == -1.2345e300) *sink = s;                                        // never true; keeps the chains alive
+}
+
+}  // namespace
+
+tf_status tf_fp64_peak(int launches, double* best_dfma_per_s, double* mean_dfma_per_s, void* cuda_stream)
+{
+    if (launches < 1 || launches > 1000) return fail(nullptr, TF_ERR_INVALID_ARG, "tf_fp64_peak: 1 <= launches <= 1000");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const unsigned grid = (unsigned)num_sms() * 16u;
+    cudaEvent_t e0, e1;
+    TF_CUDA(nullptr, cudaEventCreate(&e0));
+    cudaError_t e = cudaEventCreate(&e1);
+    if (e != cudaSuccess) { cudaEventDestroy(e0); return cuda_fail(nullptr, e, "cudaEventCreate"); }
+    const double work = (double)grid * 256.0 * DFMA_CHAINS * DFMA_ITERS;
+    double best = 0.0, total_ms = 0.0;
+    for (int l = -1; l < launches && e == cudaSuccess; ++l) {                // l = -1: untimed warm-up
+        cudaEventRecord(e0, st);
+        dfma_probe_kernel<<<grid, 256, 0, st>>>(nullptr, 0.999999, 1e-6);
+        cudaEventRecord(e1, st);
+        count_launch(1);
+        e = cudaEventSynchronize(e1);
+        float ms = 0.0f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (e == cudaSuccess && l >= 0) { total_ms += ms; best = std::max(best, work / (ms * 1e-3)); }
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "tf_fp64_peak");
+    if (best_dfma_per_s) *best_dfma_per_s = best;
+    if (mean_dfma_per_s) *mean_dfma_per_s = work * launches / (total_ms * 1e-3);
+    return TF_OK;
+}
+
 size_t tf_betti_workspace_bytes(int nx, int ny, int nthr)
 {
     if (nx < 1 || ny < 1 || nthr < 1) return 0;

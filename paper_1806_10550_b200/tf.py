@@ -80,6 +80,7 @@ SYMBOLS = {
     "tf_get_profile": (ctypes.c_int, [_vp, _dp, ctypes.POINTER(ctypes.c_ulonglong)]),
     "tf_last_error": (ctypes.c_char_p, [_vp]),
     "tf_kernel_launches": (ctypes.c_ulonglong, []),
+    "tf_fp64_peak": (ctypes.c_int, [ctypes.c_int, _dp, _dp, _vp]),
 }
 
 
@@ -111,6 +112,17 @@ def _err(handle, status, what):
 
 def kernel_launches():
     return int(lib().tf_kernel_launches())
+
+
+def fp64_peak(launches=5, stream=None):
+    """tf_fp64_peak: (best, mean) thread-level DFMA instructions per second of the current device, measured."""
+    torch = _torch()
+    best, mean = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    st = (torch.cuda.current_stream() if stream is None else stream).cuda_stream
+    rc = lib().tf_fp64_peak(int(launches), ctypes.byref(best), ctypes.byref(mean), st)
+    if rc != OK:
+        _err(None, rc, "tf_fp64_peak")
+    return best.value, mean.value
 
 
 def _torch():

@@ -12,7 +12,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def declared_symbols():
     src = open(os.path.join(ROOT, "include", "tf.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return set(re.findall(r"\b(tf_[a-z_]+)\s*\(", src))
+    return set(re.findall(r"\b(tf_[a-z0-9_]+)\s*\(", src))
 
 
 def test_library_exports_every_declared_symbol():
