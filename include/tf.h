@@ -141,7 +141,7 @@ tf_status tf_set_solution_criteria(tf_ctx* ctx, double max_rel_change);
  * field of the workspace).  A converged step is accepted only if
  *     max_ij (dt^3/12) |u_ttt| / |u^{n+1}|  <=  max_rel_truncation,
  * else tf_step returns TF_REJECTED with the state (and the stored a_{n-1/2}) untouched.  The first step after
- * tf_set_state, tf_accept or tf_advance_adaptive_device has no history and is not tested.  0 = off (default).
+ * tf_set_state or tf_accept has no history and is not tested.  0 = off (default).
  * tf_last_truncation_estimate: the estimate of the last converged step that was tested (0 if none).
  * One fused pass over four fields per step (40 B per grid point), order-independent max.
  */
@@ -175,7 +175,10 @@ tf_status tf_advance_adaptive(tf_ctx* ctx, tf_adaptive* ctl, int n_accept, int m
  * The host reads the control block once per chunk.  Same arguments, same results as tf_advance_adaptive: the sequence
  * of (dt, status, iterations, residual) and the films are identical bit for bit, for any number of attempts (the device
  * records them in a ring of 1024 entries that the host drains between chunks).
- * TF_ERR_UNSUPPORTED with fixed_iters > 0 or the extra solution criterion switched on.
+ * Both extra solution criteria (tf_set_solution_criteria, tf_set_truncation_criterion) are decided on the device too:
+ * their reductions run behind a converged attempt and read dt, dt_prev and the history flag from device memory; a
+ * rejected attempt is recorded as TF_REJECTED and shrinks dt as on the host.  The stored a_{n-1/2} carries over from
+ * and to tf_step.  TF_ERR_UNSUPPORTED with fixed_iters > 0.
  */
 tf_status tf_advance_adaptive_device(tf_ctx* ctx, tf_adaptive* ctl, int n_accept, int max_attempts,
                                      double* t_advanced, tf_step_record* hist, int hist_cap, int* nhist);

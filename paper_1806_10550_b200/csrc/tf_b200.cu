@@ -816,14 +816,18 @@ tf_status tf_advance_adaptive_device(tf_ctx* c, tf_adaptive* ctl, int n_accept, 
         !std::isfinite(ctl->dt_max))
         return fail(c, TF_ERR_INVALID_ARG, "tf_advance_adaptive_device: need dt > 0, 0 < shrink < 1, grow >= 1, grow_after >= 1, 0 < dt_min <= dt_max");
     if (!c->have_state) return fail(c, TF_ERR_STATE, "no state set");
-    if (c->fixed_iters > 0 || c->max_rel_change > 0.0 || c->max_trunc > 0.0)
-        return fail(c, TF_ERR_UNSUPPORTED, "tf_advance_adaptive_device: fixed_iters and the extra solution criterion need the host controller");
+    if (c->fixed_iters > 0)
+        return fail(c, TF_ERR_UNSUPPORTED, "tf_advance_adaptive_device: fixed_iters needs the host controller");
     if (max_attempts <= 0) max_attempts = 50 * std::max(n_accept, 1);
     CtlParams P;
     P.shrink = ctl->shrink; P.grow = ctl->grow; P.dt_min = ctl->dt_min; P.dt_max = ctl->dt_max; P.tol = c->tol;
     P.grow_after = ctl->grow_after; P.n_accept = n_accept; P.max_attempts = max_attempts; P.kmax = c->max_iter;
+    P.max_rel_change = c->max_rel_change; P.max_trunc = c->max_trunc;
+    const bool crit_change = c->max_rel_change > 0.0, crit_trunc = c->max_trunc > 0.0;
     double init[CT_SIZE] = {0};
     init[CT_DT] = std::min(ctl->dt, ctl->dt_max);
+    init[CT_HAVE_ACC] = (crit_trunc && c->have_acc) ? 1.0 : 0.0;         // the history of the host-side steps carries over
+    init[CT_DT_PREV] = c->dt_prev;
     TF_CUDA(c, cudaMemcpyAsync(c->ctl, init, sizeof(init), cudaMemcpyHostToDevice, c->stream));
     TF_CUDA(c, cudaStreamSynchronize(c->stream));                        // `init` is on the stack
     const size_t n = (size_t)c->P.nx * c->P.ny;
@@ -854,9 +858,16 @@ tf_status tf_advance_adaptive_device(tf_ctx* c, tf_adaptive* ctl, int n_accept, 
             ctl_begin_kernel<<<1, 256, 0, c->stream>>>(c->ctl, c->red, P);
             for (int k = 0; k < c->max_iter; ++k)
                 TF_CUDA(c, launch_iteration(c, 1.0, k, -1, true, 3, c->ctl + CT_S, c->ctl + CT_GATE_RES));
+            ctl_mid_kernel<<<1, 1, 0, c->stream>>>(c->ctl, c->red, P);
+            if (crit_change)
+                max_rel_change_ctl_kernel<<<RED_BLOCKS, RED_THREADS, 0, c->stream>>>(n, c->u, c->uk, c->ctl + CT_CONV, c->ctl + CT_CHANGE);
+            if (crit_trunc)
+                truncation_ctl_kernel<<<RED_BLOCKS, RED_THREADS, 0, c->stream>>>(n, c->u, c->uk, c->bn, c->acc, c->w, c->ctl + CT_CONV,
+                                                                                  c->ctl + CT_DT, c->ctl + CT_DT_PREV,
+                                                                                  c->ctl + CT_HAVE_ACC, c->ctl + CT_TRUNC);
             ctl_end_kernel<<<1, 1, 0, c->stream>>>(c->ctl, c->red, c->ctl_hist, P);
-            ctl_commit_kernel<<<gcopy, 256, 0, c->stream>>>(n, c->uk, c->u, c->ctl);
-            count_launch(3);
+            ctl_commit_kernel<<<gcopy, 256, 0, c->stream>>>(n, c->uk, c->u, c->w, c->acc, c->ctl);
+            count_launch(4 + (crit_change ? 1 : 0) + (crit_trunc ? 1 : 0));
         }
         TF_CUDA(c, cudaGetLastError());
         TF_CUDA(c, cudaMemcpyAsync(hc, c->ctl, sizeof(double) * CT_SIZE, cudaMemcpyDeviceToHost, c->stream));
@@ -870,7 +881,10 @@ tf_status tf_advance_adaptive_device(tf_ctx* c, tf_adaptive* ctl, int n_accept, 
     }
     TF_CUDA(c, drain(attempts));
     ctl->dt = hc[CT_DT];
-    c->have_acc = false;
+    c->have_acc = crit_trunc && hc[CT_HAVE_ACC] != 0.0;                  // a_{n-1/2} of the last accepted step sits in c->acc
+    if (c->have_acc) c->dt_prev = hc[CT_DT_PREV];
+    if (crit_trunc) c->last_trunc = hc[CT_TRUNC];
+    if (crit_change) c->last_change = hc[CT_CHANGE];
     if (t_advanced) *t_advanced = hc[CT_T];
     if (nhist) *nhist = attempts;
     if (done == 2) return fail(c, TF_NOT_CONVERGED, "tf_advance_adaptive_device: dt fell below dt_min");

@@ -39,8 +39,8 @@ sum_check_kernel(size_t n, const double* __restrict__ h, double* __restrict__ pa
 
 // extra solution criterion of Fig. 1 (PAPER.md:252 Note 2): out[0] = max |u_new - u_old| / u_old over the field
 // (order-independent max on the bit patterns of non-negative doubles -> bitwise reproducible; NaN surfaces)
-__global__ void __launch_bounds__(RED_THREADS)
-max_rel_change_kernel(size_t n, const double* __restrict__ u_old, const double* __restrict__ u_new, double* __restrict__ out)
+__device__ __forceinline__ void
+max_rel_change_body(size_t n, const double* __restrict__ u_old, const double* __restrict__ u_new, double* __restrict__ out)
 {
     double acc = 0.0;
     for (size_t p = (size_t)blockIdx.x * RED_THREADS + threadIdx.x; p < n; p += (size_t)RED_BLOCKS * RED_THREADS) {
@@ -60,9 +60,15 @@ max_rel_change_kernel(size_t n, const double* __restrict__ u_old, const double* 
 // Writes a_{n+1/2} to a_new (committed by the host only if the step is accepted) and max |tau| / |u^{n+1}| to out.
 // have_prev == 0 (first step after tf_set_state): only a_new is written.
 __global__ void __launch_bounds__(RED_THREADS)
-truncation_kernel(size_t n, const double* __restrict__ u_old, const double* __restrict__ u_new, const double* __restrict__ bn,
-                  const double* __restrict__ a_prev, double* __restrict__ a_new, double two_over_dt2, double scale,
-                  int have_prev, double* __restrict__ out)
+max_rel_change_kernel(size_t n, const double* __restrict__ u_old, const double* __restrict__ u_new, double* __restrict__ out)
+{
+    max_rel_change_body(n, u_old, u_new, out);
+}
+
+__device__ __forceinline__ void
+truncation_body(size_t n, const double* __restrict__ u_old, const double* __restrict__ u_new, const double* __restrict__ bn,
+                const double* __restrict__ a_prev, double* __restrict__ a_new, double two_over_dt2, double scale,
+                int have_prev, double* __restrict__ out)
 {
     double acc = 0.0;
     for (size_t p = (size_t)blockIdx.x * RED_THREADS + threadIdx.x; p < n; p += (size_t)RED_BLOCKS * RED_THREADS) {
@@ -76,6 +82,39 @@ truncation_kernel(size_t n, const double* __restrict__ u_old, const double* __re
     }
     acc = warp_max_nonneg(acc);
     if ((threadIdx.x & 31) == 0) atomic_max_nonneg(out, acc);
+}
+
+__global__ void __launch_bounds__(RED_THREADS)
+truncation_kernel(size_t n, const double* __restrict__ u_old, const double* __restrict__ u_new, const double* __restrict__ bn,
+                  const double* __restrict__ a_prev, double* __restrict__ a_new, double two_over_dt2, double scale,
+                  int have_prev, double* __restrict__ out)
+{
+    truncation_body(n, u_old, u_new, bn, a_prev, a_new, two_over_dt2, scale, have_prev, out);
+}
+
+// The same two reductions for the on-device controller (tf_control.cuh): they run only if the attempt converged
+// (`conv`), and the truncation estimate takes dt, dt_prev and "a history exists" from device memory.  The scalars are
+// formed by the operations tf_step uses on the host, in its order, none of them contractible into an FMA: same bits.
+__global__ void __launch_bounds__(RED_THREADS)
+max_rel_change_ctl_kernel(size_t n, const double* __restrict__ u_old, const double* __restrict__ u_new,
+                          const double* __restrict__ conv, double* __restrict__ out)
+{
+    if (__ldcg(conv) == 0.0) return;
+    max_rel_change_body(n, u_old, u_new, out);
+}
+
+__global__ void __launch_bounds__(RED_THREADS)
+truncation_ctl_kernel(size_t n, const double* __restrict__ u_old, const double* __restrict__ u_new, const double* __restrict__ bn,
+                      const double* __restrict__ a_prev, double* __restrict__ a_new, const double* __restrict__ conv,
+                      const double* __restrict__ dt_p, const double* __restrict__ dt_prev_p, const double* __restrict__ have_p,
+                      double* __restrict__ out)
+{
+    if (__ldcg(conv) == 0.0) return;
+    const double dt = __ldcg(dt_p), dt_prev = __ldcg(dt_prev_p);
+    const int have = __ldcg(have_p) != 0.0 ? 1 : 0;
+    const double dt2 = __dmul_rn(dt, dt);
+    const double scale = have ? __ddiv_rn(__ddiv_rn(__dmul_rn(dt2, dt), 12.0), __dmul_rn(0.5, __dadd_rn(dt, dt_prev))) : 0.0;
+    truncation_body(n, u_old, u_new, bn, a_prev, a_new, __ddiv_rn(2.0, dt2), scale, have, out);
 }
 
 __global__ void __launch_bounds__(1024)

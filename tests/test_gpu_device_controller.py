@@ -122,8 +122,9 @@ def test_config2_on_device_equals_host(tf):
 
 
 # ------------------------------------------------------------------ the truncation-error criterion (PAPER.md:252 Note 2, R25)
-def test_truncation_criterion_against_the_oracle_transcription(tf, tfo):
-    """tf_set_truncation_criterion + tf_advance_adaptive against oracle/tfo.py's TruncationStepper under the same flow
+@pytest.mark.parametrize("on_device", [False, True])
+def test_truncation_criterion_against_the_oracle_transcription(tf, tfo, on_device):
+    """tf_set_truncation_criterion + tf_advance_adaptive (host controller / every decision on the device) against oracle/tfo.py's TruncationStepper under the same flow
     chart: same accept / REJECTED sequence, same time steps, same Newton counts, estimates equal to 1e-3, same film.
     The limit is taken from a first oracle run so that the growing step is rejected several times."""
     cfg = inputs.config(0)
@@ -151,7 +152,7 @@ def test_truncation_criterion_against_the_oracle_transcription(tf, tfo):
     g.set_newton(1e-14, 200, 0)
     g.set_truncation_criterion(limit)
     g.set_state(h)
-    t_g, dt_g, hist_g = tf.advance_adaptive(g, DT0, 12, **kw)
+    t_g, dt_g, hist_g = tf.advance_adaptive(g, DT0, 12, on_device=on_device, **kw)
     st = [x_[1] for x_ in hist_g]
     assert st == [x_[1] for x_ in hist_o] and st.count(tf.REJECTED) >= 2 and st[0] == tf.OK
     assert [x_[0] for x_ in hist_g] == [x_[0] for x_ in hist_o] and (t_g, dt_g) == (t_o, dt_o)
@@ -205,3 +206,53 @@ def test_device_controller_takes_more_attempts_than_its_record_ring_holds(tf):
     assert len(dev[2]) > 1100 and sum(1 for x in dev[2] if x[1] == tf.OK) == 1100      # it rejected on the way
     assert dev[0] == host[0] and dev[1] == host[1] and dev[2] == host[2]
     assert np.array_equal(dev[3], host[3])
+
+
+@pytest.mark.parametrize("criteria", ["change", "truncation", "both"])
+def test_device_controller_with_the_extra_criteria_equals_host_bit_for_bit(tf, criteria):
+    """Row f-4 joined: Fig. 1 on the device WITH the extra solution criteria of PAPER.md:252 Note 2.  The same run under
+    the host controller (tf_step decides each criterion on the host) and under tf_advance_adaptive_device (the
+    reductions are gated on "converged" and read dt, dt_prev from device memory): every record (dt, status, iterations,
+    residual), the time, the next dt and the film are identical bit for bit; the run contains TF_REJECTED attempts.
+    Afterwards one more tf_step on each context: the stored a_{n-1/2} and its dt carried over from the device run."""
+    cfg = inputs.config(0)
+    nx, ny = 96, 80
+    x = (np.arange(nx) + 0.5) / nx
+    y = (np.arange(ny) + 0.5) / ny
+    h = np.ascontiguousarray(1.0 + 0.2 * np.cos(2 * np.pi * x)[None, :] * np.cos(np.pi * y)[:, None])
+    DT0 = 0.05
+    kw = dict(grow=1.5, shrink=0.5, dt_max=1.0, dt_min=1e-9, grow_after=1)
+    # limits from a probe run on the host path: four equal steps, criteria switched on with limits that never reject
+    g = tf.ThinFilm(nx, ny, cfg["dx"], cfg["dy"], K, HS, 3, 2)
+    g.set_newton(1e-14, 200, 0)
+    g.set_truncation_criterion(1.0)
+    g.set_state(h)
+    for _ in range(4):
+        before = g.get_state()
+        assert g.step(DT0)[0] == tf.OK
+    lim_trunc = 2.0 * g.last_truncation_estimate()            # a step 1.5x longer (tau ~ dt^3) violates it
+    lim_change = 1.2 * float(np.max(np.abs(g.get_state() - before) / before))   # ... and so does its change of h
+    g.close()
+    assert lim_trunc > 1e-11 and lim_change > 0
+    outs = []
+    for on_device in (True, False):
+        g = tf.ThinFilm(nx, ny, cfg["dx"], cfg["dy"], K, HS, 3, 2)
+        g.set_newton(1e-14, 200, 0)
+        if criteria in ("change", "both"):
+            g.set_solution_criteria(lim_change)
+        if criteria in ("truncation", "both"):
+            g.set_truncation_criterion(lim_trunc)
+        g.set_state(h)
+        t, dt, hist = tf.advance_adaptive(g, DT0, 12, on_device=on_device, **kw)
+        after_run = g.get_state()
+        extra = g.step(dt)                                    # the next step of the schedule, decided by tf_step on the host
+        outs.append((t, dt, hist, after_run, extra, g.get_state(), g.last_truncation_estimate()))
+        g.close()
+    dev, host = outs
+    st = [r[1] for r in dev[2]]
+    assert st.count(tf.REJECTED) >= 2 and st.count(tf.OK) == 12 and st[0] == tf.OK
+    assert dev[0] == host[0] and dev[1] == host[1] and dev[2] == host[2]
+    assert np.array_equal(dev[3], host[3])
+    assert dev[4] == host[4] and np.array_equal(dev[5], host[5])
+    if criteria != "change":
+        assert dev[6] == host[6] and dev[6] > 0.0

@@ -263,7 +263,8 @@ def test_launch_ahead_is_exactly_the_per_iteration_decision(tf, nx, ny):
 
 
 # ------------------------------------------------------------------ Fig. 1 with an extra solution criterion (Note 2)
-def test_solution_criterion_and_native_controller_against_the_flow_chart(tf, tfo):
+@pytest.mark.parametrize("on_device", [False, True])
+def test_solution_criterion_and_native_controller_against_the_flow_chart(tf, tfo, on_device):
     """tf_set_solution_criteria + tf_advance_adaptive against the oracle's transcription of Fig. 1 with the same
     criterion (max relative change of h per step): same accept / reject sequence (including TF_REJECTED), same time
     steps, same fields.  The limit is set from the oracle so that the first attempts are rejected by the criterion."""
@@ -280,7 +281,8 @@ def test_solution_criterion_and_native_controller_against_the_flow_chart(tf, tfo
     g.set_solution_criteria(limit)
     stepper = tfo.CriteriaStepper(o, limit)
     t_o, dt_o, hist_o, failed = tfo.advance_adaptive(stepper, 1e-2, 12, grow=1.3, shrink=0.5, dt_max=0.05, dt_min=1e-9, grow_after=2)
-    t_g, dt_g, hist_g = tf.advance_adaptive(g, 1e-2, 12, grow=1.3, shrink=0.5, dt_max=0.05, dt_min=1e-9, grow_after=2)
+    t_g, dt_g, hist_g = tf.advance_adaptive(g, 1e-2, 12, grow=1.3, shrink=0.5, dt_max=0.05, dt_min=1e-9, grow_after=2,
+                                            on_device=on_device)
     assert not failed
     assert [x[1] for x in hist_g] == [x[1] for x in hist_o]
     assert tf.REJECTED in [x[1] for x in hist_g] and hist_g[0][1] == tf.REJECTED
