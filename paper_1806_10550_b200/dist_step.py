@@ -36,9 +36,12 @@ class TorchComm:
         self.dist, self.group = dist, group
         self.world, self.rank = dist.get_world_size(group), dist.get_rank(group)
 
-    def all_to_all(self, send, send_counts, recv_counts):
+    def all_to_all(self, send, send_counts, recv_counts, out=None):
+        """`out`: a preallocated receive buffer of at least sum(recv_counts) elements (Exchange keeps one per direction,
+        so the per-iteration exchanges allocate nothing); None: a fresh tensor"""
         import torch
-        recv = torch.empty(int(sum(recv_counts)), dtype=send.dtype, device=send.device)
+        total = int(sum(recv_counts))
+        recv = out[:total] if out is not None else torch.empty(total, dtype=send.dtype, device=send.device)
         self.dist.all_to_all_single(recv, send, list(map(int, recv_counts)), list(map(int, send_counts)), group=self.group)
         return recv
 
@@ -98,6 +101,7 @@ class Exchange:
             self.rc_rcount.append(cnt)
             off += cnt
         self.rc_recv_rects = tf.make_rects(blocks)
+        self.rc_recv = torch.empty(max(off, 1), dtype=torch.float64, device=device)
         self.rc_self = (0, a, j0, loc, nyl, b - a)      # src row0, col0 -> dst row0, col0, rows, cols
         self.refl_left = (r == 0)                      # h_{-1} = h_0, h_{-2} = h_1
         self.refl_right_at = n + 2 if r == lay.world - 1 else -1
@@ -118,6 +122,7 @@ class Exchange:
             self.cr_rcount.append(cnt)
             off += cnt
         self.cr_recv_rects = tf.make_rects(blocks)
+        self.cr_recv = torch.empty(max(off, 1), dtype=torch.float64, device=device)
         self.cr_self = (j0, lay.HALO, 0, i0, nyl, n)
 
     def rows_to_cols(self, comm, f_rows, f_cols):
@@ -126,7 +131,7 @@ class Exchange:
         self.tf.block_copy(f_rows, sr, sc, f_cols, dr, dc, nr, nc, self.refl_left, self.refl_right_at)
         if self.lay.world > 1:
             self.tf.blocks_gather(f_rows, self.rc_send_rects, self.rc_send)
-            recv = comm.all_to_all(self.rc_send, self.rc_scount, self.rc_rcount)
+            recv = comm.all_to_all(self.rc_send, self.rc_scount, self.rc_rcount, out=self.rc_recv)
             self.tf.blocks_scatter(recv, self.rc_recv_rects, f_cols, self.refl_left, self.refl_right_at)
 
     def cols_to_rows(self, comm, f_cols, f_rows):
@@ -135,7 +140,7 @@ class Exchange:
         self.tf.block_copy(f_cols, sr, sc, f_rows, dr, dc, nr, nc)
         if self.lay.world > 1:
             self.tf.blocks_gather(f_cols, self.cr_send_rects, self.cr_send)
-            recv = comm.all_to_all(self.cr_send, self.cr_scount, self.cr_rcount)
+            recv = comm.all_to_all(self.cr_send, self.cr_scount, self.cr_rcount, out=self.cr_recv)
             self.tf.blocks_scatter(recv, self.cr_recv_rects, f_rows)
 
 
@@ -176,7 +181,9 @@ class DistributedFilm:
 
     def step(self, dt, batch=None):
         """returns (status, newton_iters, residual) like ThinFilm.step; on rejection the state is unchanged.
-        Iterations are enqueued `batch` at a time (the first batch as long as the previous accepted step's count) and
+        Iterations are enqueued `batch` at a time (the first batch one shorter than the previous accepted step's count:
+        an iteration enqueued past the deciding one still moves the whole field twice over the interconnect, so the
+        speculation stops just short of where the last step ended and goes on two at a time) and
         the host reads the records of a batch at once: the sweeps of iteration k are gated on the ALL-REDUCED record
         of iteration k-1, which is written into both contexts, so iterations past the deciding one do nothing on any
         rank (their redistributions move unchanged data) -- the scheme of tf_set_launch_ahead across ranks."""
@@ -184,7 +191,7 @@ class DistributedFilm:
         tf, cx, cy = self.tf, self.ctx_x, self.ctx_y
         rx, ry = cx.field(cx.FIELD_RECORDS), cy.field(cy.FIELD_RECORDS)
         gate = cx.SWEEP_GATED
-        batch = max(1, int(batch if batch is not None else self.last_iters))
+        batch = max(1, int(batch if batch is not None else self.last_iters - 1))
         k = done = 0
         res, status, decided = 0.0, tf.NOT_CONVERGED, False
         while not decided and done < self.max_iter:

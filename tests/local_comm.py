@@ -15,7 +15,7 @@ class LocalComm:
     def __init__(self, shared, rank):
         self.s, self.rank, self.world = shared, rank, shared.world
 
-    def all_to_all(self, send, send_counts, recv_counts):
+    def all_to_all(self, send, send_counts, recv_counts, out=None):
         if send.is_cuda:
             torch.cuda.synchronize()
         self.s.box[self.rank] = (send, list(map(int, send_counts)))
@@ -27,6 +27,9 @@ class LocalComm:
             assert counts[self.rank] == int(recv_counts[p]), "split sizes of sender and receiver disagree"
             pieces.append(buf[off:off + counts[self.rank]])
         recv = torch.cat(pieces).clone()
+        if out is not None:                                   # the caller's preallocated receive buffer, as TorchComm fills it
+            out[:recv.numel()].copy_(recv)
+            recv = out[:recv.numel()]
         if recv.is_cuda:
             torch.cuda.synchronize()
         self.s.barrier.wait()
