@@ -19,7 +19,9 @@
  * order, G(u)=0 at convergence, fixed point, transpose symmetry.
  * The NLC (1.8)-(1.9) and polymer (1.12) disjoining pressures are pinned by finite
  * differences of Pi(h) as the paper defines it, the finite-difference Jacobian, G(u) = 0 and the dispersion
- * relation (tests/test_oracle_models.py).  Parity unpinned: nothing in this file.
+ * relation (tests/test_oracle_models.py).  The order of the two sweeps in tfo_step ((2.19) before (2.20)) and the two
+ * lines of reading R18 (a finite, non-positive iterate ends the step; a NaN ratio surfaces in the residual) are pinned
+ * by O12 / O13 of tests/test_oracle_pins.py.  Parity unpinned: nothing in this file.
  *
  * The optional "#pragma omp parallel for" lines are no-ops unless compiled with
  * -fopenmp (second build, used only for the all-core timed baseline).
